@@ -1,0 +1,444 @@
+/*
+ * gm_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, fp64 CPU statement of what the short-range force pipeline of GALAMOST-style
+ * coarse-grained polymer MD computes (arXiv 1310.2041, "PAPER.md").  It shares no code, header,
+ * table or constant generator with the CUDA path under paper_1310_2041_b200/, and neither side
+ * imports the other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.
+ *
+ * Nature of the result: cell list, Verlet list, skin and SFC order are exact
+ * accelerations -- they never change the mathematical result -- so for neighbor sets and forces this
+ * file is the plain definition (all-pairs O(N^2); an independent cell-list O(N) mode exists only so
+ * that large systems finish, and is checked against the O(N^2) mode), and for trajectories it is the
+ * integrator written out step by step.
+ *
+ * What follows the paper, and what the paper leaves to a stated reading:
+ *   - neighbor set within r_cut + r_buffer, full list
+ *   - minimum image in a cuboid periodic box                      PAPER.md:L133, Alg. 2 line 6 (L458)
+ *   - Lennard-Jones, Eq. (1)
+ *   - harmonic bond U = k (r - r0)^2, Eq. (7) (no 1/2)
+ *   - bonds act from both ends, no exclusions
+ *   - velocity-Verlet NVE / "BD" (Langevin) / GW-VV for DPD
+ *   - FENE, WCA, the DPD force law, Philox: not in PAPER.md; readings c-3..c-8:
+ *     Kremer-Grest FENE, Groot-Warren DPD with uniform unit-variance noise, Philox4x32-10
+ *     (Salmon et al., SC'11) keyed (seed; min tag, max tag, step, stream).
+ *
+ * Pins (tests/test_oracle_pins.py, -m "not gpu"): closed forms of Eq. (1) and FENE+WCA, force =
+ * -grad(energy) by central differences, O(N^2) vs cell mode, Newton's third law / zero net force,
+ * translation / image / permutation invariance, NVE conservation ~ dt^2 and time reversal, harmonic
+ * dimer frequency (omega = 2 sqrt(k) under Eq. (7)), free flight, Philox known answers, thermostat
+ * temperatures.  Unpinned: equilibrium <Rg^2> of the melts in absolute terms ("parity unpinned";
+ * compared GPU-vs-oracle only).
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+enum { ORC_PAIR_NONE = 0, ORC_PAIR_LJ = 1, ORC_PAIR_DPD = 2 };
+enum { ORC_BOND_NONE = 0, ORC_BOND_FENE = 1, ORC_BOND_HARMONIC = 2 };
+enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2 };
+enum { ORC_OK = 0, ORC_ERR_BOND_OVERSTRETCH = -7, ORC_ERR_ARG = -1 };
+
+typedef struct {
+    int64_t n;              /* beads */
+    int32_t n_types;
+    int32_t pair_style;
+    int32_t bond_style;
+    int32_t integrator;
+    double box[3];          /* origin-centred cuboid: x in [-L/2, L/2) */
+    double dt, kT, gamma, lambda;
+    uint64_t seed;
+    const double *eps;      /* [n_types^2]  LJ epsilon | DPD a           */
+    const double *sigma;    /* [n_types^2]  LJ sigma   | unused          */
+    const double *rc;       /* [n_types^2]  cutoff                        */
+    const double *ushift;   /* [n_types^2]  LJ energy shift (0 = plain cut) */
+    int64_t n_bonds;
+    const int32_t *bond_i, *bond_j, *bond_type;
+    const double *bond_k, *bond_r0;     /* per bond type; FENE: r0 is R0 */
+    const int32_t *type;    /* [n] */
+    const double *mass;     /* [n] */
+    int32_t use_cells;      /* 0: all pairs O(N^2) (the definition); 1: cell-list O(N) */
+    int32_t n_threads;      /* OpenMP threads for the per-bead loops; <=0: library default */
+} orc_params;
+
+/* ------------------------------------------------------------------------------------------ */
+/* O6. Philox4x32-10 exactly as published (Salmon, Moraes, Dror, Shaw, SC'11).                  */
+void orc_philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t out[4])
+{
+    const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;      /* multipliers */
+    const uint32_t W0 = 0x9E3779B9u, W1 = 0xBB67AE85u;      /* Weyl key increments */
+    uint32_t c0 = ctr_in[0], c1 = ctr_in[1], c2 = ctr_in[2], c3 = ctr_in[3];
+    uint32_t k0 = key_in[0], k1 = key_in[1];
+    for (int round = 0; round < 10; ++round) {
+        if (round > 0) { k0 += W0; k1 += W1; }
+        uint64_t p0 = (uint64_t)M0 * c0;
+        uint64_t p1 = (uint64_t)M1 * c2;
+        uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+        uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+        uint32_t n0 = hi1 ^ c1 ^ k0;
+        uint32_t n1 = lo1;
+        uint32_t n2 = hi0 ^ c3 ^ k1;
+        uint32_t n3 = lo0;
+        c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+/* Uniform in (0,1) from the top 24 bits of a word, u = (k + 1/2) 2^-24.  The method only uses the
+   symmetric variate 2u - 1 = (2k + 1 - 2^24) 2^-24, which is exact in fp32 as well as fp64. */
+double orc_u24(uint32_t x) { return ((double)(x >> 8) + 0.5) * (1.0 / 16777216.0); }
+
+/* counter = (A, B, step low 32, stream); key = (seed low 32, seed high 32) */
+static void noise_words(uint64_t seed, uint32_t a, uint32_t b, uint64_t step, uint32_t stream, uint32_t out[4])
+{
+    uint32_t ctr[4] = { a, b, (uint32_t)(step & 0xFFFFFFFFu), stream };
+    uint32_t key[2] = { (uint32_t)(seed & 0xFFFFFFFFu), (uint32_t)(seed >> 32) };
+    orc_philox4x32_10(ctr, key, out);
+}
+
+/* DPD pair noise theta_ij = theta_ji: uniform, zero mean, unit variance (reading c-4). */
+double orc_pair_theta(uint64_t seed, uint64_t step, int64_t tag_i, int64_t tag_j)
+{
+    uint32_t lo = (uint32_t)(tag_i < tag_j ? tag_i : tag_j);
+    uint32_t hi = (uint32_t)(tag_i < tag_j ? tag_j : tag_i);
+    uint32_t w[4];
+    noise_words(seed, lo, hi, step, 0u, w);
+    return sqrt(3.0) * (2.0 * orc_u24(w[0]) - 1.0);
+}
+
+/* Langevin per-bead noise xi in (-1,1)^3, variance 1/3 per component. */
+void orc_bead_xi(uint64_t seed, uint64_t step, int64_t tag, double xi[3])
+{
+    uint32_t w[4];
+    noise_words(seed, (uint32_t)tag, 0u, step, 1u, w);
+    xi[0] = 2.0 * orc_u24(w[0]) - 1.0;
+    xi[1] = 2.0 * orc_u24(w[1]) - 1.0;
+    xi[2] = 2.0 * orc_u24(w[2]) - 1.0;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O1. Geometry.                                                                                */
+double orc_min_image(double d, double L) { return d - L * nearbyint(d / L); }
+
+static double wrap1(double x, double L)
+{
+    /* one conditional add/subtract per component: a step never moves a bead by a box length */
+    if (x >= 0.5 * L) x -= L;
+    else if (x < -0.5 * L) x += L;
+    return x;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* The oracle's own cell list (used only when use_cells = 1): n_d = floor(L_d / r), w_d = L_d / n_d. */
+typedef struct {
+    int nc[3];
+    int64_t *start;     /* [ncells+1] */
+    int64_t *item;      /* [n] bead ids grouped by cell */
+    int ok;             /* 0: fewer than 3 cells in some dimension -> caller must use all pairs */
+} orc_cells;
+
+static int cell_coord(double x, double L, int nc)
+{
+    double u = (x + 0.5 * L) / L;
+    u -= floor(u);                          /* beads given outside the box land in their image's cell */
+    int c = (int)floor(u * nc);
+    if (c < 0) c = 0;
+    if (c >= nc) c = nc - 1;
+    return c;
+}
+
+static void cells_build(orc_cells *cl, int64_t n, const double *pos, const double box[3], double r)
+{
+    cl->ok = 1;
+    for (int d = 0; d < 3; ++d) {
+        cl->nc[d] = (int)floor(box[d] / r);
+        if (cl->nc[d] < 3) cl->ok = 0;
+    }
+    cl->start = NULL; cl->item = NULL;
+    if (!cl->ok) return;
+    int64_t ncells = (int64_t)cl->nc[0] * cl->nc[1] * cl->nc[2];
+    cl->start = (int64_t *)calloc((size_t)ncells + 1, sizeof(int64_t));
+    cl->item = (int64_t *)malloc((size_t)(n > 0 ? n : 1) * sizeof(int64_t));
+    int64_t *cid = (int64_t *)malloc((size_t)(n > 0 ? n : 1) * sizeof(int64_t));
+    for (int64_t i = 0; i < n; ++i) {
+        int cx = cell_coord(pos[3 * i + 0], box[0], cl->nc[0]);
+        int cy = cell_coord(pos[3 * i + 1], box[1], cl->nc[1]);
+        int cz = cell_coord(pos[3 * i + 2], box[2], cl->nc[2]);
+        cid[i] = ((int64_t)cz * cl->nc[1] + cy) * cl->nc[0] + cx;
+        cl->start[cid[i] + 1] += 1;
+    }
+    for (int64_t c = 0; c < ncells; ++c) cl->start[c + 1] += cl->start[c];
+    int64_t *fill = (int64_t *)calloc((size_t)ncells, sizeof(int64_t));
+    for (int64_t i = 0; i < n; ++i) {
+        int64_t c = cid[i];
+        cl->item[cl->start[c] + fill[c]] = i;
+        fill[c] += 1;
+    }
+    free(fill); free(cid);
+}
+
+static void cells_free(orc_cells *cl) { free(cl->start); free(cl->item); }
+
+/* ------------------------------------------------------------------------------------------ */
+/* O2. Neighbor set S = {(i,j), i<j : |minimg(r_i - r_j)|^2 < r_list^2}.        */
+/* Returns the number of pairs; writes at most cap of them as (i,j) with i<j.                   */
+int64_t orc_neighbor_pairs(int64_t n, const double *pos, const double box[3], double r_list,
+                           int32_t use_cells, int64_t cap, int32_t *pairs)
+{
+    const double r2l = r_list * r_list;
+    int64_t cnt = 0;
+    orc_cells cl; cl.ok = 0; cl.start = NULL; cl.item = NULL;
+    if (use_cells) cells_build(&cl, n, pos, box, r_list);
+    if (!use_cells || !cl.ok) {
+        for (int64_t i = 0; i < n; ++i)
+            for (int64_t j = i + 1; j < n; ++j) {
+                double dx = orc_min_image(pos[3 * i + 0] - pos[3 * j + 0], box[0]);
+                double dy = orc_min_image(pos[3 * i + 1] - pos[3 * j + 1], box[1]);
+                double dz = orc_min_image(pos[3 * i + 2] - pos[3 * j + 2], box[2]);
+                if (dx * dx + dy * dy + dz * dz < r2l) {
+                    if (cnt < cap) { pairs[2 * cnt] = (int32_t)i; pairs[2 * cnt + 1] = (int32_t)j; }
+                    ++cnt;
+                }
+            }
+        if (use_cells) cells_free(&cl);
+        return cnt;
+    }
+    for (int64_t i = 0; i < n; ++i) {
+        int cx = cell_coord(pos[3 * i + 0], box[0], cl.nc[0]);
+        int cy = cell_coord(pos[3 * i + 1], box[1], cl.nc[1]);
+        int cz = cell_coord(pos[3 * i + 2], box[2], cl.nc[2]);
+        for (int oz = -1; oz <= 1; ++oz) for (int oy = -1; oy <= 1; ++oy) for (int ox = -1; ox <= 1; ++ox) {
+            int ax = (cx + ox + cl.nc[0]) % cl.nc[0];
+            int ay = (cy + oy + cl.nc[1]) % cl.nc[1];
+            int az = (cz + oz + cl.nc[2]) % cl.nc[2];
+            int64_t c = ((int64_t)az * cl.nc[1] + ay) * cl.nc[0] + ax;
+            for (int64_t s = cl.start[c]; s < cl.start[c + 1]; ++s) {
+                int64_t j = cl.item[s];
+                if (j <= i) continue;
+                double dx = orc_min_image(pos[3 * i + 0] - pos[3 * j + 0], box[0]);
+                double dy = orc_min_image(pos[3 * i + 1] - pos[3 * j + 1], box[1]);
+                double dz = orc_min_image(pos[3 * i + 2] - pos[3 * j + 2], box[2]);
+                if (dx * dx + dy * dy + dz * dz < r2l) {
+                    if (cnt < cap) { pairs[2 * cnt] = (int32_t)i; pairs[2 * cnt + 1] = (int32_t)j; }
+                    ++cnt;
+                }
+            }
+        }
+    }
+    cells_free(&cl);
+    return cnt;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+/* O3 + O5. Contribution of bead j to the force on bead i.                                      */
+/* vel is the velocity the DPD dissipative term sees (v-tilde in GW-VV); unused for LJ.         */
+/* Adds to f[3]; adds the FULL pair energy to *u (the caller halves the double count).          */
+/* Returns 1 if the pair is inside its cutoff.                                                  */
+static int pair_term(const orc_params *p, const double *pos, const double *vel, uint64_t step,
+                     int64_t i, int64_t j, double f[3], double *u)
+{
+    double dx = orc_min_image(pos[3 * i + 0] - pos[3 * j + 0], p->box[0]);
+    double dy = orc_min_image(pos[3 * i + 1] - pos[3 * j + 1], p->box[1]);
+    double dz = orc_min_image(pos[3 * i + 2] - pos[3 * j + 2], p->box[2]);
+    double r2 = dx * dx + dy * dy + dz * dz;
+    int t = p->type[i] * p->n_types + p->type[j];
+    double rc = p->rc[t];
+    if (!(r2 < rc * rc)) return 0;
+    if (p->pair_style == ORC_PAIR_LJ) {
+        /* Eq. (1): U = 4 eps [(s/r)^12 - (s/r)^6];  F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij */
+        double eps = p->eps[t], sig = p->sigma[t];
+        double s2 = sig * sig / r2;
+        double s6 = s2 * s2 * s2;
+        double s12 = s6 * s6;
+        double fs = 24.0 * eps / r2 * (2.0 * s12 - s6);
+        f[0] += fs * dx; f[1] += fs * dy; f[2] += fs * dz;
+        *u += 4.0 * eps * (s12 - s6) - p->ushift[t];
+        return 1;
+    }
+    if (p->pair_style == ORC_PAIR_DPD) {
+        /* Groot-Warren (reading c-3): F_ij = [a w - gamma w^2 (e.v_ij) + sigma_R w theta / sqrt(dt)] e */
+        if (r2 < 1e-12) return 1;   /* e undefined */
+        double r = sqrt(r2);
+        double w = 1.0 - r / rc;
+        double ex = dx / r, ey = dy / r, ez = dz / r;
+        double dvx = vel[3 * i + 0] - vel[3 * j + 0];
+        double dvy = vel[3 * i + 1] - vel[3 * j + 1];
+        double dvz = vel[3 * i + 2] - vel[3 * j + 2];
+        double edv = ex * dvx + ey * dvy + ez * dvz;
+        double sigma_r = sqrt(2.0 * p->gamma * p->kT);
+        double theta = orc_pair_theta(p->seed, step, i, j);
+        double a = p->eps[t];
+        double fs = a * w - p->gamma * w * w * edv + sigma_r * w * theta / sqrt(p->dt);
+        f[0] += fs * ex; f[1] += fs * ey; f[2] += fs * ez;
+        *u += 0.5 * a * rc * w * w;
+        return 1;
+    }
+    return 0;
+}
+
+static double max_cutoff(const orc_params *p)
+{
+    double r = 0.0;
+    for (int t = 0; t < p->n_types * p->n_types; ++t) if (p->rc[t] > r) r = p->rc[t];
+    return r;
+}
+
+/* O3-O5. Conservative (+ DPD dissipative/random) forces at positions pos.                      */
+/* out[0] = pair energy, out[1] = bond energy, out[2] = number of unique pairs inside r_c.      */
+int orc_pair_bond_forces(const orc_params *p, const double *pos, const double *vel, uint64_t step,
+                         double *frc, double out[3])
+{
+    const int64_t n = p->n;
+    double pe_pair = 0.0, n_in = 0.0;
+    orc_cells cl; cl.ok = 0; cl.start = NULL; cl.item = NULL;
+    int have_pairs = (p->pair_style != ORC_PAIR_NONE);
+    if (have_pairs && p->use_cells) cells_build(&cl, n, pos, p->box, max_cutoff(p));
+#ifdef _OPENMP
+    if (p->n_threads > 0) omp_set_num_threads(p->n_threads);
+#endif
+    if (!have_pairs) {
+        memset(frc, 0, (size_t)(3 * n) * sizeof(double));
+    } else if (!p->use_cells || !cl.ok) {
+#pragma omp parallel for schedule(static) reduction(+ : pe_pair, n_in)
+        for (int64_t i = 0; i < n; ++i) {
+            double f[3] = { 0, 0, 0 }, u = 0.0;
+            for (int64_t j = 0; j < n; ++j) {
+                if (j == i) continue;
+                n_in += pair_term(p, pos, vel, step, i, j, f, &u);
+            }
+            frc[3 * i] = f[0]; frc[3 * i + 1] = f[1]; frc[3 * i + 2] = f[2];
+            pe_pair += 0.5 * u;
+        }
+    } else {
+#pragma omp parallel for schedule(static) reduction(+ : pe_pair, n_in)
+        for (int64_t i = 0; i < n; ++i) {
+            double f[3] = { 0, 0, 0 }, u = 0.0;
+            int cx = cell_coord(pos[3 * i + 0], p->box[0], cl.nc[0]);
+            int cy = cell_coord(pos[3 * i + 1], p->box[1], cl.nc[1]);
+            int cz = cell_coord(pos[3 * i + 2], p->box[2], cl.nc[2]);
+            for (int oz = -1; oz <= 1; ++oz) for (int oy = -1; oy <= 1; ++oy) for (int ox = -1; ox <= 1; ++ox) {
+                int ax = (cx + ox + cl.nc[0]) % cl.nc[0];
+                int ay = (cy + oy + cl.nc[1]) % cl.nc[1];
+                int az = (cz + oz + cl.nc[2]) % cl.nc[2];
+                int64_t c = ((int64_t)az * cl.nc[1] + ay) * cl.nc[0] + ax;
+                for (int64_t s = cl.start[c]; s < cl.start[c + 1]; ++s) {
+                    int64_t j = cl.item[s];
+                    if (j == i) continue;
+                    n_in += pair_term(p, pos, vel, step, i, j, f, &u);
+                }
+            }
+            frc[3 * i] = f[0]; frc[3 * i + 1] = f[1]; frc[3 * i + 2] = f[2];
+            pe_pair += 0.5 * u;
+        }
+    }
+    if (have_pairs && p->use_cells) cells_free(&cl);
+
+    /* O4. Bonds: each bond (i,j) once, acting on both ends (the GPU evaluates it from both ends,
+       PAPER.md:L97; the sum is the same). */
+    double pe_bond = 0.0;
+    int status = ORC_OK;
+    if (p->bond_style != ORC_BOND_NONE) {
+        for (int64_t b = 0; b < p->n_bonds; ++b) {
+            int64_t i = p->bond_i[b], j = p->bond_j[b];
+            double k = p->bond_k[p->bond_type[b]], r0 = p->bond_r0[p->bond_type[b]];
+            double dx = orc_min_image(pos[3 * i + 0] - pos[3 * j + 0], p->box[0]);
+            double dy = orc_min_image(pos[3 * i + 1] - pos[3 * j + 1], p->box[1]);
+            double dz = orc_min_image(pos[3 * i + 2] - pos[3 * j + 2], p->box[2]);
+            double r2 = dx * dx + dy * dy + dz * dz;
+            double fs;
+            if (p->bond_style == ORC_BOND_FENE) {
+                /* U = -1/2 k R0^2 ln(1 - r^2/R0^2);  F_i = -k r_ij / (1 - r^2/R0^2)   (reading c-8) */
+                double q = 1.0 - r2 / (r0 * r0);
+                if (!(q > 0.0)) { status = ORC_ERR_BOND_OVERSTRETCH; continue; }
+                fs = -k / q;
+                pe_bond += -0.5 * k * r0 * r0 * log(q);
+            } else {
+                /* Eq. (7): U = k (r - r0)^2;  F_i = -2 k (1 - r0/r) r_ij */
+                double r = sqrt(r2);
+                if (r0 == 0.0) fs = -2.0 * k;
+                else fs = (r > 0.0) ? -2.0 * k * (1.0 - r0 / r) : 0.0;
+                pe_bond += k * (r - r0) * (r - r0);
+            }
+            frc[3 * i] += fs * dx; frc[3 * i + 1] += fs * dy; frc[3 * i + 2] += fs * dz;
+            frc[3 * j] -= fs * dx; frc[3 * j + 1] -= fs * dy; frc[3 * j + 2] -= fs * dz;
+        }
+    }
+    if (out) { out[0] = pe_pair; out[1] = pe_bond; out[2] = 0.5 * n_in; }
+    return status;
+}
+
+/* The force the integrator uses at time level `step` (O7):
+ *   NVE, GW-VV : F(pos [, vel])
+ *   Langevin   : F_c(pos) - gamma m v + sqrt(6 gamma m kT / dt) xi(tag, step)   (reading c-7)
+ * vel is v (initial call), v' (Langevin half-step velocity) or v-tilde (GW-VV).              */
+int orc_compute_forces(const orc_params *p, const double *pos, const double *vel, uint64_t step,
+                       double *frc, double out[3])
+{
+    int status = orc_pair_bond_forces(p, pos, vel, step, frc, out);
+    if (p->integrator == ORC_LANGEVIN) {
+        for (int64_t i = 0; i < p->n; ++i) {
+            double xi[3], m = p->mass[i];
+            orc_bead_xi(p->seed, step, i, xi);
+            double amp = sqrt(6.0 * p->gamma * m * p->kT / p->dt);
+            for (int d = 0; d < 3; ++d)
+                frc[3 * i + d] += -p->gamma * m * vel[3 * i + d] + amp * xi[d];
+        }
+    }
+    return status;
+}
+
+/* O7. n_steps of the integrator, starting at time level step0 with frc = orc_compute_forces(step0). */
+/* scratch: 6n doubles (GW-VV: v-tilde and the old acceleration).                                  */
+int orc_run(const orc_params *p, double *pos, double *vel, double *frc, uint64_t step0, int64_t n_steps,
+            double *scratch)
+{
+    const int64_t n = p->n;
+    const double dt = p->dt;
+    int status = ORC_OK;
+    for (int64_t s = 0; s < n_steps; ++s) {
+        uint64_t step = step0 + (uint64_t)s + 1;    /* time level of the new force */
+        if (p->integrator == ORC_NVE || p->integrator == ORC_LANGEVIN) {
+            /* v' = v + dt/2 a;  r = r + dt v';  wrap;  a = F(r)/m;  v = v' + dt/2 a */
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d) {
+                    vel[3 * i + d] += 0.5 * dt * frc[3 * i + d] / p->mass[i];
+                    pos[3 * i + d] = wrap1(pos[3 * i + d] + dt * vel[3 * i + d], p->box[d]);
+                }
+            int st = orc_compute_forces(p, pos, vel, step, frc, NULL);   /* Langevin drag sees v' */
+            if (st != ORC_OK) status = st;
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d)
+                    vel[3 * i + d] += 0.5 * dt * frc[3 * i + d] / p->mass[i];
+        } else {
+            /* GW-VV: r += dt v + dt^2/2 f;  v~ = v + lambda dt f;  f' = F(r, v~);  v += dt/2 (f + f') */
+            double *vt = scratch, *f_old = scratch + 3 * n;
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d) {
+                    double f = frc[3 * i + d] / p->mass[i];
+                    pos[3 * i + d] = wrap1(pos[3 * i + d] + dt * vel[3 * i + d] + 0.5 * dt * dt * f, p->box[d]);
+                    vt[3 * i + d] = vel[3 * i + d] + p->lambda * dt * f;
+                    f_old[3 * i + d] = f;
+                }
+            int st = orc_compute_forces(p, pos, vt, step, frc, NULL);
+            if (st != ORC_OK) status = st;
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d)
+                    vel[3 * i + d] += 0.5 * dt * (f_old[3 * i + d] + frc[3 * i + d] / p->mass[i]);
+        }
+    }
+    return status;
+}
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}

@@ -1,0 +1,39 @@
+"""Small helpers shared by the tests (no arithmetic of the method)."""
+from __future__ import annotations
+
+import numpy as np
+
+from workloads import Workload
+
+
+def custom(pos, box, vel=None, typ=None, bonds=None, pair_style="lj", eps=1.0, sigma=1.0, rc=2.5,
+           shift=True, a=25.0, bond_style="none", k=30.0, r0=1.5, integrator="nve", dt=0.005,
+           kT=1.0, gamma=0.0, lam=0.65, r_skin=0.4, seed=7, n_types=1, mass=None) -> Workload:
+    pos = np.asarray(pos, dtype=np.float32).reshape(-1, 3)
+    n = pos.shape[0]
+    box = np.asarray(box, dtype=np.float32).reshape(-1)
+    if box.size == 1:
+        box = np.repeat(box, 3)
+    vel = np.zeros((n, 3), np.float32) if vel is None else np.asarray(vel, np.float32).reshape(n, 3)
+    typ = np.zeros(n, np.int32) if typ is None else np.asarray(typ, np.int32)
+    bonds = np.zeros((0, 2), np.int32) if bonds is None else np.asarray(bonds, np.int32).reshape(-1, 2)
+    mass = np.ones(n, np.float32) if mass is None else np.asarray(mass, np.float32)
+
+    def mat(x):
+        x = np.asarray(x, np.float32)
+        return np.broadcast_to(x, (n_types, n_types)).copy() if x.ndim == 0 else x.reshape(n_types, n_types).copy()
+
+    if pair_style == "dpd":
+        pair = dict(a=mat(a), rc=mat(rc))
+    else:
+        pair = dict(eps=mat(eps), sigma=mat(sigma), rc=mat(rc), shift=shift)
+    return Workload(
+        name="custom", box=box, pos=pos, vel=vel, type=typ, mass=mass, bonds=bonds,
+        bond_type=np.zeros(len(bonds), np.int32), n_types=n_types, pair_style=pair_style, pair=pair,
+        bond_style=bond_style, bond=dict(k=np.array([k], np.float32), r0=np.array([r0], np.float32)),
+        integrator=integrator, dt=dt, kT=kT, gamma=gamma, lam=lam, r_skin=r_skin, seed=seed,
+    )
+
+
+def pairs_to_set(pairs) -> set:
+    return set(map(tuple, np.asarray(pairs).tolist()))
