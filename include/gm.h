@@ -1,0 +1,179 @@
+/*
+ * gm.h -- C ABI of libgm: the per-timestep short-range force pipeline of GALAMOST-style
+ * coarse-grained polymer MD (arXiv 1310.2041, "PAPER.md") on one NVIDIA B200 (sm_100a), fp32.
+ *
+ * The pipeline:
+ *   a1 cell binning by counting sort         PAPER.md:L57 (cell list CL/CN), Alg. 1 Kernel 1 L376-388
+ *   a2 periodic space-filling-curve reorder  PAPER.md:L33, L199 (SFCPACK memory sort)
+ *   a3 skin-padded FULL Verlet list NL/NN    PAPER.md:L51 (table form NL[k*Np+i]), L57 (27 cells,
+ *                                            r_cut + r_buffer)
+ *   a4 rebuild when a bead moved > skin/2
+ *   a5 Lennard-Jones / WCA pair force        PAPER.md:L59-61 Eq. (1); loop shape Alg. 2
+ *   a6 DPD pair force (Groot-Warren)         PAPER.md:L43, L135, L197 (law itself: ref. 24; DESIGN.md c-3)
+ *   a7 bond force from the BL/BN table       PAPER.md:L97, Eq. (7) L99-101 (harmonic); FENE: DESIGN.md c-8
+ *   a8 velocity-Verlet NVE / Langevin "BD" / GW-VV
+ *   a9 energies (validation quantities)
+ *
+ * Conventions common to every call
+ *   - Every function returns a gm_status (0 = GM_OK, < 0 = error) and never throws, exits or
+ *     prints.  gm_last_error() gives a message for the last failing call on that system.
+ *   - "host or device": each array argument says which; calls taking `on_device` accept either
+ *     (on_device = 0: plain host memory, pinned or not; 1: device memory on the system's GPU).
+ *   - Ownership: the caller owns every buffer it passes, including the device workspace and the
+ *     CUDA stream.  The library copies inputs in, writes outputs out, and never frees or keeps a
+ *     caller pointer other than the workspace and the stream (which must outlive the system).
+ *   - All particle arrays cross this boundary in TAG order (the order given to gm_set_particles),
+ *     whatever the internal space-filling-curve storage order is.
+ *   - The box is an origin-centred cuboid, x_d in [-box_d/2, box_d/2), periodic in all three
+ *     dimensions.  Units are reduced (sigma, epsilon, m).
+ *   - Work is enqueued on the stream given at creation; calls that return data to the host
+ *     (on_device = 0 outputs, gm_energies, gm_get_stats) synchronise that stream before returning.
+ *   - Device-side conditions (neighbor-row overflow, FENE over-stretch, non-finite coordinates) are
+ *     latched in a device word and reported by the next synchronising call.
+ */
+#ifndef GM_H
+#define GM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gm_system gm_system; /* opaque; owns only small host state + CUDA graphs */
+typedef int gm_status;
+
+enum {
+    GM_OK = 0,
+    GM_ERR_INVALID_ARG = -1,
+    GM_ERR_STATE = -2,               /* call order: e.g. gm_step before gm_set_particles          */
+    GM_ERR_CUDA = -3,                /* a CUDA runtime call failed; message has the CUDA string   */
+    GM_ERR_WORKSPACE_TOO_SMALL = -4,
+    GM_ERR_BOX_TOO_SMALL = -5,       /* box_d < 3 (r_cut_max + r_skin) in some dimension (27-cell search) */
+    GM_ERR_NEIGHBOR_OVERFLOW = -6,   /* a bead has more neighbors than nl_row_capacity            */
+    GM_ERR_BOND_OVERSTRETCH = -7,    /* FENE bond with r >= R0                                    */
+    GM_ERR_NONFINITE = -8            /* a coordinate became NaN/Inf                               */
+};
+
+enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2 };
+enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2 };
+enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2 };
+
+#define GM_MAX_TYPES 8       /* particle types; pair tables are n_types x n_types */
+#define GM_MAX_BOND_TYPES 8
+
+/* Plain-old-data configuration, versioned by struct_size (= sizeof(gm_config)). */
+typedef struct {
+    uint32_t struct_size;
+    int32_t device;                  /* CUDA device ordinal                                        */
+    void *stream;                    /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy default */
+    int64_t n_particles;             /* N >= 1, < 2^31                                             */
+    int32_t n_types;                 /* 1..GM_MAX_TYPES                                            */
+    int32_t max_bonds_per_particle;  /* rows of the BL table (Fig. 2); 0 = no bonds  */
+    float box[3];                    /* cuboid edge lengths                                        */
+    float r_cut_max;                 /* largest pair cutoff that will be set (cell width = r_cut_max + r_skin) */
+    float r_skin;                    /* r_buffer of PAPER.md:L57                                   */
+    float dt;
+    uint64_t seed;                   /* key of the counter-based Philox4x32-10 noise               */
+    int32_t pair_style;              /* GM_PAIR_*                                                  */
+    int32_t bond_style;              /* GM_BOND_*                                                  */
+    int32_t integrator;              /* GM_NVE | GM_LANGEVIN | GM_DPD_GWVV                         */
+    float kT, gamma, lambda;         /* thermostat temperature, friction, GW-VV lambda             */
+    int32_t sfc_period;              /* steps between SFC reorders; 0 = only at the first build    */
+    int32_t nl_row_capacity;         /* rows of the NL table; 0 = choose from density              */
+    int32_t flags;                   /* GM_FLAG_*                                                  */
+    int32_t reserved;
+} gm_config;
+
+enum {
+    GM_FLAG_NO_GRAPH = 1,            /* launch every kernel directly (debugging)                   */
+    GM_FLAG_NO_COND_NODES = 2        /* gate the rebuild with early-exit kernels instead of a CUDA conditional graph node */
+};
+
+/* Bytes of device workspace gm_create needs for this configuration (all of the library's device
+ * memory: particle arrays, cell list, NL/NN and BL/BN tables, scratch).  Host-only. */
+gm_status gm_query_workspace(const gm_config *cfg, size_t *bytes);
+
+/* Create a system on a caller-allocated DEVICE workspace of at least gm_query_workspace() bytes,
+ * 256-byte aligned.  The workspace and the stream stay the caller's; they must outlive the system.
+ * Errors: INVALID_ARG (sizes, styles, n_types), BOX_TOO_SMALL, WORKSPACE_TOO_SMALL, CUDA. */
+gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t bytes, gm_system **out);
+
+/* Frees host state and CUDA graphs only (never the workspace).  Synchronises the stream. */
+gm_status gm_destroy(gm_system *s);
+
+/* Pair parameters for the type pair (ti, tj) and (tj, ti).  `p` is a HOST array of n floats:
+ *   GM_PAIR_LJ  (Eq. (1)): n = 4: eps, sigma, r_cut, shift_flag
+ *               (shift_flag != 0: the energy is shifted by U(r_cut) so that it vanishes at the
+ *               cutoff; the force is never altered -- DESIGN.md c-9)
+ *   GM_PAIR_DPD (DESIGN.md c-3):         n = 2: a, r_cut   (gamma and kT are global, gm_config)
+ * r_cut must be <= cfg.r_cut_max.  Errors: INVALID_ARG. */
+gm_status gm_set_pair_params(gm_system *s, int ti, int tj, const float *p, int n);
+
+/* Bond parameters of bond type `btype`: FENE (k, R0): U = -1/2 k R0^2 ln(1 - r^2/R0^2);
+ * harmonic (k, r0): U = k (r - r0)^2 -- Eq. (7), no factor 1/2. */
+gm_status gm_set_bond_params(gm_system *s, int btype, float k, float r0_or_R0);
+
+/* Particles in tag order, length N each: pos3/vel3 are (N,3) row-major floats, type is int32 in
+ * [0, n_types), mass may be NULL (all 1).  Positions outside the box are wrapped in.  Resets the
+ * step counter to 0 and invalidates the neighbor list.  vel3 are full-step velocities v(t).
+ * Errors: INVALID_ARG (NULL pos3/vel3/type), CUDA. */
+gm_status gm_set_particles(gm_system *s, const float *pos3, const float *vel3, const int32_t *type,
+                           const float *mass, int on_device);
+
+/* Bonds as n_bonds tag pairs (n_bonds,2) + a bond type each (NULL = all 0).  Each bond is entered
+ * in the BL table under BOTH ends.  Errors: INVALID_ARG if a bead would exceed
+ * max_bonds_per_particle or a tag is out of range (checked on the host; device inputs are copied
+ * to the host for this -- set-up path, not hot path). */
+gm_status gm_set_bonds(gm_system *s, int64_t n_bonds, const int32_t *tag_pairs2, const int32_t *btype,
+                       int on_device);
+
+/* Set the time-level counter (the `step` word of the Philox counter).  For restarts. */
+gm_status gm_set_step(gm_system *s, uint64_t step);
+
+/* a1 (+ a2 when due) + a3 now, at the current positions, unconditionally. */
+gm_status gm_build_neighbors(gm_system *s);
+
+/* a4 -> (a1, a3 if needed) -> a5/a6 + a7 at the current positions; the per-bead force is kept
+ * (gm_get_particles returns it).  For GM_LANGEVIN the drag and noise of the current time level are
+ * included (the force the integrator uses); for DPD the dissipative and random parts are included.
+ * Errors: STATE (no particles yet). */
+gm_status gm_compute_forces(gm_system *s);
+
+/* n_steps of a4..a8 (fused force + integrate kernel per step, rebuild gated on the device).
+ * Asynchronous on the stream.  Errors: STATE, INVALID_ARG (n_steps < 0), CUDA. */
+gm_status gm_step(gm_system *s, int64_t n_steps);
+
+/* out (HOST, 8 doubles): kinetic energy, pair PE, bond PE, temperature (3N-3 dof), px, py, pz,
+ * number of unique pairs inside r_cut.  fp32 terms, fp64 sums.  Synchronises. */
+gm_status gm_energies(gm_system *s, double out[8]);
+
+/* Current state in tag order; any of pos3/vel3/force3 may be NULL.  vel3 are full-step velocities
+ * v(t) (the library stores half-step velocities and completes them here); force3 is the force of
+ * the current time level (computed if not current). */
+gm_status gm_get_particles(gm_system *s, float *pos3, float *vel3, float *force3, int on_device);
+
+/* The neighbor list in TAG space: nn[tag] and nl_tags[tag * row_stride + k], k < nn[tag]
+ * (row order unspecified).  Builds the list first if none is current.  row_stride >= max nn
+ * (see gm_get_stats), else INVALID_ARG. */
+gm_status gm_get_neighbors(gm_system *s, int32_t *nn, int32_t *nl_tags, int64_t row_stride, int on_device);
+
+/* out (HOST, 8 int64): steps taken, neighbor rebuilds, SFC reorders, max nn of the current list,
+ * sum of nn of the current list, latched device error word (0 = none), nl_row_capacity,
+ * number of cells.  Synchronises; returns the latched device error as status if one is set. */
+gm_status gm_get_stats(gm_system *s, int64_t out[8]);
+
+/* Host-only utility (a2): the space-filling-curve rank of every cell of an nc[0] x nc[1] x nc[2] grid
+ * (linear cell id = (z * nc[1] + y) * nc[0] + x), i.e. the permutation the reorder sorts beads by:
+ * cells in Hilbert-curve order.  rank_out: HOST array of nc[0]*nc[1]*nc[2] uint32.  The order only
+ * affects memory locality, never results. */
+gm_status gm_sfc_cell_order(const int32_t nc[3], uint32_t *rank_out);
+
+/* Message of the last failing call on `s` (or a static string if s is NULL).  Never NULL. */
+const char *gm_last_error(const gm_system *s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GM_H */

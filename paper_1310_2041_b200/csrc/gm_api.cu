@@ -1,0 +1,696 @@
+// gm_api.cu -- the C ABI of include/gm.h: host-side state, workspace layout, the step scheduler
+// (CUDA graphs with the rebuild inside a conditional node) and marshalling.  All device work is in
+// gm_sort.cu / gm_nlist.cu / gm_force.cu / gm_io.cu; there is no CPU fallback for any of it.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "gm_internal.cuh"
+
+#define GM_GRAPH_STEPS 16   // steps per big graph launch (even)
+
+struct gm_system {
+    gm_config cfg;
+    GmParams P;
+    GmDev D;
+    cudaStream_t st, cap_st, cap_st2;
+    int cur;                       // which pos/vt buffer holds the current time level
+    bool have_particles, lagged, nl_valid, force_current, bonds_dirty, pair_set_any;
+    uint64_t step, last_reorder_step;
+    int64_t n_reorders;
+    bool use_graph, use_cond;
+    cudaGraphExec_t exec_big, exec_two;
+    char err[512];
+};
+
+static const char *k_null_msg = "gm: null system";
+
+static gm_status fail(gm_system *s, gm_status code, const char *fmt, const char *arg = "")
+{
+    if (s) snprintf(s->err, sizeof(s->err), fmt, arg);
+    return code;
+}
+
+#define CU(call)                                                                         \
+    do {                                                                                 \
+        cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess) return fail(s, GM_ERR_CUDA, "CUDA: %s", cudaGetErrorString(e_)); \
+    } while (0)
+
+static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// ---- geometry and constants derived from the configuration ----------------------------------------
+static gm_status derive(const gm_config *c, GmParams *P)
+{
+    memset(P, 0, sizeof(*P));
+    if (!c || c->struct_size != sizeof(gm_config)) return GM_ERR_INVALID_ARG;
+    if (c->n_particles < 1 || c->n_particles >= (1ll << GM_BOND_SHIFT)) return GM_ERR_INVALID_ARG;
+    if (c->n_types < 1 || c->n_types > GM_MAX_TYPES) return GM_ERR_INVALID_ARG;
+    if (c->max_bonds_per_particle < 0 || c->max_bonds_per_particle > 16) return GM_ERR_INVALID_ARG;
+    if (c->pair_style < GM_PAIR_NONE || c->pair_style > GM_PAIR_DPD) return GM_ERR_INVALID_ARG;
+    if (c->bond_style < GM_BOND_NONE || c->bond_style > GM_BOND_HARMONIC) return GM_ERR_INVALID_ARG;
+    if (c->integrator < GM_NVE || c->integrator > GM_DPD_GWVV) return GM_ERR_INVALID_ARG;
+    if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
+    for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
+    P->n = (int)c->n_particles;
+    P->n_types = c->n_types;
+    P->max_bonds = c->max_bonds_per_particle;
+    const double r_list = (double)c->r_cut_max + (double)c->r_skin;
+    double vol = 1.0;
+    for (int d = 0; d < 3; ++d) {
+        P->box[d] = c->box[d];
+        P->half[d] = 0.5f * c->box[d];
+        // cell width >= r_list with a 1e-4 relative margin for the fp32 cell assignment (reading c-12)
+        P->nc[d] = (int)std::floor((double)c->box[d] / (r_list * 1.0001));
+        if (P->nc[d] < 3) return GM_ERR_BOX_TOO_SMALL;
+        if (P->nc[d] > 1024) P->nc[d] = 1024;
+        vol *= c->box[d];
+    }
+    // sparse boxes: no more cells than a few per bead (wider cells stay correct)
+    while ((long long)P->nc[0] * P->nc[1] * P->nc[2] > 8ll * P->n + 64) {
+        int d = 0;
+        if (P->nc[1] > P->nc[d]) d = 1;
+        if (P->nc[2] > P->nc[d]) d = 2;
+        if (P->nc[d] <= 3) break;
+        P->nc[d] -= 1;
+    }
+    P->n_cells = P->nc[0] * P->nc[1] * P->nc[2];
+    for (int d = 0; d < 3; ++d) P->inv_w[d] = (float)((double)P->nc[d] / (double)c->box[d]);
+    P->r_list2 = (float)(r_list * r_list);
+    P->half_skin2 = (float)(0.25 * (double)c->r_skin * (double)c->r_skin);
+    P->edge_margin = (float)(r_list + (double)c->r_skin);
+    P->dt = c->dt; P->kT = c->kT; P->gamma = c->gamma; P->lambda = c->lambda;
+    P->sigma_r_sqrt_inv_dt = (float)std::sqrt(2.0 * (double)c->gamma * (double)c->kT / (double)c->dt);
+    P->lang_amp2 = (float)(6.0 * (double)c->gamma * (double)c->kT / (double)c->dt);
+    P->seed_lo = (uint32_t)(c->seed & 0xFFFFFFFFu);
+    P->seed_hi = (uint32_t)(c->seed >> 32);
+    P->pair_style = c->pair_style; P->bond_style = c->bond_style; P->integrator = c->integrator;
+    int cap = c->nl_row_capacity;
+    if (cap <= 0) {
+        double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
+        cap = (int)(2.0 * nbar) + 32;
+    }
+    cap = (cap + 7) / 8 * 8;
+    if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
+    P->nl_cap = cap;
+    for (int t = 0; t < GM_MAX_TYPES * GM_MAX_TYPES; ++t) { P->pair[t].c0 = 0.f; P->pair[t].c1 = 0.f; P->pair[t].c2 = 0.f; P->pair[t].c3 = 0.f; }
+    return GM_OK;
+}
+
+// ---- workspace layout: one pass with base == nullptr sizes it, a second pass assigns pointers ------
+static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> char * {
+        char *p = base ? base + off : nullptr;
+        off += align_up(bytes);
+        return p;
+    };
+    const size_t n = (size_t)P.n;
+    GmDev d;
+    memset(&d, 0, sizeof(d));
+    d.ctl = (GmCtl *)take(sizeof(GmCtl));
+    d.pos[0] = (float4 *)take(n * 16); d.pos[1] = (float4 *)take(n * 16);
+    d.vel = (float4 *)take(n * 16);
+    if (c.pair_style == GM_PAIR_DPD) { d.vt[0] = (float4 *)take(n * 16); d.vt[1] = (float4 *)take(n * 16); }
+    d.frc = (float4 *)take(n * 16);
+    d.ref = (float4 *)take(n * 16);
+    d.cpos = (float4 *)take(n * 16);
+    d.tmp4 = (float4 *)take(n * 16);
+    d.tag = (int *)take(n * 4); d.rtag = (int *)take(n * 4);
+    d.nn = (int *)take(n * 4);
+    d.nl = (int *)take(n * 4 * (size_t)P.nl_cap);
+    if (P.max_bonds > 0) {
+        d.bn = (int *)take(n * 4); d.bl = (int *)take(n * 4 * (size_t)P.max_bonds);
+        d.bn_tag = (int *)take(n * 4); d.bl_tag = (int *)take(n * 4 * (size_t)P.max_bonds);
+    }
+    d.key = (int *)take(n * 4); d.rank = (int *)take(n * 4); d.sorted = (int *)take(n * 4);
+    d.tmpi = (int *)take(n * 4);
+    d.cstart = (int *)take(((size_t)P.n_cells + 1) * 4);
+    size_t per = (size_t)GM_SCAN_BLOCK * GM_SCAN_ITEMS;
+    d.scan_sums = (int *)take((((size_t)P.n_cells + 1 + per - 1) / per + 1) * 4);
+    d.cell_rank = (uint32_t *)take((size_t)P.n_cells * 4);
+    d.stage = (float *)take(n * 4 * 11);
+    d.esum = (double *)take(((size_t)GM_ESUM_BLOCKS + 1) * 8 * sizeof(double));
+    if (D) *D = d;
+    return off;
+}
+
+// ---- a2: Hilbert order of the cells ------------------------------------------------------------------
+// Skilling's transpose form of the Hilbert curve (J. Skilling, "Programming the Hilbert curve", AIP
+// Conf. Proc. 707, 2004), restated: axes -> transposed index in place, then the bits are interleaved.
+static uint64_t hilbert_index(uint32_t x, uint32_t y, uint32_t z, int bits)
+{
+    uint32_t X[3] = { x, y, z };
+    const uint32_t M = 1u << (bits - 1);
+    for (uint32_t Q = M; Q > 1; Q >>= 1) {
+        const uint32_t Pm = Q - 1;
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= Pm;
+            else { uint32_t t = (X[0] ^ X[i]) & Pm; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    for (int i = 1; i < 3; ++i) X[i] ^= X[i - 1];
+    uint32_t t = 0;
+    for (uint32_t Q = M; Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
+    for (int i = 0; i < 3; ++i) X[i] ^= t;
+    uint64_t h = 0;
+    for (int b = bits - 1; b >= 0; --b)
+        for (int i = 0; i < 3; ++i) h = (h << 1) | ((X[i] >> b) & 1u);
+    return h;
+}
+
+extern "C" gm_status gm_sfc_cell_order(const int32_t nc[3], uint32_t *rank_out)
+{
+    if (!nc || !rank_out || nc[0] < 1 || nc[1] < 1 || nc[2] < 1) return GM_ERR_INVALID_ARG;
+    int mx = std::max(nc[0], std::max(nc[1], nc[2]));
+    int bits = 1;
+    while ((1 << bits) < mx) ++bits;
+    const size_t ncell = (size_t)nc[0] * nc[1] * nc[2];
+    std::vector<std::pair<uint64_t, uint32_t>> v(ncell);
+    for (int z = 0; z < nc[2]; ++z)
+        for (int y = 0; y < nc[1]; ++y)
+            for (int x = 0; x < nc[0]; ++x) {
+                uint32_t c = (uint32_t)((z * nc[1] + y) * nc[0] + x);
+                v[c] = std::make_pair(hilbert_index((uint32_t)x, (uint32_t)y, (uint32_t)z, bits), c);
+            }
+    std::sort(v.begin(), v.end());
+    for (size_t r = 0; r < ncell; ++r) rank_out[v[r].second] = (uint32_t)r;
+    return GM_OK;
+}
+
+// ---- create / destroy -----------------------------------------------------------------------------
+extern "C" gm_status gm_query_workspace(const gm_config *cfg, size_t *bytes)
+{
+    GmParams P;
+    gm_status r = derive(cfg, &P);
+    if (r != GM_OK) return r;
+    if (!bytes) return GM_ERR_INVALID_ARG;
+    *bytes = carve(P, *cfg, nullptr, nullptr);
+    return GM_OK;
+}
+
+static void drop_graphs(gm_system *s)
+{
+    if (s->exec_big) { cudaGraphExecDestroy(s->exec_big); s->exec_big = nullptr; }
+    if (s->exec_two) { cudaGraphExecDestroy(s->exec_two); s->exec_two = nullptr; }
+}
+
+extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t bytes, gm_system **out)
+{
+    if (!out) return GM_ERR_INVALID_ARG;
+    *out = nullptr;
+    GmParams P;
+    gm_status r = derive(cfg, &P);
+    if (r != GM_OK) return r;
+    if (!dev_workspace || ((uintptr_t)dev_workspace & 255)) return GM_ERR_INVALID_ARG;
+    if (bytes < carve(P, *cfg, nullptr, nullptr)) return GM_ERR_WORKSPACE_TOO_SMALL;
+    gm_system *s = new (std::nothrow) gm_system;
+    if (!s) return GM_ERR_INVALID_ARG;
+    memset(s, 0, sizeof(*s));
+    s->cfg = *cfg;
+    s->P = P;
+    carve(P, *cfg, (char *)dev_workspace, &s->D);
+    s->st = (cudaStream_t)cfg->stream;
+    s->use_graph = !(cfg->flags & GM_FLAG_NO_GRAPH);
+    s->use_cond = !(cfg->flags & GM_FLAG_NO_COND_NODES);
+    s->err[0] = 0;
+    cudaError_t e = cudaSetDevice(cfg->device);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st2, cudaStreamNonBlocking);
+    if (e == cudaSuccess) {
+        std::vector<uint32_t> rank((size_t)P.n_cells);
+        gm_sfc_cell_order(P.nc, rank.data());
+        e = cudaMemcpyAsync(s->D.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, s->st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+    }
+    if (e == cudaSuccess && P.max_bonds > 0) {
+        e = cudaMemsetAsync(s->D.bn_tag, 0, (size_t)P.n * 4, s->st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(s->D.bn, 0, (size_t)P.n * 4, s->st);
+    }
+    if (e == cudaSuccess) { gm_launch_set_ctl(s->D, 0, 1, s->st); e = cudaGetLastError(); }
+    if (e != cudaSuccess) {
+        if (s->cap_st) cudaStreamDestroy(s->cap_st);
+        if (s->cap_st2) cudaStreamDestroy(s->cap_st2);
+        delete s;
+        return GM_ERR_CUDA;
+    }
+    s->bonds_dirty = true;
+    *out = s;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_destroy(gm_system *s)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    cudaSetDevice(s->cfg.device);
+    cudaStreamSynchronize(s->st);
+    drop_graphs(s);
+    cudaStreamDestroy(s->cap_st);
+    cudaStreamDestroy(s->cap_st2);
+    delete s;
+    return GM_OK;
+}
+
+extern "C" const char *gm_last_error(const gm_system *s) { return s ? s->err : k_null_msg; }
+
+// ---- parameters -------------------------------------------------------------------------------------
+extern "C" gm_status gm_set_pair_params(gm_system *s, int ti, int tj, const float *p, int n)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!p || ti < 0 || tj < 0 || ti >= s->P.n_types || tj >= s->P.n_types)
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: bad type index or NULL%s");
+    GmPair c;
+    if (s->P.pair_style == GM_PAIR_LJ) {
+        if (n != 4) return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: LJ takes eps, sigma, r_cut, shift%s");
+        double eps = p[0], sig = p[1], rc = p[2];
+        if (!(rc > 0.0) || rc > (double)s->cfg.r_cut_max * (1.0 + 1e-6))
+            return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: r_cut outside (0, r_cut_max]%s");
+        double s6 = std::pow(sig, 6.0), s12 = s6 * s6;
+        double q6 = std::pow(sig / rc, 6.0);
+        c.c0 = (float)(rc * rc);
+        c.c1 = (float)(48.0 * eps * s12);
+        c.c2 = (float)(24.0 * eps * s6);
+        c.c3 = (p[3] != 0.f) ? (float)(4.0 * eps * (q6 * q6 - q6)) : 0.f;
+    } else if (s->P.pair_style == GM_PAIR_DPD) {
+        if (n != 2) return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: DPD takes a, r_cut%s");
+        double rc = p[1];
+        if (!(rc > 0.0) || rc > (double)s->cfg.r_cut_max * (1.0 + 1e-6))
+            return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: r_cut outside (0, r_cut_max]%s");
+        c.c0 = (float)(rc * rc); c.c1 = p[0]; c.c2 = (float)(1.0 / rc); c.c3 = p[1];
+    } else {
+        return fail(s, GM_ERR_STATE, "gm_set_pair_params: pair_style is GM_PAIR_NONE%s");
+    }
+    s->P.pair[ti * s->P.n_types + tj] = c;
+    s->P.pair[tj * s->P.n_types + ti] = c;
+    s->force_current = false;
+    drop_graphs(s);     // kernel parameters are baked into the graphs
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_bond_params(gm_system *s, int btype, float k, float r0)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (btype < 0 || btype >= GM_MAX_BOND_TYPES) return fail(s, GM_ERR_INVALID_ARG, "gm_set_bond_params: bad bond type%s");
+    if (s->P.bond_style == GM_BOND_FENE && !(r0 > 0.f)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_bond_params: FENE needs R0 > 0%s");
+    s->P.bond_k[btype] = k;
+    s->P.bond_r0[btype] = r0;
+    s->force_current = false;
+    drop_graphs(s);
+    return GM_OK;
+}
+
+// ---- particles and bonds ----------------------------------------------------------------------------
+extern "C" gm_status gm_set_particles(gm_system *s, const float *pos3, const float *vel3, const int32_t *type,
+                                      const float *mass, int on_device)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!pos3 || !vel3 || !type) return fail(s, GM_ERR_INVALID_ARG, "gm_set_particles: NULL array%s");
+    CU(cudaSetDevice(s->cfg.device));
+    const size_t n = (size_t)s->P.n;
+    const float *dp = pos3, *dv = vel3, *dm = mass;
+    const int *dt = type;
+    if (!on_device) {
+        float *st = s->D.stage;
+        CU(cudaMemcpyAsync(st, pos3, n * 12, cudaMemcpyHostToDevice, s->st));
+        CU(cudaMemcpyAsync(st + 3 * n, vel3, n * 12, cudaMemcpyHostToDevice, s->st));
+        CU(cudaMemcpyAsync(st + 9 * n, type, n * 4, cudaMemcpyHostToDevice, s->st));
+        if (mass) CU(cudaMemcpyAsync(st + 10 * n, mass, n * 4, cudaMemcpyHostToDevice, s->st));
+        dp = st; dv = st + 3 * n; dt = (const int *)(st + 9 * n); dm = mass ? st + 10 * n : nullptr;
+    }
+    s->cur = 0;
+    gm_launch_pack(s->P, s->D, 0, dp, dv, dt, dm, s->st);
+    gm_launch_set_ctl(s->D, 0, 1, s->st);
+    CU(cudaGetLastError());
+    s->step = 0;
+    s->n_reorders = 0;
+    s->have_particles = true;
+    s->lagged = false;
+    s->nl_valid = false;
+    s->force_current = false;
+    s->bonds_dirty = true;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_bonds(gm_system *s, int64_t n_bonds, const int32_t *tag_pairs2, const int32_t *btype,
+                                  int on_device)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (n_bonds < 0 || (n_bonds > 0 && !tag_pairs2)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_bonds: bad arguments%s");
+    if (s->P.max_bonds <= 0) {
+        if (n_bonds == 0) return GM_OK;
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_bonds: max_bonds_per_particle is 0%s");
+    }
+    CU(cudaSetDevice(s->cfg.device));
+    std::vector<int32_t> hp, ht;
+    const int32_t *pp = tag_pairs2, *tt = btype;
+    if (on_device && n_bonds > 0) {
+        hp.resize((size_t)n_bonds * 2);
+        CU(cudaMemcpyAsync(hp.data(), tag_pairs2, hp.size() * 4, cudaMemcpyDeviceToHost, s->st));
+        if (btype) { ht.resize((size_t)n_bonds); CU(cudaMemcpyAsync(ht.data(), btype, ht.size() * 4, cudaMemcpyDeviceToHost, s->st)); }
+        CU(cudaStreamSynchronize(s->st));
+        pp = hp.data(); tt = btype ? ht.data() : nullptr;
+    }
+    const size_t n = (size_t)s->P.n;
+    const int mb = s->P.max_bonds;
+    std::vector<int32_t> bn(n, 0), bl(n * (size_t)mb, 0);
+    for (int64_t b = 0; b < n_bonds; ++b) {
+        int32_t i = pp[2 * b], j = pp[2 * b + 1];
+        int32_t t = tt ? tt[b] : 0;
+        if (i < 0 || j < 0 || (size_t)i >= n || (size_t)j >= n || i == j || t < 0 || t >= GM_MAX_BOND_TYPES)
+            return fail(s, GM_ERR_INVALID_ARG, "gm_set_bonds: tag or bond type out of range%s");
+        if (bn[i] >= mb || bn[j] >= mb)
+            return fail(s, GM_ERR_INVALID_ARG, "gm_set_bonds: a bead exceeds max_bonds_per_particle%s");
+        bl[(size_t)bn[i] * n + i] = j | (t << GM_BOND_SHIFT); bn[i] += 1;   // stored under both ends
+        bl[(size_t)bn[j] * n + j] = i | (t << GM_BOND_SHIFT); bn[j] += 1;
+    }
+    CU(cudaMemcpyAsync(s->D.bn_tag, bn.data(), n * 4, cudaMemcpyHostToDevice, s->st));
+    CU(cudaMemcpyAsync(s->D.bl_tag, bl.data(), n * 4 * (size_t)mb, cudaMemcpyHostToDevice, s->st));
+    CU(cudaStreamSynchronize(s->st));      // the host vectors go out of scope
+    s->bonds_dirty = true;
+    s->force_current = false;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_step(gm_system *s, uint64_t step)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    CU(cudaSetDevice(s->cfg.device));
+    gm_launch_set_ctl(s->D, step, 0, s->st);
+    CU(cudaGetLastError());
+    s->step = step;
+    s->last_reorder_step = step;
+    s->nl_valid = false;       // `need` was reset: rebuild before the next force evaluation
+    s->force_current = false;
+    return GM_OK;
+}
+
+// ---- rebuild / reorder scheduling -------------------------------------------------------------------
+static void enqueue_rebuild(gm_system *s, int gate, cudaStream_t st)
+{
+    const float4 *pos = s->D.pos[s->cur];
+    gm_launch_sort_keys(s->P, s->D, pos, 0, gate, s->cur, st);
+    gm_launch_cell_finish(s->P, s->D, pos, 1, gate, s->cur, st);
+    gm_launch_nl_build(s->P, s->D, pos, gate, s->cur, st);
+}
+
+static bool reorder_due(const gm_system *s)
+{
+    if (s->cfg.sfc_period < 0) return false;
+    if (s->n_reorders == 0) return true;
+    return s->cfg.sfc_period > 0 && s->step - s->last_reorder_step >= (uint64_t)s->cfg.sfc_period;
+}
+
+// Make the NL usable for a force evaluation at the current time level, outside the graphs.
+static gm_status ensure_list(gm_system *s)
+{
+    bool forced = !s->nl_valid;
+    if (reorder_due(s)) {
+        const float4 *pos = s->D.pos[s->cur];
+        gm_launch_sort_keys(s->P, s->D, pos, 1, 0, s->cur, s->st);
+        gm_launch_cell_finish(s->P, s->D, pos, 0, 0, s->cur, s->st);
+        gm_launch_reorder(s->P, s->D, s->cur, s->st);
+        s->n_reorders += 1;
+        s->last_reorder_step = s->step;
+        s->bonds_dirty = true;
+        s->force_current = false;
+        forced = true;
+    }
+    if (s->bonds_dirty) { gm_launch_bonds_to_index(s->P, s->D, s->st); s->bonds_dirty = false; }
+    enqueue_rebuild(s, forced ? 0 : 1, s->st);
+    s->nl_valid = true;
+    CU(cudaGetLastError());
+    return GM_OK;
+}
+
+static void kicks(const gm_system *s, float *kick, float *kick_vt)
+{
+    const float dt = s->P.dt;
+    *kick = s->lagged ? dt : 0.5f * dt;
+    if (s->P.integrator == GM_DPD_GWVV) *kick_vt = s->lagged ? (0.5f + s->P.lambda) * dt : s->P.lambda * dt;
+    else *kick_vt = *kick;
+}
+
+static void enqueue_step_kernel(gm_system *s, bool lagged, cudaStream_t st)
+{
+    bool keep = s->lagged;
+    s->lagged = lagged;
+    float kick, kick_vt;
+    kicks(s, &kick, &kick_vt);
+    s->lagged = keep;
+    gm_launch_force(s->P, s->D, GM_MODE_STEP, s->cur, kick, kick_vt, 0, st);
+    s->cur ^= 1;
+}
+
+// Capture `nsteps` (even) steps starting from buffer 0 into an executable graph.  Each step is:
+// gate -> IF(rebuild due){a1, a3} -> fused force + integrate kernel.  Without conditional nodes the
+// rebuild kernels are launched every step and return at once when no rebuild is due.
+static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
+{
+    const int cur0 = s->cur;
+    cudaGraph_t graph = nullptr;
+    s->cur = 0;
+    cudaError_t e = cudaStreamBeginCapture(s->cap_st, cudaStreamCaptureModeRelaxed);
+    bool ok = (e == cudaSuccess);
+    for (int k = 0; ok && k < nsteps; ++k) {
+        if (s->use_cond) {
+            cudaStreamCaptureStatus status;
+            cudaGraph_t g = nullptr;
+            const cudaGraphNode_t *deps = nullptr;
+            size_t ndeps = 0;
+            ok = cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, &deps, &ndeps) == cudaSuccess;
+            cudaGraphConditionalHandle h;
+            ok = ok && cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+            if (ok) gm_launch_gate(s->D, s->cur, (unsigned long long)h, s->cap_st);
+            ok = ok && cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, &deps, &ndeps) == cudaSuccess;
+            cudaGraphNodeParams np = {};
+            np.type = cudaGraphNodeTypeConditional;
+            np.conditional.handle = h;
+            np.conditional.type = cudaGraphCondTypeIf;
+            np.conditional.size = 1;
+            cudaGraphNode_t node = nullptr;
+            ok = ok && cudaGraphAddNode(&node, g, deps, ndeps, &np) == cudaSuccess;
+            if (ok) {
+                cudaGraph_t body = np.conditional.phGraph_out[0];
+                ok = cudaStreamBeginCaptureToGraph(s->cap_st2, body, nullptr, nullptr, 0,
+                                                   cudaStreamCaptureModeRelaxed) == cudaSuccess;
+                if (ok) {
+                    enqueue_rebuild(s, 0, s->cap_st2);
+                    cudaGraph_t tmp = nullptr;
+                    ok = cudaStreamEndCapture(s->cap_st2, &tmp) == cudaSuccess;
+                }
+                ok = ok && cudaStreamUpdateCaptureDependencies(s->cap_st, &node, 1,
+                                                               cudaStreamSetCaptureDependencies) == cudaSuccess;
+            }
+        } else {
+            enqueue_rebuild(s, 1, s->cap_st);
+        }
+        if (ok) enqueue_step_kernel(s, true, s->cap_st);
+    }
+    e = cudaStreamEndCapture(s->cap_st, &graph);
+    ok = ok && e == cudaSuccess && graph != nullptr;
+    if (ok) ok = cudaGraphInstantiate(exec, graph, 0) == cudaSuccess;
+    if (graph) cudaGraphDestroy(graph);
+    s->cur = cur0;
+    if (!ok) {
+        cudaGetLastError();
+        *exec = nullptr;
+        return GM_ERR_CUDA;
+    }
+    return GM_OK;
+}
+
+static gm_status get_graph(gm_system *s, int nsteps, cudaGraphExec_t *slot)
+{
+    if (*slot) return GM_OK;
+    gm_status r = capture_graph(s, nsteps, slot);
+    if (r != GM_OK && s->use_cond) {      // conditional nodes unavailable: fall back to early-exit gating
+        s->use_cond = false;
+        r = capture_graph(s, nsteps, slot);
+    }
+    if (r != GM_OK) return fail(s, GM_ERR_CUDA, "CUDA graph capture failed%s");
+    return GM_OK;
+}
+
+extern "C" gm_status gm_build_neighbors(gm_system *s)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_build_neighbors: no particles set%s");
+    CU(cudaSetDevice(s->cfg.device));
+    s->nl_valid = false;
+    return ensure_list(s);
+}
+
+extern "C" gm_status gm_compute_forces(gm_system *s)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_compute_forces: no particles set%s");
+    CU(cudaSetDevice(s->cfg.device));
+    gm_status r = ensure_list(s);
+    if (r != GM_OK) return r;
+    gm_launch_force(s->P, s->D, GM_MODE_FORCES, s->cur, 0.f, 0.f, 0, s->st);
+    CU(cudaGetLastError());
+    s->force_current = true;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_step(gm_system *s, int64_t n_steps)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_step: no particles set%s");
+    if (n_steps < 0) return fail(s, GM_ERR_INVALID_ARG, "gm_step: n_steps < 0%s");
+    CU(cudaSetDevice(s->cfg.device));
+    int64_t left = n_steps;
+    while (left > 0) {
+        if (!s->nl_valid || reorder_due(s) || s->bonds_dirty) {
+            gm_status r = ensure_list(s);
+            if (r != GM_OK) return r;
+        }
+        int64_t chunk = left;
+        if (s->cfg.sfc_period > 0) {
+            int64_t until = (int64_t)s->cfg.sfc_period - (int64_t)(s->step - s->last_reorder_step);
+            if (until < 1) until = 1;
+            chunk = std::min(chunk, until);
+        }
+        int64_t done = 0;
+        while (done < chunk) {
+            const int64_t rem = chunk - done;
+            if (s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
+                const bool big = rem >= GM_GRAPH_STEPS;
+                cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
+                const int ns = big ? GM_GRAPH_STEPS : 2;
+                gm_status r = get_graph(s, ns, slot);
+                if (r != GM_OK) return r;
+                CU(cudaGraphLaunch(*slot, s->st));
+                done += ns;
+                s->step += (uint64_t)ns;
+            } else {
+                enqueue_rebuild(s, 1, s->st);
+                enqueue_step_kernel(s, s->lagged, s->st);
+                s->lagged = true;
+                done += 1;
+                s->step += 1;
+            }
+        }
+        left -= chunk;
+    }
+    CU(cudaGetLastError());
+    if (n_steps > 0) s->force_current = false;
+    return GM_OK;
+}
+
+// ---- results ----------------------------------------------------------------------------------------
+static gm_status dev_error(gm_system *s, const GmCtl &c)
+{
+    if (c.err & GM_DEV_ERR_NONFINITE) return fail(s, GM_ERR_NONFINITE, "a coordinate became non-finite%s");
+    if (c.err & GM_DEV_ERR_OVERSTRETCH) return fail(s, GM_ERR_BOND_OVERSTRETCH, "a FENE bond reached r >= R0%s");
+    if (c.err & GM_DEV_ERR_OVERFLOW) return fail(s, GM_ERR_NEIGHBOR_OVERFLOW, "a neighbor row exceeded nl_row_capacity%s");
+    return GM_OK;
+}
+
+static gm_status sync_and_check(gm_system *s, GmCtl *out = nullptr)
+{
+    GmCtl c;
+    CU(cudaMemcpyAsync(&c, s->D.ctl, sizeof(c), cudaMemcpyDeviceToHost, s->st));
+    CU(cudaStreamSynchronize(s->st));
+    if (out) *out = c;
+    return dev_error(s, c);
+}
+
+extern "C" gm_status gm_energies(gm_system *s, double out[8])
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!out) return fail(s, GM_ERR_INVALID_ARG, "gm_energies: NULL out%s");
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_energies: no particles set%s");
+    CU(cudaSetDevice(s->cfg.device));
+    gm_status r = ensure_list(s);
+    if (r != GM_OK) return r;
+    gm_launch_force(s->P, s->D, GM_MODE_ENERGY, s->cur, 0.f, 0.f, s->lagged ? 1 : 0, s->st);
+    CU(cudaGetLastError());
+    double h[8];
+    CU(cudaMemcpyAsync(h, s->D.esum + (size_t)GM_ESUM_BLOCKS * 8, sizeof(h), cudaMemcpyDeviceToHost, s->st));
+    r = sync_and_check(s);
+    const double dof = s->P.n > 1 ? 3.0 * s->P.n - 3.0 : 3.0;
+    out[0] = h[0]; out[1] = h[1]; out[2] = h[2];
+    out[3] = 2.0 * h[0] / dof;
+    out[4] = h[3]; out[5] = h[4]; out[6] = h[5]; out[7] = h[6];
+    return r;
+}
+
+extern "C" gm_status gm_get_particles(gm_system *s, float *pos3, float *vel3, float *force3, int on_device)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_get_particles: no particles set%s");
+    CU(cudaSetDevice(s->cfg.device));
+    if ((force3 || (vel3 && s->lagged)) && !s->force_current) {
+        gm_status r = gm_compute_forces(s);
+        if (r != GM_OK) return r;
+    }
+    const size_t n = (size_t)s->P.n;
+    float *st = s->D.stage;
+    float *dp = pos3, *dv = vel3, *df = force3;
+    if (!on_device) {
+        dp = pos3 ? st : nullptr; dv = vel3 ? st + 3 * n : nullptr; df = force3 ? st + 6 * n : nullptr;
+    }
+    gm_launch_unpack(s->P, s->D, s->cur, dp, dv, df, s->lagged ? 1 : 0, s->st);
+    CU(cudaGetLastError());
+    if (!on_device) {
+        if (pos3) CU(cudaMemcpyAsync(pos3, dp, n * 12, cudaMemcpyDeviceToHost, s->st));
+        if (vel3) CU(cudaMemcpyAsync(vel3, dv, n * 12, cudaMemcpyDeviceToHost, s->st));
+        if (force3) CU(cudaMemcpyAsync(force3, df, n * 12, cudaMemcpyDeviceToHost, s->st));
+        return sync_and_check(s);
+    }
+    return GM_OK;
+}
+
+extern "C" gm_status gm_get_neighbors(gm_system *s, int32_t *nn, int32_t *nl_tags, int64_t row_stride, int on_device)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_get_neighbors: no particles set%s");
+    if (!nn || !nl_tags || row_stride < 1) return fail(s, GM_ERR_INVALID_ARG, "gm_get_neighbors: bad arguments%s");
+    CU(cudaSetDevice(s->cfg.device));
+    if (!s->nl_valid) { gm_status r = ensure_list(s); if (r != GM_OK) return r; }
+    GmCtl c;
+    gm_status r = sync_and_check(s, &c);
+    if (r != GM_OK) return r;
+    if (row_stride < c.max_nn) return fail(s, GM_ERR_INVALID_ARG, "gm_get_neighbors: row_stride < max nn%s");
+    const size_t n = (size_t)s->P.n;
+    if (on_device) {
+        gm_launch_unpack_neighbors(s->P, s->D, nn, nl_tags, row_stride, s->st);
+        CU(cudaGetLastError());
+        return GM_OK;
+    }
+    // validation path: a temporary device image of the tag-space table
+    int *tmp = nullptr;
+    CU(cudaMalloc(&tmp, n * 4 * (size_t)(row_stride + 1)));
+    gm_launch_unpack_neighbors(s->P, s->D, tmp, tmp + n, row_stride, s->st);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(nn, tmp, n * 4, cudaMemcpyDeviceToHost, s->st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(nl_tags, tmp + n, n * 4 * (size_t)row_stride, cudaMemcpyDeviceToHost, s->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+    cudaFree(tmp);
+    if (e != cudaSuccess) return fail(s, GM_ERR_CUDA, "CUDA: %s", cudaGetErrorString(e));
+    return GM_OK;
+}
+
+extern "C" gm_status gm_get_stats(gm_system *s, int64_t out[8])
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!out) return fail(s, GM_ERR_INVALID_ARG, "gm_get_stats: NULL out%s");
+    CU(cudaSetDevice(s->cfg.device));
+    GmCtl c;
+    gm_status r = sync_and_check(s, &c);
+    if (r == GM_ERR_CUDA) return r;
+    out[0] = (int64_t)s->step;
+    out[1] = (int64_t)c.n_rebuilds;
+    out[2] = s->n_reorders;
+    out[3] = c.max_nn;
+    out[4] = (int64_t)c.sum_nn;
+    out[5] = c.err;
+    out[6] = s->P.nl_cap;
+    out[7] = s->P.n_cells;
+    return r;
+}

@@ -1,0 +1,291 @@
+// gm_force.cu -- a4..a9: pair + bond forces from the NL/BL tables, fused with the integrator and the
+// displacement test.
+//
+//   a5  Lennard-Jones, Eq. (1); gather loop over NL[(i,k)] with minimum image and a
+//       cutoff test as in Alg. 2, L458.  One thread owns bead i and sums all of its forces
+//       ("one thread calculates and sums all non-bonded forces of a particle"), so a pair
+//       is evaluated from both sides and no atomics are needed.
+//   a6  DPD (Groot-Warren; reading c-3) with one Philox4x32-10 draw per pair keyed
+//       (seed; min tag, max tag, step, 0) so that theta_ij = theta_ji without communication.
+//   a7  bonds from BL/BN, each bond evaluated from both ends; harmonic Eq. (7),
+//       FENE (reading c-8).
+//   a8  velocity-Verlet NVE / Langevin ("BD") / GW-VV in kick-drift form: the kernel
+//       at time level m computes a(r^m), then u^{m} = u^{m-1} + kick a, r^{m+1} = r^m + dt u^m, where u
+//       is the half-step velocity v^{m-1/2} (kick = dt), or the full-step v^m right after
+//       gm_set_particles (kick = dt/2).  The force never leaves registers.
+//   a4  displacement test |r^{m+1} - r_ref| > skin/2 -> ctl->need = m + 1.
+//   a9  energies: fp32 terms, fp64 sums, fixed-order two-stage reduction.
+#include "gm_internal.cuh"
+
+#define FORCE_BLOCK 128
+
+struct BeadForce {
+    float fx, fy, fz;
+    float pe_pair, pe_bond;   // this bead's half share
+    float cnt;                // partners inside r_cut
+};
+
+template <int PAIR, bool NT1, bool ENERGY, bool MI>
+__device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
+                                          const float4 *__restrict__ vt, int i, const float4 pi, const int ti,
+                                          const float4 vti, unsigned long long step, BeadForce &o)
+{
+    const int nn = D.nn[i];
+    const int *__restrict__ nl = D.nl + i;
+    const size_t n = (size_t)P.n;
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
+    const GmPair p0 = P.pair[0];
+    for (int k = 0; k < nn; ++k) {
+        const int j = nl[(size_t)k * n];
+        const float4 pj = pos[j];
+        float dx, dy, dz;
+        if (MI) {
+            dx = gm_min_image(pi.x, pj.x, P.half[0]);
+            dy = gm_min_image(pi.y, pj.y, P.half[1]);
+            dz = gm_min_image(pi.z, pj.z, P.half[2]);
+        } else {
+            dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
+        }
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        GmPair c = p0;
+        if (!NT1) c = P.pair[ti * P.n_types + __float_as_int(pj.w)];
+        if (r2 < c.c0) {
+            if (PAIR == GM_PAIR_LJ) {
+                // F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij
+                const float r2i = gm_rcp(r2);
+                const float r6i = r2i * r2i * r2i;
+                const float fs = r2i * r6i * (c.c1 * r6i - c.c2);
+                fx += fs * dx; fy += fs * dy; fz += fs * dz;
+                if (ENERGY) {
+                    pe += r6i * (c.c1 * (1.0f / 12.0f) * r6i - c.c2 * (1.0f / 6.0f)) - c.c3;
+                    cnt += 1.0f;
+                }
+            } else if (PAIR == GM_PAIR_DPD) {
+                if (ENERGY) cnt += 1.0f;
+                if (r2 >= 1e-12f) {
+                    // F_ij = [a w - gamma w^2 (e.v_ij) + sigma_R w theta / sqrt(dt)] e,  w = 1 - r/r_c
+                    const float4 vtj = vt[j];
+                    const float ri = rsqrtf(r2);
+                    const float r = r2 * ri;
+                    const float w = 1.0f - r * c.c2;
+                    const float edv = (dx * (vti.x - vtj.x) + dy * (vti.y - vtj.y) + dz * (vti.z - vtj.z)) * ri;
+                    const uint32_t ta = (uint32_t)__float_as_int(vti.w), tb = (uint32_t)__float_as_int(vtj.w);
+                    const uint4 rn = gm_philox4x32_10(make_uint4(min(ta, tb), max(ta, tb), (uint32_t)step, 0u),
+                                                      make_uint2(P.seed_lo, P.seed_hi));
+                    const float theta = 1.7320508075688772f * gm_sym24(rn.x);
+                    const float fs = (c.c1 * w - P.gamma * w * w * edv + P.sigma_r_sqrt_inv_dt * w * theta) * ri;
+                    fx += fs * dx; fy += fs * dy; fz += fs * dz;
+                    if (ENERGY) pe += 0.5f * c.c1 * c.c3 * w * w;
+                }
+            }
+        }
+    }
+    o.fx = fx; o.fy = fy; o.fz = fz;
+    o.pe_pair = 0.5f * pe;
+    o.cnt = cnt;
+}
+
+template <bool ENERGY>
+__device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
+                                          int i, const float4 pi, BeadForce &o)
+{
+    float pe = 0.f;
+    if (P.max_bonds > 0 && P.bond_style != GM_BOND_NONE) {
+        const int nb = D.bn[i];
+        const size_t n = (size_t)P.n;
+        for (int k = 0; k < nb; ++k) {
+            const int e = D.bl[(size_t)k * n + i];
+            const int j = e & GM_BOND_MASK, bt = (unsigned)e >> GM_BOND_SHIFT;
+            const float4 pj = pos[j];
+            const float dx = gm_min_image(pi.x, pj.x, P.half[0]);
+            const float dy = gm_min_image(pi.y, pj.y, P.half[1]);
+            const float dz = gm_min_image(pi.z, pj.z, P.half[2]);
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const float kb = P.bond_k[bt], r0 = P.bond_r0[bt];
+            float fs;
+            if (P.bond_style == GM_BOND_FENE) {
+                // U = -1/2 k R0^2 ln(1 - r^2/R0^2);  F_i = -k r_ij / (1 - r^2/R0^2)
+                const float q = 1.0f - r2 / (r0 * r0);
+                if (!(q > 0.0f)) { atomicOr(&D.ctl->err, GM_DEV_ERR_OVERSTRETCH); continue; }
+                fs = -kb / q;
+                if (ENERGY) pe += -0.5f * kb * r0 * r0 * logf(q);
+            } else {
+                // Eq. (7): U = k (r - r0)^2;  F_i = -2 k (1 - r0/r) r_ij
+                if (r0 == 0.0f) {
+                    fs = -2.0f * kb;
+                    if (ENERGY) pe += kb * r2;
+                } else {
+                    const float r = sqrtf(r2);
+                    fs = (r > 0.0f) ? -2.0f * kb * (1.0f - r0 / r) : 0.0f;
+                    if (ENERGY) pe += kb * (r - r0) * (r - r0);
+                }
+            }
+            o.fx += fs * dx; o.fy += fs * dy; o.fz += fs * dz;
+        }
+    }
+    o.pe_bond = 0.5f * pe;
+}
+
+// Force on bead i at time level `step`, conservative + (DPD) dissipative/random.  vti: own v~ and tag.
+template <int PAIR, bool NT1, bool ENERGY>
+__device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
+                                                const float4 *__restrict__ vt, int i, const float4 pi,
+                                                const float4 vti, unsigned long long step)
+{
+    BeadForce o;
+    o.fx = o.fy = o.fz = o.pe_pair = o.pe_bond = o.cnt = 0.f;
+    const int ti = __float_as_int(pi.w);
+    if (PAIR != GM_PAIR_NONE) {
+        // A bead further than r_list + skin from every face cannot have a listed partner across the
+        // boundary (both moved < skin/2 since the build): plain differences, no image test.
+        const float m = P.edge_margin;
+        const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
+                              fabsf(pi.z) < P.half[2] - m;
+        if (interior) pair_loop<PAIR, NT1, ENERGY, false>(P, D, pos, vt, i, pi, ti, vti, step, o);
+        else pair_loop<PAIR, NT1, ENERGY, true>(P, D, pos, vt, i, pi, ti, vti, step, o);
+    }
+    bond_loop<ENERGY>(P, D, pos, i, pi, o);
+    return o;
+}
+
+// Acceleration the integrator uses: F/m, plus Langevin drag on the stored velocity and the per-bead
+// noise of this time level (reading c-7): a = F/m - gamma u + sqrt(6 gamma kT / (dt m)) xi.
+__device__ __forceinline__ float3 bead_accel(const GmParams &P, const GmDev &D, int i, const BeadForce &f,
+                                             const float4 u, unsigned long long step)
+{
+    const float im = 1.0f / u.w;
+    float3 a = make_float3(f.fx * im, f.fy * im, f.fz * im);
+    if (P.integrator == GM_LANGEVIN) {
+        const uint4 rn = gm_philox4x32_10(make_uint4((uint32_t)D.tag[i], 0u, (uint32_t)step, 1u),
+                                          make_uint2(P.seed_lo, P.seed_hi));
+        const float amp = sqrtf(P.lang_amp2 * im);
+        a.x += -P.gamma * u.x + amp * gm_sym24(rn.x);
+        a.y += -P.gamma * u.y + amp * gm_sym24(rn.y);
+        a.z += -P.gamma * u.z + amp * gm_sym24(rn.z);
+    }
+    return a;
+}
+
+// ---- the per-step kernel (MODE_STEP) and the force-materialising kernel (MODE_FORCES) ---------------
+template <int PAIR, bool NT1, int MODE>
+__global__ void __launch_bounds__(FORCE_BLOCK)
+k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long step = D.ctl->step[parity];
+    if (MODE == GM_MODE_STEP && blockIdx.x == 0 && threadIdx.x == 0) D.ctl->step[parity ^ 1] = step + 1;
+    if (i >= P.n) return;
+    const float4 *__restrict__ pos = D.pos[parity];
+    const float4 *__restrict__ vt = D.vt[parity];
+    const float4 pi = pos[i];
+    float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (PAIR == GM_PAIR_DPD) vti = vt[i];
+    const BeadForce f = bead_force<PAIR, NT1, MODE == GM_MODE_FORCES>(P, D, pos, vt, i, pi, vti, step);
+    const float4 u = D.vel[i];
+    const float3 a = bead_accel(P, D, i, f, u, step);
+    if (MODE == GM_MODE_FORCES) {
+        D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
+        return;
+    }
+    // a8: kick, drift, wrap
+    if (PAIR == GM_PAIR_DPD)
+        D.vt[parity ^ 1][i] = make_float4(u.x + kick_vt * a.x, u.y + kick_vt * a.y, u.z + kick_vt * a.z, vti.w);
+    const float ux = u.x + kick * a.x, uy = u.y + kick * a.y, uz = u.z + kick * a.z;
+    D.vel[i] = make_float4(ux, uy, uz, u.w);
+    const float x = gm_wrap(pi.x + P.dt * ux, P.half[0], P.box[0]);
+    const float y = gm_wrap(pi.y + P.dt * uy, P.half[1], P.box[1]);
+    const float z = gm_wrap(pi.z + P.dt * uz, P.half[2], P.box[2]);
+    D.pos[parity ^ 1][i] = make_float4(x, y, z, pi.w);
+    // a4: displacement since the last NL build
+    const float4 rf = D.ref[i];
+    const float dx = gm_min_image(x, rf.x, P.half[0]);
+    const float dy = gm_min_image(y, rf.y, P.half[1]);
+    const float dz = gm_min_image(z, rf.z, P.half[2]);
+    if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) D.ctl->need = step + 1;
+}
+
+// ---- a9 energies: grid-stride, fp64 accumulation, per-block partials in fixed order ----------------
+template <int PAIR, bool NT1>
+__global__ void __launch_bounds__(FORCE_BLOCK)
+k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
+{
+    const unsigned long long step = D.ctl->step[parity];
+    const float4 *__restrict__ pos = D.pos[parity];
+    const float4 *__restrict__ vt = D.vt[parity];
+    double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };   // ke, pe_pair, pe_bond, px, py, pz, pairs
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += gridDim.x * blockDim.x) {
+        const float4 pi = pos[i];
+        float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (PAIR == GM_PAIR_DPD) vti = vt[i];
+        const BeadForce f = bead_force<PAIR, NT1, true>(P, D, pos, vt, i, pi, vti, step);
+        const float4 u = D.vel[i];
+        float vx = u.x, vy = u.y, vz = u.z;
+        if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m
+            const float3 a = bead_accel(P, D, i, f, u, step);
+            vx += 0.5f * P.dt * a.x; vy += 0.5f * P.dt * a.y; vz += 0.5f * P.dt * a.z;
+        }
+        acc[0] += 0.5 * (double)u.w * ((double)vx * vx + (double)vy * vy + (double)vz * vz);
+        acc[1] += (double)f.pe_pair;
+        acc[2] += (double)f.pe_bond;
+        acc[3] += (double)u.w * vx; acc[4] += (double)u.w * vy; acc[5] += (double)u.w * vz;
+        acc[6] += 0.5 * (double)f.cnt;
+    }
+    __shared__ double sh[FORCE_BLOCK / 32][7];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int q = 0; q < 7; ++q) {
+        double v = acc[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (lane == 0) sh[wid][q] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 7) {
+        double v = 0.0;
+        for (int w = 0; w < FORCE_BLOCK / 32; ++w) v += sh[w][threadIdx.x];
+        D.esum[(size_t)blockIdx.x * 8 + threadIdx.x] = v;
+    }
+}
+
+__global__ void k_energy_final(GmDev D, int n_blocks)
+{
+    if (threadIdx.x < 7) {
+        double v = 0.0;
+        for (int b = 0; b < n_blocks; ++b) v += D.esum[(size_t)b * 8 + threadIdx.x];
+        D.esum[(size_t)GM_ESUM_BLOCKS * 8 + threadIdx.x] = v;
+    }
+}
+
+template <int PAIR, bool NT1>
+static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
+                           int lagged, cudaStream_t st)
+{
+    int nb = (P.n + FORCE_BLOCK - 1) / FORCE_BLOCK;
+    if (mode == GM_MODE_STEP)
+        k_force<PAIR, NT1, GM_MODE_STEP><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+    else if (mode == GM_MODE_FORCES)
+        k_force<PAIR, NT1, GM_MODE_FORCES><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+    else {
+        int g = nb < GM_ESUM_BLOCKS ? nb : GM_ESUM_BLOCKS;
+        k_energy<PAIR, NT1><<<g, FORCE_BLOCK, 0, st>>>(P, D, parity, lagged);
+        k_energy_final<<<1, 32, 0, st>>>(D, g);
+    }
+}
+
+void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
+                     int lagged, cudaStream_t st)
+{
+    const bool nt1 = (P.n_types == 1);
+    switch (P.pair_style) {
+    case GM_PAIR_LJ:
+        if (nt1) launch_force_t<GM_PAIR_LJ, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_t<GM_PAIR_LJ, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        break;
+    case GM_PAIR_DPD:
+        if (nt1) launch_force_t<GM_PAIR_DPD, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_t<GM_PAIR_DPD, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        break;
+    default:
+        launch_force_t<GM_PAIR_NONE, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+    }
+}

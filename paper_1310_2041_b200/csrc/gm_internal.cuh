@@ -1,0 +1,166 @@
+// gm_internal.cuh -- shared declarations of libgm's CUDA path (sm_100a).  Nothing here is used by,
+// or derived from, the CPU oracle under oracle/.
+//
+// Device data layout:
+//   pos[2]  float4[N]  x, y, z, type (int bits)          ping-pong; STORAGE order (SFC order of the
+//   vel     float4[N]  u_x, u_y, u_z, mass               last reorder).  u is the half-step velocity
+//   vt[2]   float4[N]  v~_x, v~_y, v~_z, tag (int bits)  DPD only: the velocity the dissipative force sees
+//   frc     float4[N]  F_x, F_y, F_z, per-bead PE        materialised only by gm_compute_forces
+//   ref     float4[N]  position at the last NL build     (displacement test a4)
+//   nl      int[cap*N] NL[k*N + i], column-major table   PAPER.md:L51, Fig. 1
+//   nn      int[N]     NN[i]
+//   bl      int[mb*N]  BL[k*N + i] = j | btype << 28     PAPER.md:L97, Fig. 2 (index space)
+//   bn      int[N]
+//   cpos    float4[N]  x, y, z, storage index            cell list CL in CSR form
+//   cstart  int[n_cells + 1]                             replaces CN: cell c holds cpos[cstart[c] .. cstart[c+1])
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/gm.h"
+
+#define GM_BOND_SHIFT 28
+#define GM_BOND_MASK ((1 << GM_BOND_SHIFT) - 1)
+
+// latched device error bits (GmCtl::err)
+enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE = 4 };
+
+// Small device control block (one per system).
+struct GmCtl {
+    unsigned long long step[2];    // time level m, indexed by the parity of the current position buffer
+    unsigned long long need;       // time level at which the NL must be rebuilt before forces (a4)
+    unsigned long long n_rebuilds;
+    unsigned long long sum_nn;
+    int max_nn;
+    int err;
+    int built;                     // 1 once a list exists
+    int pad;
+};
+
+// Per-type-pair coefficients.  LJ: c0 = r_c^2, c1 = 48 eps sigma^12, c2 = 24 eps sigma^6, c3 = U_shift.
+//                              DPD: c0 = r_c^2, c1 = a, c2 = 1/r_c, c3 = r_c.
+struct GmPair { float c0, c1, c2, c3; };
+
+// Constants of one system, passed to kernels by value (constant bank).
+struct GmParams {
+    int n, n_types, max_bonds, nl_cap;
+    int nc[3], n_cells;
+    float box[3], half[3], inv_w[3];
+    float r_list2, half_skin2;
+    float edge_margin;             // r_list + r_skin: beads further than this from every face need no image test
+    float dt, kT, gamma, lambda;
+    float sigma_r_sqrt_inv_dt;     // sqrt(2 gamma kT / dt)             (DPD random force amplitude)
+    float lang_amp2;               // 6 gamma kT / dt                   (Langevin: amp/m = sqrt(lang_amp2 / m))
+    uint32_t seed_lo, seed_hi;
+    int pair_style, bond_style, integrator;
+    GmPair pair[GM_MAX_TYPES * GM_MAX_TYPES];
+    float bond_k[GM_MAX_BOND_TYPES], bond_r0[GM_MAX_BOND_TYPES];
+};
+
+// Device pointers that do not ping-pong.
+struct GmDev {
+    float4 *pos[2];
+    float4 *vel;
+    float4 *vt[2];
+    float4 *frc;
+    float4 *ref;
+    int *tag, *rtag;
+    int *nn, *nl;
+    int *bn, *bl;            // index space
+    int *bn_tag, *bl_tag;    // tag space master copy (bl_tag[k*N + tag] = partner tag | btype << 28)
+    int *key, *rank, *sorted;
+    int *cstart;             // n_cells + 1
+    int *scan_sums;          // per scan block
+    uint32_t *cell_rank;     // SFC rank of each linear cell id
+    float4 *cpos;
+    float4 *tmp4;            // N float4 scratch (reorder)
+    int *tmpi;               // N int scratch (reorder)
+    float *stage;            // 10 N floats: I/O staging (pos3, vel3, force3, mass) ; reused as ints
+    double *esum;            // [GM_ESUM_BLOCKS * 8] partials, then [8] totals at the end
+    GmCtl *ctl;
+};
+
+#define GM_ESUM_BLOCKS 1184      // 8 x 148: grid of the energy reduction
+#define GM_SCAN_BLOCK 1024
+#define GM_SCAN_ITEMS 4          // per thread
+
+enum { GM_MODE_STEP = 0, GM_MODE_FORCES = 1, GM_MODE_ENERGY = 2 };
+
+// ---- launch wrappers (each enqueues on `st`; `gate` != 0: run only if ctl->need == ctl->step[parity]) ----
+void gm_launch_sort_keys(const GmParams &P, const GmDev &D, const float4 *pos, int use_sfc_rank, int gate,
+                         int parity, cudaStream_t st);
+void gm_launch_cell_finish(const GmParams &P, const GmDev &D, const float4 *pos, int write_cpos, int gate,
+                           int parity, cudaStream_t st);
+void gm_launch_nl_build(const GmParams &P, const GmDev &D, const float4 *pos, int gate, int parity,
+                        cudaStream_t st);
+void gm_launch_reorder(const GmParams &P, GmDev &D, int cur, cudaStream_t st);   // uses D.sorted as the permutation
+void gm_launch_bonds_to_index(const GmParams &P, const GmDev &D, cudaStream_t st);
+void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
+                     int lagged, cudaStream_t st);
+void gm_launch_pack(const GmParams &P, const GmDev &D, int cur, const float *pos3, const float *vel3,
+                    const int *type, const float *mass, cudaStream_t st);
+void gm_launch_unpack(const GmParams &P, const GmDev &D, int cur, float *pos3, float *vel3, float *force3,
+                      int lagged, cudaStream_t st);
+void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,
+                                cudaStream_t st);
+void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, cudaStream_t st);
+void gm_launch_gate(const GmDev &D, int parity, unsigned long long cond_handle, cudaStream_t st);
+
+// ---- device helpers ---------------------------------------------------------------------------------
+#ifdef __CUDACC__
+// Minimum image of a - b in a periodic box (PAPER.md: Alg. 2 line 6, L458).  A direct a - b is exact
+// (Sterbenz) or rounded to half an ulp of the SMALL result when the pair does not cross the box; a
+// pair across the boundary has |a - b| ~ L, where the subtraction would round at ulp(L) -- so those
+// are taken relative to the two faces, (a -+ L/2) - (b +- L/2), which is again exact for any pair
+// closer than L/3.
+__device__ __forceinline__ float gm_min_image(float a, float b, float half)
+{
+    float d = a - b;
+    if (d > half) d = (a - half) - (b + half);
+    else if (d < -half) d = (a + half) - (b - half);
+    return d;
+}
+
+__device__ __forceinline__ float gm_wrap(float x, float half, float L)
+{
+    if (x >= half) x -= L;
+    else if (x < -half) x += L;
+    return x;
+}
+
+__device__ __forceinline__ int gm_cell_coord(float x, float half, float inv_w, int nc)
+{
+    int c = (int)((x + half) * inv_w);
+    return min(max(c, 0), nc - 1);
+}
+
+__device__ __forceinline__ float gm_rcp(float x)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), written from the publication: ten rounds of
+// two 32x32->64 multiplies with the key bumped by the Weyl constants between rounds.
+__device__ __forceinline__ uint4 gm_philox4x32_10(uint4 c, uint2 k)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        c = make_uint4(hi1 ^ c.y ^ k.x, lo1, hi0 ^ c.w ^ k.y, lo0);
+        k.x += 0x9E3779B9u;
+        k.y += 0xBB67AE85u;
+    }
+    return c;
+}
+
+// Symmetric uniform variate in (-1, 1) from the top 24 bits: 2u - 1 with u = (k + 1/2) 2^-24,
+// i.e. (2k + 1 - 2^24) 2^-24 -- an odd integer below 2^24 in magnitude, exact in fp32.
+__device__ __forceinline__ float gm_sym24(uint32_t x)
+{
+    int k = (int)(x >> 8);
+    return (float)(2 * k + 1 - 16777216) * (1.0f / 16777216.0f);
+}
+#endif

@@ -1,0 +1,314 @@
+"""ctypes binding of include/gm.h -- argument marshalling only; every step of the path runs in the
+CUDA kernels of libgm.so.  PyTorch supplies device memory (the workspace blob, device-side I/O
+tensors) and the CUDA stream, nothing else.
+
+Function names and argument order are those of include/gm.h; each wrapper raises GmError on a
+non-zero status.  `System` bundles create + parameter calls for a workload description (any object
+with the attributes of workloads.Workload; this module does not import it).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgm.so")
+
+GM_OK = 0
+GM_ERR_INVALID_ARG, GM_ERR_STATE, GM_ERR_CUDA, GM_ERR_WORKSPACE_TOO_SMALL = -1, -2, -3, -4
+GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_NONFINITE = -5, -6, -7, -8
+GM_PAIR = {"none": 0, "lj": 1, "dpd": 2}
+GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
+GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
+GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES = 1, 2
+
+SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_bond_params",
+           "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
+           "gm_step", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
+           "gm_sfc_cell_order", "gm_last_error"]
+
+
+class gm_config(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("device", C.c_int32), ("stream", C.c_void_p),
+        ("n_particles", C.c_int64), ("n_types", C.c_int32), ("max_bonds_per_particle", C.c_int32),
+        ("box", C.c_float * 3), ("r_cut_max", C.c_float), ("r_skin", C.c_float), ("dt", C.c_float),
+        ("seed", C.c_uint64),
+        ("pair_style", C.c_int32), ("bond_style", C.c_int32), ("integrator", C.c_int32),
+        ("kT", C.c_float), ("gamma", C.c_float), ("lam", C.c_float),
+        ("sfc_period", C.c_int32), ("nl_row_capacity", C.c_int32), ("flags", C.c_int32),
+        ("reserved", C.c_int32),
+    ]
+
+
+class GmError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"gm status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Load libgm.so (no GPU needed to load; CUDA is initialised on the first device call)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1310_2041_b200.build` "
+                              "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64 = C.c_void_p, C.c_int, C.c_int64
+        L.gm_query_workspace.argtypes = [C.POINTER(gm_config), C.POINTER(C.c_size_t)]
+        L.gm_create.argtypes = [C.POINTER(gm_config), vp, C.c_size_t, C.POINTER(vp)]
+        L.gm_destroy.argtypes = [vp]
+        L.gm_set_pair_params.argtypes = [vp, i32, i32, vp, i32]
+        L.gm_set_bond_params.argtypes = [vp, i32, C.c_float, C.c_float]
+        L.gm_set_particles.argtypes = [vp, vp, vp, vp, vp, i32]
+        L.gm_set_bonds.argtypes = [vp, i64, vp, vp, i32]
+        L.gm_set_step.argtypes = [vp, C.c_uint64]
+        L.gm_build_neighbors.argtypes = [vp]
+        L.gm_compute_forces.argtypes = [vp]
+        L.gm_step.argtypes = [vp, i64]
+        L.gm_energies.argtypes = [vp, vp]
+        L.gm_get_particles.argtypes = [vp, vp, vp, vp, i32]
+        L.gm_get_neighbors.argtypes = [vp, vp, vp, i64, i32]
+        L.gm_get_stats.argtypes = [vp, vp]
+        L.gm_sfc_cell_order.argtypes = [vp, vp]
+        L.gm_last_error.argtypes = [vp]
+        L.gm_last_error.restype = C.c_char_p
+        for name in SYMBOLS[:-1]:
+            getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(status: int, handle=None):
+    if status != GM_OK:
+        msg = lib().gm_last_error(handle).decode() if handle else "(no system)"
+        raise GmError(status, msg)
+
+
+def _ptr(a):
+    """Pointer + residency of a numpy array (host) or torch tensor (host or device)."""
+    if a is None:
+        return None, None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return a.ctypes.data, False
+    assert a.is_contiguous()
+    return a.data_ptr(), a.is_cuda
+
+
+def _same_side(*arrs) -> int:
+    sides = {d for _, d in (_ptr(a) for a in arrs) if d is not None}
+    if len(sides) > 1:
+        raise ValueError("arrays of one call must all be host or all be device")
+    return int(sides.pop()) if sides else 0
+
+
+# ---- one function per entry of include/gm.h ----------------------------------------------------------
+def gm_query_workspace(cfg: gm_config) -> int:
+    out = C.c_size_t(0)
+    _check(lib().gm_query_workspace(C.byref(cfg), C.byref(out)))
+    return int(out.value)
+
+
+def gm_create(cfg: gm_config, workspace) -> int:
+    h = C.c_void_p(0)
+    _check(lib().gm_create(C.byref(cfg), workspace.data_ptr(), workspace.numel() * workspace.element_size(), C.byref(h)))
+    return h.value
+
+
+def gm_destroy(h):
+    _check(lib().gm_destroy(h))
+
+
+def gm_set_pair_params(h, ti: int, tj: int, p):
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    _check(lib().gm_set_pair_params(h, ti, tj, p.ctypes.data, p.size), h)
+
+
+def gm_set_bond_params(h, btype: int, k: float, r0: float):
+    _check(lib().gm_set_bond_params(h, btype, k, r0), h)
+
+
+def gm_set_particles(h, pos3, vel3, type_, mass=None):
+    dev = _same_side(pos3, vel3, type_, mass)
+    _check(lib().gm_set_particles(h, _ptr(pos3)[0], _ptr(vel3)[0], _ptr(type_)[0], _ptr(mass)[0], dev), h)
+
+
+def gm_set_bonds(h, tag_pairs2, btype=None):
+    n = 0 if tag_pairs2 is None else int(tag_pairs2.shape[0])
+    dev = _same_side(tag_pairs2, btype)
+    _check(lib().gm_set_bonds(h, n, _ptr(tag_pairs2)[0], _ptr(btype)[0], dev), h)
+
+
+def gm_set_step(h, step: int):
+    _check(lib().gm_set_step(h, step), h)
+
+
+def gm_build_neighbors(h):
+    _check(lib().gm_build_neighbors(h), h)
+
+
+def gm_compute_forces(h):
+    _check(lib().gm_compute_forces(h), h)
+
+
+def gm_step(h, n_steps: int):
+    _check(lib().gm_step(h, n_steps), h)
+
+
+def gm_energies(h) -> np.ndarray:
+    out = np.zeros(8, dtype=np.float64)
+    _check(lib().gm_energies(h, out.ctypes.data), h)
+    return out
+
+
+def gm_get_particles(h, pos3=None, vel3=None, force3=None):
+    dev = _same_side(pos3, vel3, force3)
+    _check(lib().gm_get_particles(h, _ptr(pos3)[0], _ptr(vel3)[0], _ptr(force3)[0], dev), h)
+
+
+def gm_get_neighbors(h, nn, nl_tags):
+    dev = _same_side(nn, nl_tags)
+    _check(lib().gm_get_neighbors(h, _ptr(nn)[0], _ptr(nl_tags)[0], int(nl_tags.shape[1]), dev), h)
+
+
+def gm_get_stats(h, check: bool = True) -> dict:
+    out = np.zeros(8, dtype=np.int64)
+    st = lib().gm_get_stats(h, out.ctypes.data)
+    if check:
+        _check(st, h)
+    keys = ["steps", "rebuilds", "reorders", "max_nn", "sum_nn", "dev_err", "nl_row_capacity", "n_cells"]
+    d = dict(zip(keys, (int(x) for x in out)))
+    d["status"] = st
+    return d
+
+
+def gm_sfc_cell_order(nc) -> np.ndarray:
+    nc = np.ascontiguousarray(nc, dtype=np.int32)
+    out = np.zeros(int(nc[0]) * int(nc[1]) * int(nc[2]), dtype=np.uint32)
+    _check(lib().gm_sfc_cell_order(nc.ctypes.data, out.ctypes.data))
+    return out
+
+
+# ---- convenience: one object per system ---------------------------------------------------------------
+class System:
+    """Create a gm_system for a workload description and keep its workspace alive.
+
+    `w` needs: n, box, pos, vel, type, mass, bonds, bond_type, n_types, pair_style, pair, bond_style,
+    bond, integrator, dt, kT, gamma, lam, r_skin, seed, sfc_period (see workloads.Workload).
+    """
+
+    def __init__(self, w, device: int = 0, flags: int = 0, nl_row_capacity: int = 0, sfc_period=None,
+                 load: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1310_2041_b200 needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.w = w
+        self.n = int(w.n)
+        self.device = torch.device("cuda", device)
+        cfg = gm_config()
+        cfg.struct_size = C.sizeof(gm_config)
+        cfg.device = device
+        cfg.stream = torch.cuda.current_stream(self.device).cuda_stream
+        cfg.n_particles = self.n
+        cfg.n_types = int(w.n_types)
+        bonds = np.ascontiguousarray(w.bonds, dtype=np.int32).reshape(-1, 2)
+        self.bonds = bonds
+        if len(bonds) and w.bond_style != "none":
+            cfg.max_bonds_per_particle = int(np.bincount(bonds.ravel(), minlength=self.n).max())
+        else:
+            cfg.max_bonds_per_particle = 0
+        for d in range(3):
+            cfg.box[d] = float(w.box[d])
+        pair = w.pair
+        cfg.r_cut_max = float(np.max(pair["rc"])) if w.pair_style != "none" else 1.0
+        cfg.r_skin = float(w.r_skin)
+        cfg.dt = float(w.dt)
+        cfg.seed = int(w.seed)
+        cfg.pair_style = GM_PAIR[w.pair_style]
+        cfg.bond_style = GM_BOND[w.bond_style] if cfg.max_bonds_per_particle else 0
+        cfg.integrator = GM_INTEG[w.integrator]
+        cfg.kT, cfg.gamma, cfg.lam = float(w.kT), float(w.gamma), float(w.lam)
+        cfg.sfc_period = int(w.sfc_period if sfc_period is None else sfc_period)
+        cfg.nl_row_capacity = int(nl_row_capacity)
+        cfg.flags = int(flags)
+        self.cfg = cfg
+        nbytes = gm_query_workspace(cfg)
+        self.workspace_bytes = nbytes
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        off = (-self.workspace.data_ptr()) % 256
+        self._ws_view = self.workspace[off:off + nbytes]
+        self.h = gm_create(cfg, self._ws_view)
+        nt = cfg.n_types
+        for ti in range(nt):
+            for tj in range(ti, nt):
+                if w.pair_style == "lj":
+                    gm_set_pair_params(self.h, ti, tj, [pair["eps"][ti][tj], pair["sigma"][ti][tj],
+                                                        pair["rc"][ti][tj], 1.0 if pair.get("shift", True) else 0.0])
+                elif w.pair_style == "dpd":
+                    gm_set_pair_params(self.h, ti, tj, [pair["a"][ti][tj], pair["rc"][ti][tj]])
+        if cfg.bond_style:
+            for bt in range(len(w.bond["k"])):
+                gm_set_bond_params(self.h, bt, float(w.bond["k"][bt]), float(w.bond["r0"][bt]))
+        if load:
+            self.set_particles(w.pos, w.vel, w.type, w.mass)
+            if cfg.max_bonds_per_particle:
+                gm_set_bonds(self.h, bonds, np.ascontiguousarray(w.bond_type, dtype=np.int32))
+
+    def close(self):
+        if getattr(self, "h", None):
+            gm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # thin forwards
+    def set_particles(self, pos, vel, typ, mass=None):
+        f32 = lambda a: None if a is None else (np.ascontiguousarray(a, dtype=np.float32) if isinstance(a, np.ndarray) else a)
+        typ = np.ascontiguousarray(typ, dtype=np.int32) if isinstance(typ, np.ndarray) else typ
+        gm_set_particles(self.h, f32(pos), f32(vel), typ, f32(mass))
+
+    def build_neighbors(self):
+        gm_build_neighbors(self.h)
+
+    def compute_forces(self):
+        gm_compute_forces(self.h)
+
+    def step(self, n: int):
+        gm_step(self.h, n)
+
+    def energies(self) -> dict:
+        e = gm_energies(self.h)
+        return dict(ke=e[0], pe_pair=e[1], pe_bond=e[2], T=e[3], p=e[4:7].copy(), n_pairs=e[7],
+                    etot=e[0] + e[1] + e[2])
+
+    def get_particles(self, pos=True, vel=True, force=False):
+        out = [np.empty((self.n, 3), np.float32) if f else None for f in (pos, vel, force)]
+        gm_get_particles(self.h, *out)
+        return out
+
+    def neighbors(self):
+        """(nn, nl_tags) on the host; nl_tags has max_nn columns."""
+        gm_build_neighbors(self.h) if self.stats()["max_nn"] == 0 and self.stats()["rebuilds"] == 0 else None
+        stride = max(1, self.stats()["max_nn"])
+        nn = np.zeros(self.n, np.int32)
+        nl = np.zeros((self.n, stride), np.int32)
+        gm_get_neighbors(self.h, nn, nl)
+        return nn, nl
+
+    def stats(self, check: bool = True) -> dict:
+        return gm_get_stats(self.h, check)
+
+    def synchronize(self):
+        self.torch.cuda.current_stream(self.device).synchronize()
