@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py -- timesteps/s and pair-interactions/s of the short-range force pipeline on the
+1,000,000-bead Kremer-Grest melt (BASELINE.json configs[2], "C3"), one B200 per rank.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config C3] [--inner 500]
+
+A bench "step" is one gm_step(inner) call: `inner` MD timesteps of the whole hot path (a1..a8 of
+SURVEY.md section 8(a): displacement test, device-gated cell binning + Verlet-list rebuild, fused
+pair+bond force and velocity-Verlet kernel, and the SFC reorder when it falls due).  The default
+inner = 500 is one SFC period of C3, so every step holds the same mix of rebuilds and one reorder.
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).
+
+--impl reference times the fp64 CPU oracle (oracle/, test infrastructure) on the host cores; each
+of its steps is ONE MD timestep of the same workload (a bounded sample).  Under torchrun only rank
+0 runs it.
+
+Multi-GPU: the path does not shard (single-GPU method, "replicas only"): with
+--gpus N every rank steps an independent replica of the same melt; value is the sum over replicas.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "timesteps/s"
+L2_BYTES = 126e6
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+class ClockSampler(threading.Thread):
+    """SM clock and throttle reasons DURING the timed region (NVML; same fields as the recipe's
+    nvidia-smi clocks line)."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, torch_device):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.max_mhz, self.power = [], set(), None, []
+        self._stop_evt = threading.Event()
+        self.h = None
+        try:
+            import pynvml
+            import torch
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            try:
+                uuid = str(torch.cuda.get_device_properties(torch_device).uuid)
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(("GPU-" + uuid) if not uuid.startswith("GPU-") else uuid)
+            except Exception:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+                idx = torch_device.index or 0
+                if vis:
+                    idx = int(vis.split(",")[idx])
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:          # no NVML: the clocks record says so instead of inventing numbers
+            self.err = repr(e)
+            self.h = None
+
+    def run(self):
+        if self.h is None:
+            return
+        nv = self.nv
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)) if hasattr(nv, "nvmlDeviceGetCurrentClocksEventReasons") \
+                    else int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def stop(self) -> dict:
+        self._stop_evt.set()
+        if self.h is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"]}
+        self.join(timeout=2)
+        s = self.samples[1:] if len(self.samples) > 2 else self.samples
+        return {"sm_mhz": float(np.median(s)) if s else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s),
+                "power_w_max": round(max(self.power), 1) if self.power else None}
+
+
+def oracle_timesteps(w, n_steps, n_threads):
+    """Time n_steps MD timesteps of the oracle as it stands (cell-list mode, OpenMP over beads)."""
+    from oracle import oracle as orc
+    o = orc.Oracle(w, use_cells=True, n_threads=n_threads)
+    o.compute_forces()
+    o.run(1)                                    # warm-up (page faults, thread pool)
+    t0 = time.perf_counter()
+    o.run(n_steps)
+    dt = time.perf_counter() - t0
+    return dt, orc.lib().orc_num_threads() if n_threads <= 0 else n_threads
+
+
+def run_reference(args, w):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    cores = os.cpu_count() or 1
+    o = orc.Oracle(w, use_cells=True, n_threads=cores)
+    o.compute_forces()
+    if w.equil_steps:
+        pass    # the oracle is timed at the start state: per-timestep cost does not depend on the thermostat
+    for _ in range(args.warmup):
+        o.run(1)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.run(1)
+    dt = time.perf_counter() - t0
+    tps = args.steps / dt
+    sample = f"{args.steps} single MD timesteps of {w.name} (N={w.n}), fp64 cell-list oracle, OpenMP"
+    line = {
+        "impl": "reference", "metric": METRIC, "value": tps, "unit": "timesteps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": describe(w), "timesteps_per_step": 1},
+        "cpu_baseline": {"value": tps, "unit": "timesteps/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": tps, "unit": "timesteps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def describe(w) -> str:
+    rc = float(np.max(w.pair["rc"]))
+    return (f"{w.name}: {w.n} beads, chains of {w.chain_len}, box {float(w.box[0]):.3f}, {w.pair_style} rc={rc:.4f}, "
+            f"{w.bond_style} bonds, {w.integrator}, dt={w.dt}, skin={w.r_skin}, sfc_period={w.sfc_period}")
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="C3")
+    ap.add_argument("--scale", type=float, default=None, help="shrink the config (debugging only)")
+    ap.add_argument("--inner", type=int, default=0, help="MD timesteps per bench step (0: one SFC period)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+
+    from workloads import make_config
+    w = make_config(args.config, scale=args.scale)
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1310_2041_b200 import gm
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    inner = args.inner or (w.sfc_period if w.sfc_period > 0 else 500)
+    hbm_gbs, peak_src = load_peaks()
+
+    # ---- set-up (untimed): the config's own protocol -----------------------------------------------
+    first = "langevin" if w.equil_steps else w.integrator
+    w_run = w
+    if w.equil_steps:
+        import copy
+        w_run = copy.copy(w)
+        w_run.integrator = "langevin"
+    s = gm.System(w_run, device=local)
+    if w.equil_steps:
+        s.step(w.equil_steps)                   # C3: 1,000 Langevin steps (kT=1, gamma=1), then NVE
+        s.set_integrator(w.integrator, w.kT, 0.0)
+    st0 = s.stats()
+    stream = torch.cuda.current_stream(dev)
+
+    # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------
+    for _ in range(args.warmup):
+        s.step(inner)
+    barrier()
+    st1 = s.stats()
+    clocks = ClockSampler(dev)
+    clocks.start()
+    time.sleep(0.05)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        s.step(inner)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop()
+    st2 = s.stats()
+    if world > 1:
+        t = torch.tensor([ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    n_ts = args.steps * inner
+    tps = world * n_ts / (ms * 1e-3)
+    rebuilds = st2["rebuilds"] - st1["rebuilds"]
+    reorders = st2["reorders"] - st1["reorders"]
+    nbar_l = st2["sum_nn"] / w.n
+    bbar = 2.0 * len(w.bonds) / w.n
+    en = s.energies()
+    pairs_in_rc = en["n_pairs"]
+
+    # kernels launched inside the timed region: per timestep the gate + the fused force/integrate kernel;
+    # per rebuild 8 (clear, keys, 3 scan, scatter, cell finish, NL build); per reorder the counting sort
+    # (7) + 5 permute/copy kernels + bond remap + an ungated rebuild (already counted in `rebuilds`)
+    launches = n_ts * 2 + rebuilds * 8 + reorders * 13
+
+    # ---- the dominant kernel alone: CUDA events around every launch (gm_step_timed) ----------------
+    n_prof = min(inner, 200)
+    tk = s.step_timed(n_prof)
+    k_ms = tk["force_ms"] / max(1, tk["force_launches"])
+    dpd = w.pair_style == "dpd"
+    bytes_kernel = w.n * ((48 + 48 if dpd else 32 + 32) + 16 + 4 + 4 * nbar_l + 4 + 4 * bbar)
+    m_interval = n_ts / max(1, rebuilds)
+    bytes_step = bytes_kernel + w.n * (80 + 4 * nbar_l) / m_interval
+    achieved = bytes_kernel / (k_ms * 1e-3) / 1e9
+    ms_ts = ms / n_ts
+    roof = {"bound": "hbm", "kernel": "k_force<STEP> (fused a4+a5+a7+a8)", "achieved": achieved, "peak": hbm_gbs,
+            "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None, "peak_source": peak_src,
+            "kernel_ms": k_ms, "algorithmic_bytes_per_launch": bytes_kernel,
+            "kernel_share_of_step": k_ms / ms_ts,
+            "whole_step": {"algorithmic_bytes_per_timestep": bytes_step, "achieved": bytes_step / (ms_ts * 1e-3) / 1e9,
+                           "frac": bytes_step / (ms_ts * 1e-3) / 1e9 / hbm_gbs,
+                           "frac_of_nominal_8TBs": bytes_step / (ms_ts * 1e-3) / 1e9 / 8000.0}}
+    tr = os.path.join(ROOT, "profiles", "traffic_r01.json")     # dram bytes/launch from the ncu --set full capture
+    if os.path.exists(tr):
+        with open(tr) as f:
+            roof["traffic"] = json.load(f).get(args.config)
+
+    # ---- end to end through the C ABI with HOST buffers ---------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        n = w.n
+        hp = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+        hv = torch.empty((n, 3), dtype=torch.float32).pin_memory()
+        ht = torch.from_numpy(np.ascontiguousarray(w.type, np.int32)).pin_memory()
+        gm.gm_get_particles(s.h, hp, hv, None)
+        k_e2e = max(2, min(args.steps, 5))
+        for _ in range(1):
+            gm.gm_set_particles(s.h, hp, hv, ht, None); s.step(inner); gm.gm_get_particles(s.h, hp, hv, None)
+        barrier()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(k_e2e):
+            gm.gm_set_particles(s.h, hp, hv, ht, None)      # H2D: pos, vel, type (pinned host memory)
+            s.step(inner)
+            gm.gm_get_particles(s.h, hp, hv, None)          # D2H: pos, vel; synchronises
+        e1.record(stream)
+        barrier()
+        ms_e = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms_e], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e = float(t.item())
+        e2e = {"value": world * k_e2e * inner / (ms_e * 1e-3), "unit": "timesteps/s",
+               "h2d_bytes_per_step": n * (12 + 12 + 4), "d2h_bytes_per_step": n * 24, "steps": k_e2e,
+               "what": "gm_set_particles(host) + gm_step(inner) + gm_get_particles(host) per step"}
+
+    # ---- the oracle beside it (rank 0, N=1 only) ----------------------------------------------------
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cores = os.cpu_count() or 1
+        t1, _ = oracle_timesteps(w, 1, cores)
+        k = int(max(2, min(50, 15.0 / max(t1, 1e-3))))
+        tt, thr = oracle_timesteps(w, k, cores)
+        cpu = {"value": k / tt, "unit": "timesteps/s", "cores": thr, "kind": "oracle",
+               "sample": f"{k} MD timesteps of {w.name} (N={w.n}) from the start state, fp64 cell-list oracle, OpenMP over beads"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": tps, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": describe(w), "timesteps_per_step": inner, "parallelism": f"replicas x{world}",
+                       "l2": f"no flush: successive timesteps are data-dependent; per-timestep working set "
+                             f"{(bytes_kernel + 16 * w.n) / 1e6:.0f} MB vs L2 {L2_BYTES / 1e6:.0f} MB",
+                       "equilibration": f"{w.equil_steps} Langevin steps (untimed set-up)" if w.equil_steps else "none"},
+            "ms_per_timestep": ms_ts,
+            "pair_interactions_per_s": tps * pairs_in_rc,
+            "list_entries_per_s": tps * st2["sum_nn"],
+            "pairs_in_rc": pairs_in_rc, "mean_nn": nbar_l, "max_nn": st2["max_nn"],
+            "rebuilds": rebuilds, "rebuild_interval": m_interval, "reorders": reorders,
+            "rebuild_ms_per_timestep_direct": tk["rebuild_ms"] / max(1, tk["force_launches"]),
+            "energy_per_bead": en["etot"] / w.n, "temperature": en["T"],
+            "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
+        }
+        print(json.dumps(line))
+    s.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

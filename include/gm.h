@@ -145,6 +145,20 @@ gm_status gm_compute_forces(gm_system *s);
  * Asynchronous on the stream.  Errors: STATE, INVALID_ARG (n_steps < 0), CUDA. */
 gm_status gm_step(gm_system *s, int64_t n_steps);
 
+/* Switch the integrator of an existing system (e.g. Langevin equilibration, then NVE: BASELINE.json
+ * config 3).  integrator: GM_NVE | GM_LANGEVIN (GM_DPD_GWVV only on a GM_PAIR_DPD system and vice
+ * versa); kT, gamma as in gm_config.  The state (positions, half-step velocities, step counter,
+ * neighbor list) is kept.  Errors: INVALID_ARG. */
+gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma);
+
+/* Measurement aid: n_steps timesteps exactly as gm_step would take them, but launched kernel by
+ * kernel (no CUDA graph) with CUDA events on the system's stream around the fused force+integrate
+ * kernel (a4..a8) and around the rebuild kernels (a1 + a3; early-exit when no rebuild is due).
+ * out (HOST, 4 doubles): summed device ms of the force+integrate launches, summed device ms of the
+ * rebuild launches, number of force+integrate launches, number of SFC reorders done inside.
+ * Synchronises.  Same results, bit for bit, as gm_step. */
+gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4]);
+
 /* out (HOST, 8 doubles): kinetic energy, pair PE, bond PE, temperature (3N-3 dof), px, py, pz,
  * number of unique pairs inside r_cut.  fp32 terms, fp64 sums.  Synchronises. */
 gm_status gm_energies(gm_system *s, double out[8]);

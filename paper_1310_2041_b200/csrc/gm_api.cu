@@ -537,17 +537,20 @@ extern "C" gm_status gm_compute_forces(gm_system *s)
     return GM_OK;
 }
 
-extern "C" gm_status gm_step(gm_system *s, int64_t n_steps)
+struct StepTiming {
+    std::vector<cudaEvent_t> ev;     // 3 per step: before rebuild, before force, after force
+    int64_t reorders;
+};
+
+static gm_status step_impl(gm_system *s, int64_t n_steps, StepTiming *tm)
 {
-    if (!s) return GM_ERR_INVALID_ARG;
-    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_step: no particles set%s");
-    if (n_steps < 0) return fail(s, GM_ERR_INVALID_ARG, "gm_step: n_steps < 0%s");
-    CU(cudaSetDevice(s->cfg.device));
     int64_t left = n_steps;
     while (left > 0) {
         if (!s->nl_valid || reorder_due(s) || s->bonds_dirty) {
+            const int64_t r0 = s->n_reorders;
             gm_status r = ensure_list(s);
             if (r != GM_OK) return r;
+            if (tm) tm->reorders += s->n_reorders - r0;
         }
         int64_t chunk = left;
         if (s->cfg.sfc_period > 0) {
@@ -558,7 +561,7 @@ extern "C" gm_status gm_step(gm_system *s, int64_t n_steps)
         int64_t done = 0;
         while (done < chunk) {
             const int64_t rem = chunk - done;
-            if (s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
+            if (!tm && s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
                 const bool big = rem >= GM_GRAPH_STEPS;
                 cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
                 const int ns = big ? GM_GRAPH_STEPS : 2;
@@ -568,8 +571,15 @@ extern "C" gm_status gm_step(gm_system *s, int64_t n_steps)
                 done += ns;
                 s->step += (uint64_t)ns;
             } else {
+                cudaEvent_t e[3] = { nullptr, nullptr, nullptr };
+                if (tm) {
+                    for (int q = 0; q < 3; ++q) { CU(cudaEventCreate(&e[q])); tm->ev.push_back(e[q]); }
+                    CU(cudaEventRecord(e[0], s->st));
+                }
                 enqueue_rebuild(s, 1, s->st);
+                if (tm) CU(cudaEventRecord(e[1], s->st));
                 enqueue_step_kernel(s, s->lagged, s->st);
+                if (tm) CU(cudaEventRecord(e[2], s->st));
                 s->lagged = true;
                 done += 1;
                 s->step += 1;
@@ -579,6 +589,56 @@ extern "C" gm_status gm_step(gm_system *s, int64_t n_steps)
     }
     CU(cudaGetLastError());
     if (n_steps > 0) s->force_current = false;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_step(gm_system *s, int64_t n_steps)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_step: no particles set%s");
+    if (n_steps < 0) return fail(s, GM_ERR_INVALID_ARG, "gm_step: n_steps < 0%s");
+    CU(cudaSetDevice(s->cfg.device));
+    return step_impl(s, n_steps, nullptr);
+}
+
+extern "C" gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4])
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_step_timed: no particles set%s");
+    if (n_steps < 0 || n_steps > 100000 || !out) return fail(s, GM_ERR_INVALID_ARG, "gm_step_timed: bad arguments%s");
+    CU(cudaSetDevice(s->cfg.device));
+    StepTiming tm;
+    tm.reorders = 0;
+    gm_status r = step_impl(s, n_steps, &tm);
+    cudaError_t e = cudaStreamSynchronize(s->st);
+    double t_force = 0.0, t_rebuild = 0.0;
+    for (size_t k = 0; k + 2 < tm.ev.size() + 0 && e == cudaSuccess; k += 3) {
+        float a = 0.f, b = 0.f;
+        e = cudaEventElapsedTime(&a, tm.ev[k], tm.ev[k + 1]);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&b, tm.ev[k + 1], tm.ev[k + 2]);
+        t_rebuild += a; t_force += b;
+    }
+    for (cudaEvent_t ev : tm.ev) cudaEventDestroy(ev);
+    if (r != GM_OK) return r;
+    if (e != cudaSuccess) return fail(s, GM_ERR_CUDA, "CUDA: %s", cudaGetErrorString(e));
+    out[0] = t_force; out[1] = t_rebuild; out[2] = (double)(tm.ev.size() / 3); out[3] = (double)tm.reorders;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (integrator < GM_NVE || integrator > GM_DPD_GWVV)
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: unknown integrator%s");
+    if ((integrator == GM_DPD_GWVV) != (s->P.pair_style == GM_PAIR_DPD))
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: GM_DPD_GWVV goes with GM_PAIR_DPD only%s");
+    if (!(kT >= 0.f) || !(gamma >= 0.f)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: kT, gamma must be >= 0%s");
+    s->cfg.integrator = integrator; s->cfg.kT = kT; s->cfg.gamma = gamma;
+    s->P.integrator = integrator; s->P.kT = kT; s->P.gamma = gamma;
+    s->P.sigma_r_sqrt_inv_dt = (float)std::sqrt(2.0 * (double)gamma * (double)kT / (double)s->P.dt);
+    s->P.lang_amp2 = (float)(6.0 * (double)gamma * (double)kT / (double)s->P.dt);
+    s->force_current = false;
+    drop_graphs(s);
     return GM_OK;
 }
 

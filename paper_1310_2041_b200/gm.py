@@ -26,7 +26,7 @@ GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES = 1, 2
 
 SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_bond_params",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
-           "gm_step", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
+           "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
            "gm_sfc_cell_order", "gm_last_error"]
 
 
@@ -72,6 +72,8 @@ def lib():
         L.gm_build_neighbors.argtypes = [vp]
         L.gm_compute_forces.argtypes = [vp]
         L.gm_step.argtypes = [vp, i64]
+        L.gm_step_timed.argtypes = [vp, i64, vp]
+        L.gm_set_integrator.argtypes = [vp, i32, C.c_float, C.c_float]
         L.gm_energies.argtypes = [vp, vp]
         L.gm_get_particles.argtypes = [vp, vp, vp, vp, i32]
         L.gm_get_neighbors.argtypes = [vp, vp, vp, i64, i32]
@@ -160,6 +162,16 @@ def gm_compute_forces(h):
 
 def gm_step(h, n_steps: int):
     _check(lib().gm_step(h, n_steps), h)
+
+
+def gm_step_timed(h, n_steps: int) -> np.ndarray:
+    out = np.zeros(4, dtype=np.float64)
+    _check(lib().gm_step_timed(h, n_steps, out.ctypes.data), h)
+    return out
+
+
+def gm_set_integrator(h, integrator: int, kT: float, gamma: float):
+    _check(lib().gm_set_integrator(h, integrator, kT, gamma), h)
 
 
 def gm_energies(h) -> np.ndarray:
@@ -287,6 +299,13 @@ class System:
 
     def step(self, n: int):
         gm_step(self.h, n)
+
+    def step_timed(self, n: int) -> dict:
+        t = gm_step_timed(self.h, n)
+        return dict(force_ms=t[0], rebuild_ms=t[1], force_launches=int(t[2]), reorders=int(t[3]))
+
+    def set_integrator(self, name: str, kT: float = 1.0, gamma: float = 0.0):
+        gm_set_integrator(self.h, GM_INTEG[name], kT, gamma)
 
     def energies(self) -> dict:
         e = gm_energies(self.h)

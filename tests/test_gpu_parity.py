@@ -273,7 +273,7 @@ def test_edge_cases(gm):
     assert s.stats(check=False)["status"] == gm.GM_ERR_BOND_OVERSTRETCH
     s.close()
     # neighbor row overflow is latched and reported
-    w = make_random_box(500, [6.0, 6.0, 6.0], seed=2)
+    w = make_random_box(1500, [9.0, 9.0, 9.0], seed=2)              # ~ 210 neighbors per bead at r_list 2.9
     s = gm.System(w, nl_row_capacity=8)
     s.build_neighbors()
     assert s.stats(check=False)["status"] == gm.GM_ERR_NEIGHBOR_OVERFLOW
