@@ -160,6 +160,9 @@ def main():
     ap.add_argument("--config", default="C3")
     ap.add_argument("--scale", type=float, default=None, help="shrink the config (debugging only)")
     ap.add_argument("--inner", type=int, default=0, help="MD timesteps per bench step (0: one SFC period)")
+    ap.add_argument("--no-cond-nodes", action="store_true",
+                    help="gate the rebuild with early-exit kernels instead of a conditional graph node "
+                         "(ncu cannot profile kernel nodes of graphs that hold conditional nodes)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -201,7 +204,7 @@ def main():
         import copy
         w_run = copy.copy(w)
         w_run.integrator = "langevin"
-    s = gm.System(w_run, device=local)
+    s = gm.System(w_run, device=local, flags=gm.GM_FLAG_NO_COND_NODES if args.no_cond_nodes else 0)
     if w.equil_steps:
         s.step(w.equil_steps)                   # C3: 1,000 Langevin steps (kT=1, gamma=1), then NVE
         s.set_integrator(w.integrator, w.kT, 0.0)
