@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <new>
 #include <vector>
 
@@ -56,6 +57,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
+    P->ns = (P->n + GM_PAD - 1) / GM_PAD * GM_PAD;
     P->n_types = c->n_types;
     P->max_bonds = c->max_bonds_per_particle;
     const double r_list = (double)c->r_cut_max + (double)c->r_skin;
@@ -91,7 +93,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     int cap = c->nl_row_capacity;
     if (cap <= 0) {
         double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
-        cap = (int)(2.0 * nbar) + 32;
+        cap = (int)(1.5 * nbar) + 32;
     }
     cap = (cap + 7) / 8 * 8;
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
@@ -109,7 +111,7 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
         off += align_up(bytes);
         return p;
     };
-    const size_t n = (size_t)P.n;
+    const size_t n = (size_t)P.ns;      // padded: whole tiles of GM_PAD beads can be bulk-copied
     GmDev d;
     memset(&d, 0, sizeof(d));
     d.ctl = (GmCtl *)take(sizeof(GmCtl));
@@ -122,6 +124,7 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     d.tmp4 = (float4 *)take(n * 16);
     d.tag = (int *)take(n * 4); d.rtag = (int *)take(n * 4);
     d.nn = (int *)take(n * 4);
+    d.nnw = (int *)take(n / 32 * 4);
     d.nl = (int *)take(n * 4 * (size_t)P.nl_cap);
     if (P.max_bonds > 0) {
         d.bn = (int *)take(n * 4); d.bl = (int *)take(n * 4 * (size_t)P.max_bonds);
@@ -179,6 +182,7 @@ extern "C" gm_status gm_sfc_cell_order(const int32_t nc[3], uint32_t *rank_out)
             }
     std::sort(v.begin(), v.end());
     for (size_t r = 0; r < ncell; ++r) rank_out[v[r].second] = (uint32_t)r;
+    if (getenv("GM_EXP_LINEAR")) for (size_t r = 0; r < ncell; ++r) rank_out[r] = (uint32_t)r;
     return GM_OK;
 }
 

@@ -32,7 +32,7 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, con
 {
     const int nn = D.nn[i];
     const int *__restrict__ nl = D.nl + i;
-    const size_t n = (size_t)P.n;
+    const size_t n = (size_t)P.ns;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
     const GmPair p0 = P.pair[0];
     for (int k = 0; k < nn; ++k) {
@@ -92,7 +92,7 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
     float pe = 0.f;
     if (P.max_bonds > 0 && P.bond_style != GM_BOND_NONE) {
         const int nb = D.bn[i];
-        const size_t n = (size_t)P.n;
+        const size_t n = (size_t)P.ns;
         for (int k = 0; k < nb; ++k) {
             const int e = D.bl[(size_t)k * n + i];
             const int j = e & GM_BOND_MASK, bt = (unsigned)e >> GM_BOND_SHIFT;

@@ -7,9 +7,9 @@
 //   vt[2]   float4[N]  v~_x, v~_y, v~_z, tag (int bits)  DPD only: the velocity the dissipative force sees
 //   frc     float4[N]  F_x, F_y, F_z, per-bead PE        materialised only by gm_compute_forces
 //   ref     float4[N]  position at the last NL build     (displacement test a4)
-//   nl      int[cap*N] NL[k*N + i], column-major table   PAPER.md:L51, Fig. 1
+//   nl      int[cap*ns] NL[k*ns + i], column-major table, ns = N rounded up to GM_PAD   PAPER.md:L51, Fig. 1
 //   nn      int[N]     NN[i]
-//   bl      int[mb*N]  BL[k*N + i] = j | btype << 28     PAPER.md:L97, Fig. 2 (index space)
+//   bl      int[mb*ns] BL[k*ns + i] = j | btype << 28    PAPER.md:L97, Fig. 2 (index space)
 //   bn      int[N]
 //   cpos    float4[N]  x, y, z, storage index            cell list CL in CSR form
 //   cstart  int[n_cells + 1]                             replaces CN: cell c holds cpos[cstart[c] .. cstart[c+1])
@@ -19,6 +19,7 @@
 
 #include "../../include/gm.h"
 
+#define GM_PAD 256               // per-bead arrays are allocated (and table rows strided) in multiples of this
 #define GM_BOND_SHIFT 28
 #define GM_BOND_MASK ((1 << GM_BOND_SHIFT) - 1)
 
@@ -44,6 +45,7 @@ struct GmPair { float c0, c1, c2, c3; };
 // Constants of one system, passed to kernels by value (constant bank).
 struct GmParams {
     int n, n_types, max_bonds, nl_cap;
+    int ns;                        // row stride of the NL and BL tables: n rounded up to GM_PAD elements
     int nc[3], n_cells;
     float box[3], half[3], inv_w[3];
     float r_list2, half_skin2;
@@ -66,6 +68,7 @@ struct GmDev {
     float4 *ref;
     int *tag, *rtag;
     int *nn, *nl;
+    int *nnw;                // max of NN over each group of 32 consecutive beads (tile height for the bulk loads)
     int *bn, *bl;            // index space
     int *bn_tag, *bl_tag;    // tag space master copy (bl_tag[k*N + tag] = partner tag | btype << 28)
     int *key, *rank, *sorted;

@@ -11,68 +11,95 @@
 
 #define NL_BLOCK 128
 
+// One row piece: candidates cpos[s0 .. s1) against bead i.  SHIFT: the piece lies across a periodic face
+// in some dimension; the displacement is then taken relative to the two faces, (a -+ L/2) - (b +- L/2)
+// (see gm_min_image), with the bead side (ax, ay, az) prepared once per piece and the candidate side
+// b + (hx, hy, hz) per candidate -- no branches in the loop.
+template <bool SHIFT>
+__device__ __forceinline__ int nl_scan_piece(const float4 *__restrict__ cpos, int s0, int s1, int i, float ax,
+                                             float ay, float az, float hx, float hy, float hz, float r_list2,
+                                             int k, int cap, int *__restrict__ col, size_t col_stride)
+{
+#pragma unroll 4
+    for (int s = s0; s < s1; ++s) {
+        const float4 q = cpos[s];
+        float dx, dy, dz;
+        if (SHIFT) { dx = ax - (q.x + hx); dy = ay - (q.y + hy); dz = az - (q.z + hz); }
+        else { dx = ax - q.x; dy = ay - q.y; dz = az - q.z; }
+        const float r2 = dx * dx + dy * dy + dz * dz;
+        const int j = __float_as_int(q.w);
+        if (r2 < r_list2 && j != i) {
+            if (k < cap) col[(size_t)k * col_stride] = j;
+            ++k;
+        }
+    }
+    return k;
+}
+
+// Thread s owns the bead in slot s of the cell-sorted array cpos[] (not storage bead s): the 32 beads
+// of a warp then sit in a few consecutive cells of one x row, so at every loop iteration the lanes read
+// the same or adjacent candidates (few L1 wavefronts per request) and run nearly equal trip counts.
 __global__ void __launch_bounds__(NL_BLOCK)
-k_nl_build(const __grid_constant__ GmParams P, GmDev D, const float4 *__restrict__ pos, int gate, int parity)
+k_nl_build(const __grid_constant__ GmParams P, GmDev D, int gate, int parity)
 {
     if (gate && D.ctl->need != D.ctl->step[parity]) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t ns = (size_t)P.ns;
+    const int cap = P.nl_cap;
     int k = 0;
-    if (i < P.n) {
-        const float4 pi = pos[i];
+    if (s < P.n) {
+        const float4 *__restrict__ cpos = D.cpos;
+        const int *__restrict__ cstart = D.cstart;
+        const float4 pi = cpos[s];
+        const int i = __float_as_int(pi.w);
+        int *__restrict__ col = D.nl + i;
         const int cx = gm_cell_coord(pi.x, P.half[0], P.inv_w[0], P.nc[0]);
         const int cy = gm_cell_coord(pi.y, P.half[1], P.inv_w[1], P.nc[1]);
         const int cz = gm_cell_coord(pi.z, P.half[2], P.inv_w[2], P.nc[2]);
         const int ncx = P.nc[0], ncy = P.nc[1], ncz = P.nc[2];
-        const float4 *__restrict__ cpos = D.cpos;
-        const int *__restrict__ cstart = D.cstart;
-        int *__restrict__ nl = D.nl + i;
-        const size_t n = (size_t)P.n;
-        const int cap = P.nl_cap;
-        // x pieces of a row: [x0, x1] contiguous, plus a wrapped single cell when cx is at an edge
-        int xa0 = max(cx - 1, 0), xa1 = min(cx + 1, ncx - 1);
-        int xb = (cx == 0) ? ncx - 1 : ((cx == ncx - 1) ? 0 : -1);
-        for (int oz = -1; oz <= 1; ++oz) {
-            int z = cz + oz;
-            z = (z < 0) ? z + ncz : ((z >= ncz) ? z - ncz : z);
-            for (int oy = -1; oy <= 1; ++oy) {
-                int y = cy + oy;
-                y = (y < 0) ? y + ncy : ((y >= ncy) ? y - ncy : y);
-                int row = (z * ncy + y) * ncx;
-#pragma unroll 1
-                for (int piece = 0; piece < 2; ++piece) {
-                    int s0, s1;
-                    if (piece == 0) { s0 = cstart[row + xa0]; s1 = cstart[row + xa1 + 1]; }
-                    else {
-                        if (xb < 0) break;
-                        s0 = cstart[row + xb]; s1 = cstart[row + xb + 1];
-                    }
-                    for (int s = s0; s < s1; ++s) {
-                        float4 q = cpos[s];
-                        int j = __float_as_int(q.w);
-                        float dx = gm_min_image(pi.x, q.x, P.half[0]);
-                        float dy = gm_min_image(pi.y, q.y, P.half[1]);
-                        float dz = gm_min_image(pi.z, q.z, P.half[2]);
-                        float r2 = dx * dx + dy * dy + dz * dz;
-                        if (r2 < P.r_list2 && j != i) {
-                            if (k < cap) nl[(size_t)k * n] = j;
-                            ++k;
-                        }
-                    }
+        const float rl2 = P.r_list2;
+        // x pieces of a row: cells [xa0, xa1] are contiguous in cpos; a bead in an edge column also
+        // sees the single cell xb on the other side of the box
+        const int xa0 = max(cx - 1, 0), xa1 = min(cx + 1, ncx - 1);
+        const int xb = (cx == 0) ? ncx - 1 : ((cx == ncx - 1) ? 0 : -1);
+        const float hxb = (cx == 0) ? -P.half[0] : P.half[0];       // candidate side of the wrapped x piece
+        const bool inner = cx > 0 && cx < ncx - 1 && cy > 0 && cy < ncy - 1 && cz > 0 && cz < ncz - 1;
+        if (inner) {
+            for (int oz = -1; oz <= 1; ++oz)
+                for (int oy = -1; oy <= 1; ++oy) {
+                    const int row = ((cz + oz) * ncy + cy + oy) * ncx;
+                    k = nl_scan_piece<false>(cpos, cstart[row + xa0], cstart[row + xa1 + 1], i, pi.x, pi.y, pi.z,
+                                             0.f, 0.f, 0.f, rl2, k, cap, col, ns);
+                }
+        } else {
+            for (int oz = -1; oz <= 1; ++oz) {
+                int z = cz + oz;
+                float az = pi.z, hz = 0.f;
+                if (z < 0) { z += ncz; az = pi.z + P.half[2]; hz = -P.half[2]; }
+                else if (z >= ncz) { z -= ncz; az = pi.z - P.half[2]; hz = P.half[2]; }
+                for (int oy = -1; oy <= 1; ++oy) {
+                    int y = cy + oy;
+                    float ay = pi.y, hy = 0.f;
+                    if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
+                    else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
+                    const int row = (z * ncy + y) * ncx;
+                    k = nl_scan_piece<true>(cpos, cstart[row + xa0], cstart[row + xa1 + 1], i, pi.x, ay, az,
+                                            0.f, hy, hz, rl2, k, cap, col, ns);
+                    if (xb >= 0)
+                        k = nl_scan_piece<true>(cpos, cstart[row + xb], cstart[row + xb + 1], i, pi.x - hxb, ay, az,
+                                                hxb, hy, hz, rl2, k, cap, col, ns);
                 }
             }
         }
-        D.nn[i] = min(k, cap);
-        D.ref[i] = pi;
+        const int kc = min(k, cap);
+        D.nn[i] = kc;
+        D.ref[i] = make_float4(pi.x, pi.y, pi.z, 0.f);
+        atomicMax(&D.nnw[i >> 5], kc);     // tile height for the step kernel's bulk loads (cleared in k_sort_clear)
         if (k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
     }
-    // list statistics (off the force path): max and sum of NN
-    int m = k;
-    unsigned int sum = (unsigned int)k;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        m = max(m, __shfl_xor_sync(0xffffffffu, m, o));
-        sum += __shfl_xor_sync(0xffffffffu, sum, o);
-    }
+    const int kc = min(k, cap);
+    const int m = __reduce_max_sync(0xffffffffu, kc);
+    const unsigned int sum = __reduce_add_sync(0xffffffffu, (unsigned int)kc);
     if ((threadIdx.x & 31) == 0 && sum > 0) {
         atomicMax(&D.ctl->max_nn, m);
         atomicAdd(&D.ctl->sum_nn, (unsigned long long)sum);
@@ -83,7 +110,8 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D, const float4 *__restrict
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, const float4 *pos, int gate, int parity,
                         cudaStream_t st)
 {
-    k_nl_build<<<(P.n + NL_BLOCK - 1) / NL_BLOCK, NL_BLOCK, 0, st>>>(P, D, pos, gate, parity);
+    (void)pos;
+    k_nl_build<<<(P.n + NL_BLOCK - 1) / NL_BLOCK, NL_BLOCK, 0, st>>>(P, D, gate, parity);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors): nn_out[tag], nl_out[tag*stride + k].
@@ -96,7 +124,7 @@ k_unpack_neighbors(GmParams P, GmDev D, int *__restrict__ nn_out, int *__restric
     int nn = D.nn[i];
     nn_out[t] = nn;
     for (int k = 0; k < nn && k < stride; ++k)
-        nl_out[(long long)t * stride + k] = D.tag[D.nl[(size_t)k * P.n + i]];
+        nl_out[(long long)t * stride + k] = D.tag[D.nl[(size_t)k * P.ns + i]];
 }
 
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,

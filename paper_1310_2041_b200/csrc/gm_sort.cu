@@ -24,6 +24,8 @@ k_sort_clear(GmParams P, GmDev D, int use_sfc_rank, int gate, int parity)
     if (gm_gated_off(D.ctl, gate, parity)) return;
     int stride = gridDim.x * blockDim.x;
     for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= P.n_cells; c += stride) D.cstart[c] = 0;
+    if (!use_sfc_rank)
+        for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < P.ns / 32; c += stride) D.nnw[c] = 0;
     if (!use_sfc_rank && blockIdx.x == 0 && threadIdx.x == 0) {
         D.ctl->n_rebuilds += 1;
         D.ctl->max_nn = 0;
@@ -237,7 +239,7 @@ __global__ void __launch_bounds__(SORT_BLOCK) k_bonds_to_index(GmParams P, GmDev
     D.bn[i] = nb;
     for (int k = 0; k < nb; ++k) {
         int e = D.bl_tag[(size_t)k * P.n + t];
-        D.bl[(size_t)k * P.n + i] = D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK);
+        D.bl[(size_t)k * P.ns + i] = D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK);
     }
 }
 
