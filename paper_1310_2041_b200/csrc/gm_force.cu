@@ -25,81 +25,114 @@ struct BeadForce {
     float cnt;                // partners inside r_cut
 };
 
+// One in-range test + force term of the pair loop (Alg. 2: displacement, cutoff test, accumulate).
+template <int PAIR, bool NT1, bool ENERGY, bool MI>
+__device__ __forceinline__ void pair_term(const GmParams &P, const float4 pi, const int ti, const float4 vti,
+                                          const float4 pj, const float4 vtj, const GmPair p0, uint32_t step,
+                                          float &fx, float &fy, float &fz, float &pe, float &cnt)
+{
+    float dx, dy, dz;
+    if (MI) {
+        dx = gm_min_image(pi.x, pj.x, P.half[0]);
+        dy = gm_min_image(pi.y, pj.y, P.half[1]);
+        dz = gm_min_image(pi.z, pj.z, P.half[2]);
+    } else {
+        dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
+    }
+    const float r2 = dx * dx + dy * dy + dz * dz;
+    GmPair c = p0;
+    if (!NT1) c = P.pair[ti * P.n_types + __float_as_int(pj.w)];
+    if (r2 < c.c0) {
+        if (PAIR == GM_PAIR_LJ) {
+            // F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij
+            const float r2i = gm_rcp(r2);
+            const float r6i = r2i * r2i * r2i;
+            const float fs = r2i * r6i * (c.c1 * r6i - c.c2);
+            fx += fs * dx; fy += fs * dy; fz += fs * dz;
+            if (ENERGY) {
+                pe += r6i * (c.c1 * (1.0f / 12.0f) * r6i - c.c2 * (1.0f / 6.0f)) - c.c3;
+                cnt += 1.0f;
+            }
+        } else if (PAIR == GM_PAIR_DPD) {
+            if (ENERGY) cnt += 1.0f;
+            if (r2 >= 1e-12f) {
+                // F_ij = [a w - gamma w^2 (e.v_ij) + sigma_R w theta / sqrt(dt)] e,  w = 1 - r/r_c
+                const float ri = rsqrtf(r2);
+                const float r = r2 * ri;
+                const float w = 1.0f - r * c.c2;
+                const float edv = (dx * (vti.x - vtj.x) + dy * (vti.y - vtj.y) + dz * (vti.z - vtj.z)) * ri;
+                const uint32_t ta = (uint32_t)__float_as_int(vti.w), tb = (uint32_t)__float_as_int(vtj.w);
+                const uint4 rn = gm_philox4x32_10(make_uint4(min(ta, tb), max(ta, tb), step, 0u),
+                                                  make_uint2(P.seed_lo, P.seed_hi));
+                const float theta = 1.7320508075688772f * gm_sym24(rn.x);
+                const float fs = (c.c1 * w - P.gamma * w * w * edv + P.sigma_r_sqrt_inv_dt * w * theta) * ri;
+                fx += fs * dx; fy += fs * dy; fz += fs * dz;
+                if (ENERGY) pe += 0.5f * c.c1 * c.c3 * w * w;
+            }
+        }
+    }
+}
+
+// Gather loop over row i of NL (Alg. 2), software-pipelined in batches of NB list
+// entries: the NB index loads of the NEXT batch and the NB position gathers of THIS batch are all in
+// flight before the first force term is evaluated, so a thread waits about two memory latencies per
+// batch instead of two per neighbor.  Slots past NN[i] read nothing and stand for a bead 1e18 away.
 template <int PAIR, bool NT1, bool ENERGY, bool MI>
 __device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
-                                          const float4 *__restrict__ vt, int i, const float4 pi, const int ti,
-                                          const float4 vti, unsigned long long step, BeadForce &o)
+                                          const float4 *__restrict__ vt, int i, const int nn, const float4 pi,
+                                          const int ti, const float4 vti, unsigned long long step, BeadForce &o)
 {
-    const int nn = D.nn[i];
+    constexpr int NB = (PAIR == GM_PAIR_DPD) ? 4 : 8;
     const int *__restrict__ nl = D.nl + i;
     const size_t n = (size_t)P.ns;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
     const GmPair p0 = P.pair[0];
-    for (int k = 0; k < nn; ++k) {
-        const int j = nl[(size_t)k * n];
-        const float4 pj = pos[j];
-        float dx, dy, dz;
-        if (MI) {
-            dx = gm_min_image(pi.x, pj.x, P.half[0]);
-            dy = gm_min_image(pi.y, pj.y, P.half[1]);
-            dz = gm_min_image(pi.z, pj.z, P.half[2]);
-        } else {
-            dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
+    const float4 far = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+    int jn[NB];
+#pragma unroll
+    for (int u = 0; u < NB; ++u) jn[u] = (u < nn) ? __ldg(nl + (size_t)u * n) : -1;
+    for (int k = 0; k < nn; k += NB) {
+        float4 pj[NB], vj[NB];
+#pragma unroll
+        for (int u = 0; u < NB; ++u) pj[u] = (jn[u] >= 0) ? __ldg(pos + jn[u]) : far;
+        if (PAIR == GM_PAIR_DPD) {
+#pragma unroll
+            for (int u = 0; u < NB; ++u) vj[u] = (jn[u] >= 0) ? __ldg(vt + jn[u]) : far;
         }
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        GmPair c = p0;
-        if (!NT1) c = P.pair[ti * P.n_types + __float_as_int(pj.w)];
-        if (r2 < c.c0) {
-            if (PAIR == GM_PAIR_LJ) {
-                // F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij
-                const float r2i = gm_rcp(r2);
-                const float r6i = r2i * r2i * r2i;
-                const float fs = r2i * r6i * (c.c1 * r6i - c.c2);
-                fx += fs * dx; fy += fs * dy; fz += fs * dz;
-                if (ENERGY) {
-                    pe += r6i * (c.c1 * (1.0f / 12.0f) * r6i - c.c2 * (1.0f / 6.0f)) - c.c3;
-                    cnt += 1.0f;
-                }
-            } else if (PAIR == GM_PAIR_DPD) {
-                if (ENERGY) cnt += 1.0f;
-                if (r2 >= 1e-12f) {
-                    // F_ij = [a w - gamma w^2 (e.v_ij) + sigma_R w theta / sqrt(dt)] e,  w = 1 - r/r_c
-                    const float4 vtj = vt[j];
-                    const float ri = rsqrtf(r2);
-                    const float r = r2 * ri;
-                    const float w = 1.0f - r * c.c2;
-                    const float edv = (dx * (vti.x - vtj.x) + dy * (vti.y - vtj.y) + dz * (vti.z - vtj.z)) * ri;
-                    const uint32_t ta = (uint32_t)__float_as_int(vti.w), tb = (uint32_t)__float_as_int(vtj.w);
-                    const uint4 rn = gm_philox4x32_10(make_uint4(min(ta, tb), max(ta, tb), (uint32_t)step, 0u),
-                                                      make_uint2(P.seed_lo, P.seed_hi));
-                    const float theta = 1.7320508075688772f * gm_sym24(rn.x);
-                    const float fs = (c.c1 * w - P.gamma * w * w * edv + P.sigma_r_sqrt_inv_dt * w * theta) * ri;
-                    fx += fs * dx; fy += fs * dy; fz += fs * dz;
-                    if (ENERGY) pe += 0.5f * c.c1 * c.c3 * w * w;
-                }
-            }
-        }
+#pragma unroll
+        for (int u = 0; u < NB; ++u) jn[u] = (k + NB + u < nn) ? __ldg(nl + (size_t)(k + NB + u) * n) : -1;
+#pragma unroll
+        for (int u = 0; u < NB; ++u)
+            pair_term<PAIR, NT1, ENERGY, MI>(P, pi, ti, vti, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : far, p0,
+                                             (uint32_t)step, fx, fy, fz, pe, cnt);
     }
-    o.fx = fx; o.fy = fy; o.fz = fz;
+    o.fx += fx; o.fy += fy; o.fz += fz;
     o.pe_pair = 0.5f * pe;
     o.cnt = cnt;
 }
 
+// Bond partners of bead i from column i of BL (Fig. 2), two at a time.
 template <bool ENERGY>
 __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
-                                          int i, const float4 pi, BeadForce &o)
+                                          int i, const int nb, const float4 pi, BeadForce &o)
 {
     float pe = 0.f;
-    if (P.max_bonds > 0 && P.bond_style != GM_BOND_NONE) {
-        const int nb = D.bn[i];
-        const size_t n = (size_t)P.ns;
-        for (int k = 0; k < nb; ++k) {
-            const int e = D.bl[(size_t)k * n + i];
-            const int j = e & GM_BOND_MASK, bt = (unsigned)e >> GM_BOND_SHIFT;
-            const float4 pj = pos[j];
-            const float dx = gm_min_image(pi.x, pj.x, P.half[0]);
-            const float dy = gm_min_image(pi.y, pj.y, P.half[1]);
-            const float dz = gm_min_image(pi.z, pj.z, P.half[2]);
+    const size_t n = (size_t)P.ns;
+    const int *__restrict__ bl = D.bl + i;
+    for (int k = 0; k < nb; k += 2) {
+        int e[2];
+        float4 pj[2];
+#pragma unroll
+        for (int u = 0; u < 2; ++u) e[u] = (k + u < nb) ? __ldg(bl + (size_t)(k + u) * n) : -1;
+#pragma unroll
+        for (int u = 0; u < 2; ++u) pj[u] = (e[u] >= 0) ? __ldg(pos + (e[u] & GM_BOND_MASK)) : pi;
+#pragma unroll
+        for (int u = 0; u < 2; ++u) {
+            if (e[u] < 0) continue;
+            const int bt = (unsigned)e[u] >> GM_BOND_SHIFT;
+            const float dx = gm_min_image(pi.x, pj[u].x, P.half[0]);
+            const float dy = gm_min_image(pi.y, pj[u].y, P.half[1]);
+            const float dz = gm_min_image(pi.z, pj[u].z, P.half[2]);
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float kb = P.bond_k[bt], r0 = P.bond_r0[bt];
             float fs;
@@ -135,16 +168,19 @@ __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &
     BeadForce o;
     o.fx = o.fy = o.fz = o.pe_pair = o.pe_bond = o.cnt = 0.f;
     const int ti = __float_as_int(pi.w);
+    const bool bonded = P.max_bonds > 0 && P.bond_style != GM_BOND_NONE;
+    const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
+    const int nb = bonded ? D.bn[i] : 0;
+    bond_loop<ENERGY>(P, D, pos, i, nb, pi, o);
     if (PAIR != GM_PAIR_NONE) {
         // A bead further than r_list + skin from every face cannot have a listed partner across the
         // boundary (both moved < skin/2 since the build): plain differences, no image test.
         const float m = P.edge_margin;
         const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
                               fabsf(pi.z) < P.half[2] - m;
-        if (interior) pair_loop<PAIR, NT1, ENERGY, false>(P, D, pos, vt, i, pi, ti, vti, step, o);
-        else pair_loop<PAIR, NT1, ENERGY, true>(P, D, pos, vt, i, pi, ti, vti, step, o);
+        if (interior) pair_loop<PAIR, NT1, ENERGY, false>(P, D, pos, vt, i, nn, pi, ti, vti, step, o);
+        else pair_loop<PAIR, NT1, ENERGY, true>(P, D, pos, vt, i, nn, pi, ti, vti, step, o);
     }
-    bond_loop<ENERGY>(P, D, pos, i, pi, o);
     return o;
 }
 
