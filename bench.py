@@ -243,9 +243,9 @@ def main():
     pairs_in_rc = en["n_pairs"]
 
     # kernels launched inside the timed region: per timestep the gate + the fused force/integrate kernel;
-    # per rebuild 8 (clear, keys, 3 scan, scatter, cell finish, NL build); per reorder the counting sort
-    # (7) + 5 permute/copy kernels + bond remap + an ungated rebuild (already counted in `rebuilds`)
-    launches = n_ts * 2 + rebuilds * 8 + reorders * 13
+    # per rebuild 6 (keys, 2 scan, scatter, permute = SFC sort of all particle arrays, NL build)
+
+    launches = n_ts * 2 + rebuilds * 6
 
     # ---- the dominant kernel alone: CUDA events around every launch (gm_step_timed) ----------------
     n_prof = min(inner, 200)

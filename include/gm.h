@@ -4,7 +4,8 @@
  *
  * The pipeline:
  *   a1 cell binning by counting sort         PAPER.md:L57 (cell list CL/CN), Alg. 1 Kernel 1 L376-388
- *   a2 periodic space-filling-curve reorder  PAPER.md:L33, L199 (SFCPACK memory sort)
+ *   a2 space-filling-curve reorder of the    PAPER.md:L33, L199 (SFCPACK memory sort); here the sort key of a1
+ *      particle arrays at every rebuild
  *   a3 skin-padded FULL Verlet list NL/NN    PAPER.md:L51 (table form NL[k*Np+i]), L57 (27 cells,
  *                                            r_cut + r_buffer)
  *   a4 rebuild when a bead moved > skin/2
@@ -80,7 +81,8 @@ typedef struct {
     int32_t bond_style;              /* GM_BOND_*                                                  */
     int32_t integrator;              /* GM_NVE | GM_LANGEVIN | GM_DPD_GWVV                         */
     float kT, gamma, lambda;         /* thermostat temperature, friction, GW-VV lambda             */
-    int32_t sfc_period;              /* steps between SFC reorders; 0 = only at the first build    */
+    int32_t sfc_period;              /* largest number of steps between two SFC sorts of the particle arrays (every
+                                        neighbor rebuild sorts; > 0 forces a rebuild after this many steps) */
     int32_t nl_row_capacity;         /* rows of the NL table; 0 = choose from density              */
     int32_t flags;                   /* GM_FLAG_*                                                  */
     int32_t reserved;
@@ -155,7 +157,7 @@ gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma)
  * kernel (no CUDA graph) with CUDA events on the system's stream around the fused force+integrate
  * kernel (a4..a8) and around the rebuild kernels (a1 + a3; early-exit when no rebuild is due).
  * out (HOST, 4 doubles): summed device ms of the force+integrate launches, summed device ms of the
- * rebuild launches, number of force+integrate launches, number of SFC reorders done inside.
+ * rebuild launches, number of force+integrate launches, number of rebuilds (= SFC sorts) done inside.
  * Synchronises.  Same results, bit for bit, as gm_step. */
 gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4]);
 
@@ -173,15 +175,15 @@ gm_status gm_get_particles(gm_system *s, float *pos3, float *vel3, float *force3
  * (see gm_get_stats), else INVALID_ARG. */
 gm_status gm_get_neighbors(gm_system *s, int32_t *nn, int32_t *nl_tags, int64_t row_stride, int on_device);
 
-/* out (HOST, 8 int64): steps taken, neighbor rebuilds, SFC reorders, max nn of the current list,
+/* out (HOST, 8 int64): steps taken, neighbor rebuilds, SFC sorts (= rebuilds), max nn of the current list,
  * sum of nn of the current list, latched device error word (0 = none), nl_row_capacity,
  * number of cells.  Synchronises; returns the latched device error as status if one is set. */
 gm_status gm_get_stats(gm_system *s, int64_t out[8]);
 
 /* Host-only utility (a2): the space-filling-curve rank of every cell of an nc[0] x nc[1] x nc[2] grid
- * (linear cell id = (z * nc[1] + y) * nc[0] + x), i.e. the permutation the reorder sorts beads by:
- * cells in Hilbert-curve order.  rank_out: HOST array of nc[0]*nc[1]*nc[2] uint32.  The order only
- * affects memory locality, never results. */
+ * (linear cell id = (z * nc[1] + y) * nc[0] + x), i.e. the key every neighbor rebuild sorts the beads by:
+ * cells run along x inside a row, the (y, z) rows follow a 2-D Hilbert curve.  rank_out: HOST array of
+ * nc[0]*nc[1]*nc[2] uint32.  The order only affects memory locality, never results. */
 gm_status gm_sfc_cell_order(const int32_t nc[3], uint32_t *rank_out);
 
 /* Message of the last failing call on `s` (or a static string if s is NULL).  Never NULL. */

@@ -20,8 +20,7 @@ struct gm_system {
     cudaStream_t st, cap_st, cap_st2;
     int cur;                       // which pos/vt buffer holds the current time level
     bool have_particles, lagged, nl_valid, force_current, bonds_dirty, pair_set_any;
-    uint64_t step, last_reorder_step;
-    int64_t n_reorders;
+    uint64_t step;
     bool use_graph, use_cond;
     cudaGraphExec_t exec_big, exec_two;
     char err[512];
@@ -57,7 +56,8 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
-    P->ns = (P->n + GM_PAD - 1) / GM_PAD * GM_PAD;
+    P->ns = (P->n + 1 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slot n: the far-away pad bead
+    P->sfc_period = c->sfc_period;
     P->n_types = c->n_types;
     P->max_bonds = c->max_bonds_per_particle;
     const double r_list = (double)c->r_cut_max + (double)c->r_skin;
@@ -95,9 +95,11 @@ static gm_status derive(const gm_config *c, GmParams *P)
         double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
         cap = (int)(1.5 * nbar) + 32;
     }
-    cap = (cap + 7) / 8 * 8;
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
+    cap = (cap + 7) / 8 * 8;
     P->nl_cap = cap;
+    P->capq = cap / 4;
+    if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
     for (int t = 0; t < GM_MAX_TYPES * GM_MAX_TYPES; ++t) { P->pair[t].c0 = 0.f; P->pair[t].c1 = 0.f; P->pair[t].c2 = 0.f; P->pair[t].c3 = 0.f; }
     return GM_OK;
 }
@@ -116,73 +118,88 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     memset(&d, 0, sizeof(d));
     d.ctl = (GmCtl *)take(sizeof(GmCtl));
     d.pos[0] = (float4 *)take(n * 16); d.pos[1] = (float4 *)take(n * 16);
-    d.vel = (float4 *)take(n * 16);
-    if (c.pair_style == GM_PAIR_DPD) { d.vt[0] = (float4 *)take(n * 16); d.vt[1] = (float4 *)take(n * 16); }
-    d.frc = (float4 *)take(n * 16);
     d.ref = (float4 *)take(n * 16);
-    d.cpos = (float4 *)take(n * 16);
-    d.tmp4 = (float4 *)take(n * 16);
-    d.tag = (int *)take(n * 4); d.rtag = (int *)take(n * 4);
+    d.vel = (float4 *)take(n * 16); d.svel = (float4 *)take(n * 16);
+    if (c.pair_style == GM_PAIR_DPD) {
+        d.vt[0] = (float4 *)take(n * 16); d.vt[1] = (float4 *)take(n * 16); d.svt = (float4 *)take(n * 16);
+    }
+    d.frc = (float4 *)take(n * 16);
+    d.tag[0] = (int *)take(n * 4); d.tag[1] = (int *)take(n * 4); d.rtag = (int *)take(n * 4);
     d.nn = (int *)take(n * 4);
     d.nnw = (int *)take(n / 32 * 4);
-    d.nl = (int *)take(n * 4 * (size_t)P.nl_cap);
+    d.nl = (int4 *)take(n * 4 * (size_t)P.nl_cap);
     if (P.max_bonds > 0) {
-        d.bn = (int *)take(n * 4); d.bl = (int *)take(n * 4 * (size_t)P.max_bonds);
-        d.bn_tag = (int *)take(n * 4); d.bl_tag = (int *)take(n * 4 * (size_t)P.max_bonds);
+        const size_t bb = n * 4 * (size_t)P.max_bonds;
+        d.bl = (int *)take(bb); d.blt[0] = (int *)take(bb); d.blt[1] = (int *)take(bb); d.bl_tag = (int *)take(bb);
     }
     d.key = (int *)take(n * 4); d.rank = (int *)take(n * 4); d.sorted = (int *)take(n * 4);
-    d.tmpi = (int *)take(n * 4);
-    d.cstart = (int *)take(((size_t)P.n_cells + 1) * 4);
+    d.cstart = (int *)take(((size_t)P.n_cells + 1 + 4) * 4);
+    d.ccount = (int *)take(((size_t)P.n_cells + 1 + 4) * 4);
     size_t per = (size_t)GM_SCAN_BLOCK * GM_SCAN_ITEMS;
     d.scan_sums = (int *)take((((size_t)P.n_cells + 1 + per - 1) / per + 1) * 4);
-    d.cell_rank = (uint32_t *)take((size_t)P.n_cells * 4);
+    d.row_rank = (uint32_t *)take((size_t)P.nc[1] * P.nc[2] * 4);
     d.stage = (float *)take(n * 4 * 11);
     d.esum = (double *)take(((size_t)GM_ESUM_BLOCKS + 1) * 8 * sizeof(double));
     if (D) *D = d;
     return off;
 }
 
-// ---- a2: Hilbert order of the cells ------------------------------------------------------------------
-// Skilling's transpose form of the Hilbert curve (J. Skilling, "Programming the Hilbert curve", AIP
-// Conf. Proc. 707, 2004), restated: axes -> transposed index in place, then the bits are interleaved.
-static uint64_t hilbert_index(uint32_t x, uint32_t y, uint32_t z, int bits)
+// ---- a2: the space-filling curve the beads are sorted along ------------------------------------------
+// Cells run along x inside a row (so the x-neighbors of a cell are its memory neighbors and the 27-cell
+// search reads 9 contiguous runs); the (y, z) rows follow a 2-D Hilbert curve, so the 8 neighbor rows
+// of a row are close in memory too.  Hilbert index in Skilling's transpose form (J. Skilling,
+// "Programming the Hilbert curve", AIP Conf. Proc. 707, 2004), restated for ND dimensions: axes ->
+// transposed index in place, then the bits are interleaved.
+template <int ND>
+static uint64_t hilbert_index(const uint32_t *axes, int bits)
 {
-    uint32_t X[3] = { x, y, z };
+    uint32_t X[ND];
+    for (int i = 0; i < ND; ++i) X[i] = axes[i];
     const uint32_t M = 1u << (bits - 1);
     for (uint32_t Q = M; Q > 1; Q >>= 1) {
         const uint32_t Pm = Q - 1;
-        for (int i = 0; i < 3; ++i) {
+        for (int i = 0; i < ND; ++i) {
             if (X[i] & Q) X[0] ^= Pm;
             else { uint32_t t = (X[0] ^ X[i]) & Pm; X[0] ^= t; X[i] ^= t; }
         }
     }
-    for (int i = 1; i < 3; ++i) X[i] ^= X[i - 1];
+    for (int i = 1; i < ND; ++i) X[i] ^= X[i - 1];
     uint32_t t = 0;
-    for (uint32_t Q = M; Q > 1; Q >>= 1) if (X[2] & Q) t ^= Q - 1;
-    for (int i = 0; i < 3; ++i) X[i] ^= t;
+    for (uint32_t Q = M; Q > 1; Q >>= 1) if (X[ND - 1] & Q) t ^= Q - 1;
+    for (int i = 0; i < ND; ++i) X[i] ^= t;
     uint64_t h = 0;
     for (int b = bits - 1; b >= 0; --b)
-        for (int i = 0; i < 3; ++i) h = (h << 1) | ((X[i] >> b) & 1u);
+        for (int i = 0; i < ND; ++i) h = (h << 1) | ((X[i] >> b) & 1u);
     return h;
+}
+
+// rank of every (y, z) row of cells along the 2-D Hilbert curve (row id = z * ncy + y)
+static void sfc_row_order(int ncy, int ncz, std::vector<uint32_t> &row_rank)
+{
+    int mx = std::max(ncy, ncz);
+    int bits = 1;
+    while ((1 << bits) < mx) ++bits;
+    const size_t nrow = (size_t)ncy * ncz;
+    std::vector<std::pair<uint64_t, uint32_t>> v(nrow);
+    for (int z = 0; z < ncz; ++z)
+        for (int y = 0; y < ncy; ++y) {
+            const uint32_t ax[2] = { (uint32_t)y, (uint32_t)z };
+            v[(size_t)z * ncy + y] = std::make_pair(hilbert_index<2>(ax, bits), (uint32_t)(z * ncy + y));
+        }
+    std::sort(v.begin(), v.end());
+    row_rank.resize(nrow);
+    for (size_t r = 0; r < nrow; ++r) row_rank[v[r].second] = (uint32_t)r;
 }
 
 extern "C" gm_status gm_sfc_cell_order(const int32_t nc[3], uint32_t *rank_out)
 {
     if (!nc || !rank_out || nc[0] < 1 || nc[1] < 1 || nc[2] < 1) return GM_ERR_INVALID_ARG;
-    int mx = std::max(nc[0], std::max(nc[1], nc[2]));
-    int bits = 1;
-    while ((1 << bits) < mx) ++bits;
-    const size_t ncell = (size_t)nc[0] * nc[1] * nc[2];
-    std::vector<std::pair<uint64_t, uint32_t>> v(ncell);
+    std::vector<uint32_t> rr;
+    sfc_row_order(nc[1], nc[2], rr);
     for (int z = 0; z < nc[2]; ++z)
         for (int y = 0; y < nc[1]; ++y)
-            for (int x = 0; x < nc[0]; ++x) {
-                uint32_t c = (uint32_t)((z * nc[1] + y) * nc[0] + x);
-                v[c] = std::make_pair(hilbert_index((uint32_t)x, (uint32_t)y, (uint32_t)z, bits), c);
-            }
-    std::sort(v.begin(), v.end());
-    for (size_t r = 0; r < ncell; ++r) rank_out[v[r].second] = (uint32_t)r;
-    if (getenv("GM_EXP_LINEAR")) for (size_t r = 0; r < ncell; ++r) rank_out[r] = (uint32_t)r;
+            for (int x = 0; x < nc[0]; ++x)
+                rank_out[((size_t)z * nc[1] + y) * nc[0] + x] = rr[(size_t)z * nc[1] + y] * (uint32_t)nc[0] + (uint32_t)x;
     return GM_OK;
 }
 
@@ -225,17 +242,26 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     cudaError_t e = cudaSetDevice(cfg->device);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st2, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = gm_nl_prepare(P);
     if (e == cudaSuccess) {
-        std::vector<uint32_t> rank((size_t)P.n_cells);
-        gm_sfc_cell_order(P.nc, rank.data());
-        e = cudaMemcpyAsync(s->D.cell_rank, rank.data(), rank.size() * 4, cudaMemcpyHostToDevice, s->st);
+        std::vector<uint32_t> rr;
+        sfc_row_order(P.nc[1], P.nc[2], rr);
+        e = cudaMemcpyAsync(s->D.row_rank, rr.data(), rr.size() * 4, cudaMemcpyHostToDevice, s->st);
         if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
     }
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->D.ccount, 0, ((size_t)P.n_cells + 1 + 4) * 4, s->st);
     if (e == cudaSuccess && P.max_bonds > 0) {
-        e = cudaMemsetAsync(s->D.bn_tag, 0, (size_t)P.n * 4, s->st);
-        if (e == cudaSuccess) e = cudaMemsetAsync(s->D.bn, 0, (size_t)P.n * 4, s->st);
+        const size_t bb = (size_t)P.ns * 4 * (size_t)P.max_bonds;       // -1 everywhere: no bonds
+        e = cudaMemsetAsync(s->D.bl, 0xFF, bb, s->st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(s->D.blt[0], 0xFF, bb, s->st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(s->D.blt[1], 0xFF, bb, s->st);
+        if (e == cudaSuccess) e = cudaMemsetAsync(s->D.bl_tag, 0xFF, bb, s->st);
     }
-    if (e == cudaSuccess) { gm_launch_set_ctl(s->D, 0, 1, s->st); e = cudaGetLastError(); }
+    if (e == cudaSuccess) {
+        gm_launch_init_pad(P, s->D, s->st);
+        gm_launch_set_ctl(s->D, 0, 1, 0, s->st);
+        e = cudaGetLastError();
+    }
     if (e != cudaSuccess) {
         if (s->cap_st) cudaStreamDestroy(s->cap_st);
         if (s->cap_st2) cudaStreamDestroy(s->cap_st2);
@@ -302,6 +328,7 @@ extern "C" gm_status gm_set_bond_params(gm_system *s, int btype, float k, float 
     if (s->P.bond_style == GM_BOND_FENE && !(r0 > 0.f)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_bond_params: FENE needs R0 > 0%s");
     s->P.bond_k[btype] = k;
     s->P.bond_r0[btype] = r0;
+    s->P.bond_c[btype] = (r0 != 0.f) ? (float)(1.0 / ((double)r0 * (double)r0)) : 0.f;
     s->force_current = false;
     drop_graphs(s);
     return GM_OK;
@@ -327,10 +354,9 @@ extern "C" gm_status gm_set_particles(gm_system *s, const float *pos3, const flo
     }
     s->cur = 0;
     gm_launch_pack(s->P, s->D, 0, dp, dv, dt, dm, s->st);
-    gm_launch_set_ctl(s->D, 0, 1, s->st);
+    gm_launch_set_ctl(s->D, 0, 1, 0, s->st);
     CU(cudaGetLastError());
     s->step = 0;
-    s->n_reorders = 0;
     s->have_particles = true;
     s->lagged = false;
     s->nl_valid = false;
@@ -358,9 +384,9 @@ extern "C" gm_status gm_set_bonds(gm_system *s, int64_t n_bonds, const int32_t *
         CU(cudaStreamSynchronize(s->st));
         pp = hp.data(); tt = btype ? ht.data() : nullptr;
     }
-    const size_t n = (size_t)s->P.n;
+    const size_t n = (size_t)s->P.n, ns = (size_t)s->P.ns;
     const int mb = s->P.max_bonds;
-    std::vector<int32_t> bn(n, 0), bl(n * (size_t)mb, 0);
+    std::vector<int32_t> bn(n, 0), bl(ns * (size_t)mb, -1);
     for (int64_t b = 0; b < n_bonds; ++b) {
         int32_t i = pp[2 * b], j = pp[2 * b + 1];
         int32_t t = tt ? tt[b] : 0;
@@ -368,11 +394,10 @@ extern "C" gm_status gm_set_bonds(gm_system *s, int64_t n_bonds, const int32_t *
             return fail(s, GM_ERR_INVALID_ARG, "gm_set_bonds: tag or bond type out of range%s");
         if (bn[i] >= mb || bn[j] >= mb)
             return fail(s, GM_ERR_INVALID_ARG, "gm_set_bonds: a bead exceeds max_bonds_per_particle%s");
-        bl[(size_t)bn[i] * n + i] = j | (t << GM_BOND_SHIFT); bn[i] += 1;   // stored under both ends
-        bl[(size_t)bn[j] * n + j] = i | (t << GM_BOND_SHIFT); bn[j] += 1;
+        bl[(size_t)bn[i] * ns + i] = j | (t << GM_BOND_SHIFT); bn[i] += 1;   // stored under both ends
+        bl[(size_t)bn[j] * ns + j] = i | (t << GM_BOND_SHIFT); bn[j] += 1;
     }
-    CU(cudaMemcpyAsync(s->D.bn_tag, bn.data(), n * 4, cudaMemcpyHostToDevice, s->st));
-    CU(cudaMemcpyAsync(s->D.bl_tag, bl.data(), n * 4 * (size_t)mb, cudaMemcpyHostToDevice, s->st));
+    CU(cudaMemcpyAsync(s->D.bl_tag, bl.data(), ns * 4 * (size_t)mb, cudaMemcpyHostToDevice, s->st));
     CU(cudaStreamSynchronize(s->st));      // the host vectors go out of scope
     s->bonds_dirty = true;
     s->force_current = false;
@@ -383,48 +408,30 @@ extern "C" gm_status gm_set_step(gm_system *s, uint64_t step)
 {
     if (!s) return GM_ERR_INVALID_ARG;
     CU(cudaSetDevice(s->cfg.device));
-    gm_launch_set_ctl(s->D, step, 0, s->st);
+    gm_launch_set_ctl(s->D, step, 0, s->cur, s->st);
     CU(cudaGetLastError());
     s->step = step;
-    s->last_reorder_step = step;
     s->nl_valid = false;       // `need` was reset: rebuild before the next force evaluation
     s->force_current = false;
     return GM_OK;
 }
 
-// ---- rebuild / reorder scheduling -------------------------------------------------------------------
+// ---- rebuild scheduling -------------------------------------------------------------------------------
+// gate kernel (decides on the device, publishes ctl->go) -> a1 + a2 (sort) -> a3 (NL build)
 static void enqueue_rebuild(gm_system *s, int gate, cudaStream_t st)
 {
-    const float4 *pos = s->D.pos[s->cur];
-    gm_launch_sort_keys(s->P, s->D, pos, 0, gate, s->cur, st);
-    gm_launch_cell_finish(s->P, s->D, pos, 1, gate, s->cur, st);
-    gm_launch_nl_build(s->P, s->D, pos, gate, s->cur, st);
-}
-
-static bool reorder_due(const gm_system *s)
-{
-    if (s->cfg.sfc_period < 0) return false;
-    if (s->n_reorders == 0) return true;
-    return s->cfg.sfc_period > 0 && s->step - s->last_reorder_step >= (uint64_t)s->cfg.sfc_period;
+    gm_launch_gate(s->D, gate, s->cur, 0ull, 0, st);
+    gm_launch_sort(s->P, s->D, s->cur, st);
+    gm_launch_nl_build(s->P, s->D, st);
 }
 
 // Make the NL usable for a force evaluation at the current time level, outside the graphs.
 static gm_status ensure_list(gm_system *s)
 {
-    bool forced = !s->nl_valid;
-    if (reorder_due(s)) {
-        const float4 *pos = s->D.pos[s->cur];
-        gm_launch_sort_keys(s->P, s->D, pos, 1, 0, s->cur, s->st);
-        gm_launch_cell_finish(s->P, s->D, pos, 0, 0, s->cur, s->st);
-        gm_launch_reorder(s->P, s->D, s->cur, s->st);
-        s->n_reorders += 1;
-        s->last_reorder_step = s->step;
-        s->bonds_dirty = true;
-        s->force_current = false;
-        forced = true;
-    }
-    if (s->bonds_dirty) { gm_launch_bonds_to_index(s->P, s->D, s->st); s->bonds_dirty = false; }
+    const bool forced = !s->nl_valid;
+    if (s->bonds_dirty) { gm_launch_bonds_from_master(s->P, s->D, s->st); s->bonds_dirty = false; }
     enqueue_rebuild(s, forced ? 0 : 1, s->st);
+    if (forced) s->force_current = false;
     s->nl_valid = true;
     CU(cudaGetLastError());
     return GM_OK;
@@ -468,7 +475,7 @@ static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
             ok = cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, &deps, &ndeps) == cudaSuccess;
             cudaGraphConditionalHandle h;
             ok = ok && cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
-            if (ok) gm_launch_gate(s->D, s->cur, (unsigned long long)h, s->cap_st);
+            if (ok) gm_launch_gate(s->D, 1, s->cur, (unsigned long long)h, 1, s->cap_st);
             ok = ok && cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, &deps, &ndeps) == cudaSuccess;
             cudaGraphNodeParams np = {};
             np.type = cudaGraphNodeTypeConditional;
@@ -482,7 +489,8 @@ static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
                 ok = cudaStreamBeginCaptureToGraph(s->cap_st2, body, nullptr, nullptr, 0,
                                                    cudaStreamCaptureModeRelaxed) == cudaSuccess;
                 if (ok) {
-                    enqueue_rebuild(s, 0, s->cap_st2);
+                    gm_launch_sort(s->P, s->D, s->cur, s->cap_st2);
+                    gm_launch_nl_build(s->P, s->D, s->cap_st2);
                     cudaGraph_t tmp = nullptr;
                     ok = cudaStreamEndCapture(s->cap_st2, &tmp) == cudaSuccess;
                 }
@@ -543,53 +551,40 @@ extern "C" gm_status gm_compute_forces(gm_system *s)
 
 struct StepTiming {
     std::vector<cudaEvent_t> ev;     // 3 per step: before rebuild, before force, after force
-    int64_t reorders;
 };
 
 static gm_status step_impl(gm_system *s, int64_t n_steps, StepTiming *tm)
 {
-    int64_t left = n_steps;
-    while (left > 0) {
-        if (!s->nl_valid || reorder_due(s) || s->bonds_dirty) {
-            const int64_t r0 = s->n_reorders;
-            gm_status r = ensure_list(s);
+    if (n_steps > 0 && (!s->nl_valid || s->bonds_dirty)) {
+        gm_status r = ensure_list(s);
+        if (r != GM_OK) return r;
+    }
+    int64_t done = 0;
+    while (done < n_steps) {
+        const int64_t rem = n_steps - done;
+        if (!tm && s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
+            const bool big = rem >= GM_GRAPH_STEPS;
+            cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
+            const int ns = big ? GM_GRAPH_STEPS : 2;
+            gm_status r = get_graph(s, ns, slot);
             if (r != GM_OK) return r;
-            if (tm) tm->reorders += s->n_reorders - r0;
-        }
-        int64_t chunk = left;
-        if (s->cfg.sfc_period > 0) {
-            int64_t until = (int64_t)s->cfg.sfc_period - (int64_t)(s->step - s->last_reorder_step);
-            if (until < 1) until = 1;
-            chunk = std::min(chunk, until);
-        }
-        int64_t done = 0;
-        while (done < chunk) {
-            const int64_t rem = chunk - done;
-            if (!tm && s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
-                const bool big = rem >= GM_GRAPH_STEPS;
-                cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
-                const int ns = big ? GM_GRAPH_STEPS : 2;
-                gm_status r = get_graph(s, ns, slot);
-                if (r != GM_OK) return r;
-                CU(cudaGraphLaunch(*slot, s->st));
-                done += ns;
-                s->step += (uint64_t)ns;
-            } else {
-                cudaEvent_t e[3] = { nullptr, nullptr, nullptr };
-                if (tm) {
-                    for (int q = 0; q < 3; ++q) { CU(cudaEventCreate(&e[q])); tm->ev.push_back(e[q]); }
-                    CU(cudaEventRecord(e[0], s->st));
-                }
-                enqueue_rebuild(s, 1, s->st);
-                if (tm) CU(cudaEventRecord(e[1], s->st));
-                enqueue_step_kernel(s, s->lagged, s->st);
-                if (tm) CU(cudaEventRecord(e[2], s->st));
-                s->lagged = true;
-                done += 1;
-                s->step += 1;
+            CU(cudaGraphLaunch(*slot, s->st));
+            done += ns;
+            s->step += (uint64_t)ns;
+        } else {
+            cudaEvent_t e[3] = { nullptr, nullptr, nullptr };
+            if (tm) {
+                for (int q = 0; q < 3; ++q) { CU(cudaEventCreate(&e[q])); tm->ev.push_back(e[q]); }
+                CU(cudaEventRecord(e[0], s->st));
             }
+            enqueue_rebuild(s, 1, s->st);
+            if (tm) CU(cudaEventRecord(e[1], s->st));
+            enqueue_step_kernel(s, s->lagged, s->st);
+            if (tm) CU(cudaEventRecord(e[2], s->st));
+            s->lagged = true;
+            done += 1;
+            s->step += 1;
         }
-        left -= chunk;
     }
     CU(cudaGetLastError());
     if (n_steps > 0) s->force_current = false;
@@ -612,8 +607,11 @@ extern "C" gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4])
     if (n_steps < 0 || n_steps > 100000 || !out) return fail(s, GM_ERR_INVALID_ARG, "gm_step_timed: bad arguments%s");
     CU(cudaSetDevice(s->cfg.device));
     StepTiming tm;
-    tm.reorders = 0;
+    GmCtl c0, c1;
+    CU(cudaMemcpyAsync(&c0, s->D.ctl, sizeof(c0), cudaMemcpyDeviceToHost, s->st));
+    CU(cudaStreamSynchronize(s->st));
     gm_status r = step_impl(s, n_steps, &tm);
+    if (cudaMemcpyAsync(&c1, s->D.ctl, sizeof(c1), cudaMemcpyDeviceToHost, s->st) != cudaSuccess) c1 = c0;
     cudaError_t e = cudaStreamSynchronize(s->st);
     double t_force = 0.0, t_rebuild = 0.0;
     for (size_t k = 0; k + 2 < tm.ev.size() + 0 && e == cudaSuccess; k += 3) {
@@ -625,7 +623,7 @@ extern "C" gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4])
     for (cudaEvent_t ev : tm.ev) cudaEventDestroy(ev);
     if (r != GM_OK) return r;
     if (e != cudaSuccess) return fail(s, GM_ERR_CUDA, "CUDA: %s", cudaGetErrorString(e));
-    out[0] = t_force; out[1] = t_rebuild; out[2] = (double)(tm.ev.size() / 3); out[3] = (double)tm.reorders;
+    out[0] = t_force; out[1] = t_rebuild; out[2] = (double)(tm.ev.size() / 3); out[3] = (double)(c1.n_rebuilds - c0.n_rebuilds);
     return GM_OK;
 }
 
@@ -750,7 +748,7 @@ extern "C" gm_status gm_get_stats(gm_system *s, int64_t out[8])
     if (r == GM_ERR_CUDA) return r;
     out[0] = (int64_t)s->step;
     out[1] = (int64_t)c.n_rebuilds;
-    out[2] = s->n_reorders;
+    out[2] = (int64_t)c.n_rebuilds;      // every rebuild sorts along the SFC
     out[3] = c.max_nn;
     out[4] = (int64_t)c.sum_nn;
     out[5] = c.err;

@@ -1,13 +1,13 @@
 // gm_force.cu -- a4..a9: pair + bond forces from the NL/BL tables, fused with the integrator and the
 // displacement test.
 //
-//   a5  Lennard-Jones, Eq. (1); gather loop over NL[(i,k)] with minimum image and a
+//   a5  Lennard-Jones, Eq. (1); gather loop over row i of NL with minimum image and a
 //       cutoff test as in Alg. 2, L458.  One thread owns bead i and sums all of its forces
 //       ("one thread calculates and sums all non-bonded forces of a particle"), so a pair
 //       is evaluated from both sides and no atomics are needed.
 //   a6  DPD (Groot-Warren; reading c-3) with one Philox4x32-10 draw per pair keyed
 //       (seed; min tag, max tag, step, 0) so that theta_ij = theta_ji without communication.
-//   a7  bonds from BL/BN, each bond evaluated from both ends; harmonic Eq. (7),
+//   a7  bonds from BL, each bond evaluated from both ends; harmonic Eq. (7),
 //       FENE (reading c-8).
 //   a8  velocity-Verlet NVE / Langevin ("BD") / GW-VV in kick-drift form: the kernel
 //       at time level m computes a(r^m), then u^{m} = u^{m-1} + kick a, r^{m+1} = r^m + dt u^m, where u
@@ -15,6 +15,12 @@
 //       gm_set_particles (kick = dt/2).  The force never leaves registers.
 //   a4  displacement test |r^{m+1} - r_ref| > skin/2 -> ctl->need = m + 1.
 //   a9  energies: fp32 terms, fp64 sums, fixed-order two-stage reduction.
+//
+// Memory plan of the step kernel: per bead it streams pos, vel, ref (48 B in), pos,
+// vel (32 B out), NN (4 B), its NL quads (16 B per 4 list entries, 512-byte coalesced per warp) and its BL
+// column; neighbor positions are 16-byte gathers that hit L1/L2 because storage order is cell order.
+// The gather loop is software-pipelined: the index quads of the next batch and all position gathers
+// of this batch are in flight before the first force term is evaluated.
 #include "gm_internal.cuh"
 
 #define FORCE_BLOCK 128
@@ -25,7 +31,8 @@ struct BeadForce {
     float cnt;                // partners inside r_cut
 };
 
-// One in-range test + force term of the pair loop (Alg. 2: displacement, cutoff test, accumulate).
+// One list entry of the pair loop (Alg. 2: displacement, cutoff test, accumulate).  The LJ term is
+// branch-free (out-of-range entries, and the far-away pad bead, select 0).
 template <int PAIR, bool NT1, bool ENERGY, bool MI>
 __device__ __forceinline__ void pair_term(const GmParams &P, const float4 pi, const int ti, const float4 vti,
                                           const float4 pj, const float4 vtj, const GmPair p0, uint32_t step,
@@ -42,18 +49,19 @@ __device__ __forceinline__ void pair_term(const GmParams &P, const float4 pi, co
     const float r2 = dx * dx + dy * dy + dz * dz;
     GmPair c = p0;
     if (!NT1) c = P.pair[ti * P.n_types + __float_as_int(pj.w)];
-    if (r2 < c.c0) {
-        if (PAIR == GM_PAIR_LJ) {
-            // F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij
-            const float r2i = gm_rcp(r2);
-            const float r6i = r2i * r2i * r2i;
-            const float fs = r2i * r6i * (c.c1 * r6i - c.c2);
-            fx += fs * dx; fy += fs * dy; fz += fs * dz;
-            if (ENERGY) {
-                pe += r6i * (c.c1 * (1.0f / 12.0f) * r6i - c.c2 * (1.0f / 6.0f)) - c.c3;
-                cnt += 1.0f;
-            }
-        } else if (PAIR == GM_PAIR_DPD) {
+    if (PAIR == GM_PAIR_LJ) {
+        // F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij
+        const bool in = r2 < c.c0;
+        const float r2i = gm_rcp(r2);
+        const float r6i = r2i * r2i * r2i;
+        const float fs = in ? r2i * r6i * (c.c1 * r6i - c.c2) : 0.0f;
+        fx += fs * dx; fy += fs * dy; fz += fs * dz;
+        if (ENERGY) {
+            pe += in ? r6i * (c.c1 * (1.0f / 12.0f) * r6i - c.c2 * (1.0f / 6.0f)) - c.c3 : 0.0f;
+            cnt += in ? 1.0f : 0.0f;
+        }
+    } else if (PAIR == GM_PAIR_DPD) {
+        if (r2 < c.c0) {
             if (ENERGY) cnt += 1.0f;
             if (r2 >= 1e-12f) {
                 // F_ij = [a w - gamma w^2 (e.v_ij) + sigma_R w theta / sqrt(dt)] e,  w = 1 - r/r_c
@@ -73,37 +81,40 @@ __device__ __forceinline__ void pair_term(const GmParams &P, const float4 pi, co
     }
 }
 
-// Gather loop over row i of NL (Alg. 2), software-pipelined in batches of NB list
-// entries: the NB index loads of the NEXT batch and the NB position gathers of THIS batch are all in
-// flight before the first force term is evaluated, so a thread waits about two memory latencies per
-// batch instead of two per neighbor.  Slots past NN[i] read nothing and stand for a bead 1e18 away.
-template <int PAIR, bool NT1, bool ENERGY, bool MI>
-__device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
-                                          const float4 *__restrict__ vt, int i, const int nn, const float4 pi,
-                                          const int ti, const float4 vti, unsigned long long step, BeadForce &o)
+__device__ __forceinline__ int quad_get(const int4 &e, int u)
 {
-    constexpr int NB = (PAIR == GM_PAIR_DPD) ? 4 : 8;
-    const int *__restrict__ nl = D.nl + i;
-    const size_t n = (size_t)P.ns;
+    return u == 0 ? e.x : (u == 1 ? e.y : (u == 2 ? e.z : e.w));
+}
+
+// Gather loop over row i of NL (Alg. 2), NQ quads (4 NQ list entries) per batch.
+template <int PAIR, bool NT1, bool ENERGY, bool MI>
+__device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, const Src &S, int i, const int nn,
+                                          const float4 pi, const int ti, const float4 vti,
+                                          unsigned long long step, BeadForce &o)
+{
+    constexpr int NQ = (PAIR == GM_PAIR_DPD) ? 1 : 2;
+    const int4 *__restrict__ t = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31);
+    const int nq = (nn + 3) >> 2;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
     const GmPair p0 = P.pair[0];
-    const float4 far = make_float4(1e18f, 1e18f, 1e18f, 0.f);
-    int jn[NB];
+    const int4 pad = make_int4(P.n, P.n, P.n, P.n);
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    int4 en[NQ];
 #pragma unroll
-    for (int u = 0; u < NB; ++u) jn[u] = (u < nn) ? __ldg(nl + (size_t)u * n) : -1;
-    for (int k = 0; k < nn; k += NB) {
-        float4 pj[NB], vj[NB];
+    for (int u = 0; u < NQ; ++u) en[u] = (u < nq) ? __ldg(t + u * 32) : pad;
+    for (int q = 0; q < nq; q += NQ) {
+        float4 pj[4 * NQ], vj[4 * NQ];
 #pragma unroll
-        for (int u = 0; u < NB; ++u) pj[u] = (jn[u] >= 0) ? __ldg(pos + jn[u]) : far;
+        for (int u = 0; u < 4 * NQ; ++u) pj[u] = __ldg(S.pos + quad_get(en[u >> 2], u & 3));
         if (PAIR == GM_PAIR_DPD) {
 #pragma unroll
-            for (int u = 0; u < NB; ++u) vj[u] = (jn[u] >= 0) ? __ldg(vt + jn[u]) : far;
+            for (int u = 0; u < 4 * NQ; ++u) vj[u] = __ldg(S.vt + quad_get(en[u >> 2], u & 3));
         }
 #pragma unroll
-        for (int u = 0; u < NB; ++u) jn[u] = (k + NB + u < nn) ? __ldg(nl + (size_t)(k + NB + u) * n) : -1;
+        for (int u = 0; u < NQ; ++u) en[u] = (q + NQ + u < nq) ? __ldg(t + (q + NQ + u) * 32) : pad;
 #pragma unroll
-        for (int u = 0; u < NB; ++u)
-            pair_term<PAIR, NT1, ENERGY, MI>(P, pi, ti, vti, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : far, p0,
+        for (int u = 0; u < 4 * NQ; ++u)
+            pair_term<PAIR, NT1, ENERGY, MI>(P, pi, ti, vti, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : zero4, p0,
                                              (uint32_t)step, fx, fy, fz, pe, cnt);
     }
     o.fx += fx; o.fy += fy; o.fz += fz;
@@ -111,21 +122,22 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, con
     o.cnt = cnt;
 }
 
-// Bond partners of bead i from column i of BL (Fig. 2), two at a time.
-template <bool ENERGY>
-__device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
-                                          int i, const int nb, const float4 pi, BeadForce &o)
+// Bond partners of bead i from column i of BL (Fig. 2), two at a time; -1 = no bond.
+template <int BOND, bool ENERGY>
+__device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, const Src &S, int i, const float4 pi,
+                                          BeadForce &o)
 {
+    if (BOND == GM_BOND_NONE) return;
     float pe = 0.f;
     const size_t n = (size_t)P.ns;
     const int *__restrict__ bl = D.bl + i;
-    for (int k = 0; k < nb; k += 2) {
+    for (int k = 0; k < P.max_bonds; k += 2) {
         int e[2];
         float4 pj[2];
 #pragma unroll
-        for (int u = 0; u < 2; ++u) e[u] = (k + u < nb) ? __ldg(bl + (size_t)(k + u) * n) : -1;
+        for (int u = 0; u < 2; ++u) e[u] = (k + u < P.max_bonds) ? __ldg(bl + (size_t)(k + u) * n) : -1;
 #pragma unroll
-        for (int u = 0; u < 2; ++u) pj[u] = (e[u] >= 0) ? __ldg(pos + (e[u] & GM_BOND_MASK)) : pi;
+        for (int u = 0; u < 2; ++u) pj[u] = (e[u] >= 0) ? __ldg(S.pos + (e[u] & GM_BOND_MASK)) : pi;
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             if (e[u] < 0) continue;
@@ -136,11 +148,11 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float kb = P.bond_k[bt], r0 = P.bond_r0[bt];
             float fs;
-            if (P.bond_style == GM_BOND_FENE) {
+            if (BOND == GM_BOND_FENE) {
                 // U = -1/2 k R0^2 ln(1 - r^2/R0^2);  F_i = -k r_ij / (1 - r^2/R0^2)
-                const float q = 1.0f - r2 / (r0 * r0);
+                const float q = 1.0f - r2 * P.bond_c[bt];
                 if (!(q > 0.0f)) { atomicOr(&D.ctl->err, GM_DEV_ERR_OVERSTRETCH); continue; }
-                fs = -kb / q;
+                fs = -kb * gm_rcp(q);
                 if (ENERGY) pe += -0.5f * kb * r0 * r0 * logf(q);
             } else {
                 // Eq. (7): U = k (r - r0)^2;  F_i = -2 k (1 - r0/r) r_ij
@@ -160,39 +172,36 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
 }
 
 // Force on bead i at time level `step`, conservative + (DPD) dissipative/random.  vti: own v~ and tag.
-template <int PAIR, bool NT1, bool ENERGY>
-__device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const float4 *__restrict__ pos,
-                                                const float4 *__restrict__ vt, int i, const float4 pi,
-                                                const float4 vti, unsigned long long step)
+template <int PAIR, bool NT1, int BOND, bool ENERGY>
+__device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const Src &S, int i,
+                                                const float4 pi, const float4 vti, unsigned long long step)
 {
     BeadForce o;
     o.fx = o.fy = o.fz = o.pe_pair = o.pe_bond = o.cnt = 0.f;
     const int ti = __float_as_int(pi.w);
-    const bool bonded = P.max_bonds > 0 && P.bond_style != GM_BOND_NONE;
     const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
-    const int nb = bonded ? D.bn[i] : 0;
-    bond_loop<ENERGY>(P, D, pos, i, nb, pi, o);
+    bond_loop<BOND, ENERGY>(P, D, S, i, pi, o);
     if (PAIR != GM_PAIR_NONE) {
         // A bead further than r_list + skin from every face cannot have a listed partner across the
         // boundary (both moved < skin/2 since the build): plain differences, no image test.
         const float m = P.edge_margin;
         const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
                               fabsf(pi.z) < P.half[2] - m;
-        if (interior) pair_loop<PAIR, NT1, ENERGY, false>(P, D, pos, vt, i, nn, pi, ti, vti, step, o);
-        else pair_loop<PAIR, NT1, ENERGY, true>(P, D, pos, vt, i, nn, pi, ti, vti, step, o);
+        if (interior) pair_loop<PAIR, NT1, ENERGY, false>(P, D, S, i, nn, pi, ti, vti, step, o);
+        else pair_loop<PAIR, NT1, ENERGY, true>(P, D, S, i, nn, pi, ti, vti, step, o);
     }
     return o;
 }
 
 // Acceleration the integrator uses: F/m, plus Langevin drag on the stored velocity and the per-bead
 // noise of this time level (reading c-7): a = F/m - gamma u + sqrt(6 gamma kT / (dt m)) xi.
-__device__ __forceinline__ float3 bead_accel(const GmParams &P, const GmDev &D, int i, const BeadForce &f,
+__device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, int i, const BeadForce &f,
                                              const float4 u, unsigned long long step)
 {
     const float im = 1.0f / u.w;
     float3 a = make_float3(f.fx * im, f.fy * im, f.fz * im);
     if (P.integrator == GM_LANGEVIN) {
-        const uint4 rn = gm_philox4x32_10(make_uint4((uint32_t)D.tag[i], 0u, (uint32_t)step, 1u),
+        const uint4 rn = gm_philox4x32_10(make_uint4((uint32_t)S.tag[i], 0u, (uint32_t)step, 1u),
                                           make_uint2(P.seed_lo, P.seed_hi));
         const float amp = sqrtf(P.lang_amp2 * im);
         a.x += -P.gamma * u.x + amp * gm_sym24(rn.x);
@@ -203,22 +212,29 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const GmDev &D, 
 }
 
 // ---- the per-step kernel (MODE_STEP) and the force-materialising kernel (MODE_FORCES) ---------------
-template <int PAIR, bool NT1, int MODE>
+template <int PAIR, bool NT1, int BOND, int MODE>
 __global__ void __launch_bounds__(FORCE_BLOCK)
 k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned long long step = D.ctl->step[parity];
-    if (MODE == GM_MODE_STEP && blockIdx.x == 0 && threadIdx.x == 0) D.ctl->step[parity ^ 1] = step + 1;
+    const Src S = current_src(D, parity, step);
+    if (MODE == GM_MODE_STEP && blockIdx.x == 0 && threadIdx.x == 0) {
+        D.ctl->step[parity ^ 1] = step + 1;
+        // a2: at most sfc_period steps between two sorts
+        if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
+            step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
+            D.ctl->need = step + 1;
+    }
     if (i >= P.n) return;
-    const float4 *__restrict__ pos = D.pos[parity];
-    const float4 *__restrict__ vt = D.vt[parity];
-    const float4 pi = pos[i];
+    const float4 pi = S.pos[i];
+    const float4 u = S.vel[i];
+    float4 rf = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (MODE == GM_MODE_STEP) rf = D.ref[i];
     float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (PAIR == GM_PAIR_DPD) vti = vt[i];
-    const BeadForce f = bead_force<PAIR, NT1, MODE == GM_MODE_FORCES>(P, D, pos, vt, i, pi, vti, step);
-    const float4 u = D.vel[i];
-    const float3 a = bead_accel(P, D, i, f, u, step);
+    if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
+    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES>(P, D, S, i, pi, vti, step);
+    const float3 a = bead_accel(P, S, i, f, u, step);
     if (MODE == GM_MODE_FORCES) {
         D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
         return;
@@ -233,7 +249,6 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, flo
     const float z = gm_wrap(pi.z + P.dt * uz, P.half[2], P.box[2]);
     D.pos[parity ^ 1][i] = make_float4(x, y, z, pi.w);
     // a4: displacement since the last NL build
-    const float4 rf = D.ref[i];
     const float dx = gm_min_image(x, rf.x, P.half[0]);
     const float dy = gm_min_image(y, rf.y, P.half[1]);
     const float dz = gm_min_image(z, rf.z, P.half[2]);
@@ -241,23 +256,22 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, flo
 }
 
 // ---- a9 energies: grid-stride, fp64 accumulation, per-block partials in fixed order ----------------
-template <int PAIR, bool NT1>
+template <int PAIR, bool NT1, int BOND>
 __global__ void __launch_bounds__(FORCE_BLOCK)
 k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
 {
     const unsigned long long step = D.ctl->step[parity];
-    const float4 *__restrict__ pos = D.pos[parity];
-    const float4 *__restrict__ vt = D.vt[parity];
+    const Src S = current_src(D, parity, step);
     double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };   // ke, pe_pair, pe_bond, px, py, pz, pairs
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += gridDim.x * blockDim.x) {
-        const float4 pi = pos[i];
+        const float4 pi = S.pos[i];
         float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (PAIR == GM_PAIR_DPD) vti = vt[i];
-        const BeadForce f = bead_force<PAIR, NT1, true>(P, D, pos, vt, i, pi, vti, step);
-        const float4 u = D.vel[i];
+        if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
+        const BeadForce f = bead_force<PAIR, NT1, BOND, true>(P, D, S, i, pi, vti, step);
+        const float4 u = S.vel[i];
         float vx = u.x, vy = u.y, vz = u.z;
         if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m
-            const float3 a = bead_accel(P, D, i, f, u, step);
+            const float3 a = bead_accel(P, S, i, f, u, step);
             vx += 0.5f * P.dt * a.x; vy += 0.5f * P.dt * a.y; vz += 0.5f * P.dt * a.z;
         }
         acc[0] += 0.5 * (double)u.w * ((double)vx * vx + (double)vy * vy + (double)vz * vz);
@@ -292,20 +306,31 @@ __global__ void k_energy_final(GmDev D, int n_blocks)
     }
 }
 
-template <int PAIR, bool NT1>
+template <int PAIR, bool NT1, int BOND>
 static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
                            int lagged, cudaStream_t st)
 {
     int nb = (P.n + FORCE_BLOCK - 1) / FORCE_BLOCK;
     if (mode == GM_MODE_STEP)
-        k_force<PAIR, NT1, GM_MODE_STEP><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+        k_force<PAIR, NT1, BOND, GM_MODE_STEP><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
     else if (mode == GM_MODE_FORCES)
-        k_force<PAIR, NT1, GM_MODE_FORCES><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+        k_force<PAIR, NT1, BOND, GM_MODE_FORCES><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
     else {
         int g = nb < GM_ESUM_BLOCKS ? nb : GM_ESUM_BLOCKS;
-        k_energy<PAIR, NT1><<<g, FORCE_BLOCK, 0, st>>>(P, D, parity, lagged);
+        k_energy<PAIR, NT1, BOND><<<g, FORCE_BLOCK, 0, st>>>(P, D, parity, lagged);
         k_energy_final<<<1, 32, 0, st>>>(D, g);
     }
+}
+
+template <int PAIR, bool NT1>
+static void launch_force_b(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
+                           int lagged, cudaStream_t st)
+{
+    const int bond = (P.max_bonds > 0) ? P.bond_style : GM_BOND_NONE;
+    if (bond == GM_BOND_FENE) launch_force_t<PAIR, NT1, GM_BOND_FENE>(P, D, mode, parity, kick, kick_vt, lagged, st);
+    else if (bond == GM_BOND_HARMONIC)
+        launch_force_t<PAIR, NT1, GM_BOND_HARMONIC>(P, D, mode, parity, kick, kick_vt, lagged, st);
+    else launch_force_t<PAIR, NT1, GM_BOND_NONE>(P, D, mode, parity, kick, kick_vt, lagged, st);
 }
 
 void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
@@ -314,14 +339,14 @@ void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, fl
     const bool nt1 = (P.n_types == 1);
     switch (P.pair_style) {
     case GM_PAIR_LJ:
-        if (nt1) launch_force_t<GM_PAIR_LJ, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
-        else launch_force_t<GM_PAIR_LJ, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        if (nt1) launch_force_b<GM_PAIR_LJ, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_b<GM_PAIR_LJ, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
         break;
     case GM_PAIR_DPD:
-        if (nt1) launch_force_t<GM_PAIR_DPD, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
-        else launch_force_t<GM_PAIR_DPD, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        if (nt1) launch_force_b<GM_PAIR_DPD, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_b<GM_PAIR_DPD, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
         break;
     default:
-        launch_force_t<GM_PAIR_NONE, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        launch_force_b<GM_PAIR_NONE, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
     }
 }

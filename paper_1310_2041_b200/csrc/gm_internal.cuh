@@ -1,18 +1,28 @@
 // gm_internal.cuh -- shared declarations of libgm's CUDA path (sm_100a).  Nothing here is used by,
 // or derived from, the CPU oracle under oracle/.
 //
-// Device data layout:
-//   pos[2]  float4[N]  x, y, z, type (int bits)          ping-pong; STORAGE order (SFC order of the
-//   vel     float4[N]  u_x, u_y, u_z, mass               last reorder).  u is the half-step velocity
-//   vt[2]   float4[N]  v~_x, v~_y, v~_z, tag (int bits)  DPD only: the velocity the dissipative force sees
-//   frc     float4[N]  F_x, F_y, F_z, per-bead PE        materialised only by gm_compute_forces
-//   ref     float4[N]  position at the last NL build     (displacement test a4)
-//   nl      int[cap*ns] NL[k*ns + i], column-major table, ns = N rounded up to GM_PAD   PAPER.md:L51, Fig. 1
-//   nn      int[N]     NN[i]
-//   bl      int[mb*ns] BL[k*ns + i] = j | btype << 28    PAPER.md:L97, Fig. 2 (index space)
-//   bn      int[N]
-//   cpos    float4[N]  x, y, z, storage index            cell list CL in CSR form
-//   cstart  int[n_cells + 1]                             replaces CN: cell c holds cpos[cstart[c] .. cstart[c+1])
+// Device data layout.  STORAGE order is the cell order of the last
+// neighbor-list rebuild: every rebuild counting-sorts the beads by cell (a1) along the space-filling
+// curve (a2) and moves all per-bead state, so bead s of cell c sits at s in [cstart[c], cstart[c+1]).
+//   pos[2]  float4[ns]  x, y, z, type (int bits)          ping-pong by time-level parity
+//   ref     float4[ns]  pos at the last rebuild, sorted    = the cell list CL in CSR form,
+//                                                          the displacement reference (a4), and the
+//                                                          position source of the step right after a rebuild
+//   vel     float4[ns]  u_x, u_y, u_z, mass               u = half-step velocity; updated in place
+//   svel    float4[ns]  vel permuted by the last rebuild  (source of the step right after a rebuild)
+//   vt[2]   float4[ns]  v~_x, v~_y, v~_z, tag (int bits)  DPD only: the velocity the dissipative force sees
+//   svt     float4[ns]  vt permuted by the last rebuild
+//   frc     float4[ns]  F_x, F_y, F_z, per-bead PE        materialised only by gm_compute_forces
+//   tag[2]  int[ns]     tag of the bead in each slot      double-buffered by rebuild parity (n_rebuilds & 1)
+//   rtag    int[ns]     slot of each tag
+//   nl      int4[n_tiles * capq * 32]  NL in tiles of 32 beads: entries 4q..4q+3 of bead (tile, lane)
+//                       are the int4 at (tile * capq + q) * 32 + lane; slots past NN hold the index n
+//                       (a far-away pad bead).  PAPER.md:L51, Fig. 1 (table form NL[k*Np+i], re-tiled)
+//   nn      int[ns]     NN[i];   nnw int[ns/32]: max NN per tile
+//   blt[2]  int[mb*ns]  BL in TAG space, storage order: blt[k*ns + i] = partner tag | btype << 28, -1 = none
+//   bl      int[mb*ns]  BL in index space: bl[k*ns + i] = j | btype << 28, -1 = none   PAPER.md:L97, Fig. 2
+//   cstart  int[n_cells + 1]   replaces CN: cell c holds slots [cstart[c], cstart[c+1])
+//   ccount  int[n_cells + 1]   histogram scratch (left zeroed by the scan)
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -22,6 +32,7 @@
 #define GM_PAD 256               // per-bead arrays are allocated (and table rows strided) in multiples of this
 #define GM_BOND_SHIFT 28
 #define GM_BOND_MASK ((1 << GM_BOND_SHIFT) - 1)
+#define GM_NEVER (~0ull)
 
 // latched device error bits (GmCtl::err)
 enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE = 4 };
@@ -30,11 +41,12 @@ enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE
 struct GmCtl {
     unsigned long long step[2];    // time level m, indexed by the parity of the current position buffer
     unsigned long long need;       // time level at which the NL must be rebuilt before forces (a4)
-    unsigned long long n_rebuilds;
+    unsigned long long rebuilt_at; // time level of the last rebuild: while == step, ref/svel/svt are current
+    unsigned long long n_rebuilds; // its low bit selects the current tag[] / blt[] buffers
     unsigned long long sum_nn;
     int max_nn;
     int err;
-    int built;                     // 1 once a list exists
+    int go;                        // decision of the last k_gate: the rebuild chain runs iff != 0
     int pad;
 };
 
@@ -45,8 +57,10 @@ struct GmPair { float c0, c1, c2, c3; };
 // Constants of one system, passed to kernels by value (constant bank).
 struct GmParams {
     int n, n_types, max_bonds, nl_cap;
-    int ns;                        // row stride of the NL and BL tables: n rounded up to GM_PAD elements
+    int ns;                        // padded bead count: n + 1 rounded up to GM_PAD (slot n is the far-away pad bead)
+    int capq;                      // nl_cap / 4: int4 quads per NL row
     int nc[3], n_cells;
+    int sfc_period;                // a rebuild (= SFC sort) is forced after this many steps without one; <= 0: never
     float box[3], half[3], inv_w[3];
     float r_list2, half_skin2;
     float edge_margin;             // r_list + r_skin: beads further than this from every face need no image test
@@ -57,28 +71,27 @@ struct GmParams {
     int pair_style, bond_style, integrator;
     GmPair pair[GM_MAX_TYPES * GM_MAX_TYPES];
     float bond_k[GM_MAX_BOND_TYPES], bond_r0[GM_MAX_BOND_TYPES];
+    float bond_c[GM_MAX_BOND_TYPES];   // FENE: 1 / R0^2
 };
 
-// Device pointers that do not ping-pong.
+// Device pointers.
 struct GmDev {
     float4 *pos[2];
-    float4 *vel;
-    float4 *vt[2];
-    float4 *frc;
     float4 *ref;
-    int *tag, *rtag;
-    int *nn, *nl;
-    int *nnw;                // max of NN over each group of 32 consecutive beads (tile height for the bulk loads)
-    int *bn, *bl;            // index space
-    int *bn_tag, *bl_tag;    // tag space master copy (bl_tag[k*N + tag] = partner tag | btype << 28)
+    float4 *vel, *svel;
+    float4 *vt[2], *svt;
+    float4 *frc;
+    int *tag[2], *rtag;
+    int *nn, *nnw;
+    int4 *nl;
+    int *bl;                 // index space
+    int *blt[2];             // tag space, storage order
+    int *bl_tag;             // tag space master copy in TAG order (bl_tag[k*ns + tag]), from gm_set_bonds
     int *key, *rank, *sorted;
-    int *cstart;             // n_cells + 1
+    int *cstart, *ccount;
     int *scan_sums;          // per scan block
-    uint32_t *cell_rank;     // SFC rank of each linear cell id
-    float4 *cpos;
-    float4 *tmp4;            // N float4 scratch (reorder)
-    int *tmpi;               // N int scratch (reorder)
-    float *stage;            // 10 N floats: I/O staging (pos3, vel3, force3, mass) ; reused as ints
+    uint32_t *row_rank;      // SFC rank of each (y, z) row of cells
+    float *stage;            // 11 ns floats: I/O staging (pos3, vel3, force3, type, mass)
     double *esum;            // [GM_ESUM_BLOCKS * 8] partials, then [8] totals at the end
     GmCtl *ctl;
 };
@@ -89,15 +102,15 @@ struct GmDev {
 
 enum { GM_MODE_STEP = 0, GM_MODE_FORCES = 1, GM_MODE_ENERGY = 2 };
 
-// ---- launch wrappers (each enqueues on `st`; `gate` != 0: run only if ctl->need == ctl->step[parity]) ----
-void gm_launch_sort_keys(const GmParams &P, const GmDev &D, const float4 *pos, int use_sfc_rank, int gate,
-                         int parity, cudaStream_t st);
-void gm_launch_cell_finish(const GmParams &P, const GmDev &D, const float4 *pos, int write_cpos, int gate,
-                           int parity, cudaStream_t st);
-void gm_launch_nl_build(const GmParams &P, const GmDev &D, const float4 *pos, int gate, int parity,
-                        cudaStream_t st);
-void gm_launch_reorder(const GmParams &P, GmDev &D, int cur, cudaStream_t st);   // uses D.sorted as the permutation
-void gm_launch_bonds_to_index(const GmParams &P, const GmDev &D, cudaStream_t st);
+// ---- launch wrappers (each enqueues on `st`; `gate` != 0: run only if ctl->need == ctl->step[parity];
+//      a rebuild is always skipped when the list is already current, ctl->rebuilt_at == ctl->step[parity]) ----
+void gm_launch_gate(const GmDev &D, int gate, int parity, unsigned long long cond_handle, int use_handle,
+                    cudaStream_t st);                                                  // decides, publishes ctl->go
+void gm_launch_sort(const GmParams &P, const GmDev &D, int parity, cudaStream_t st);    // a1 + a2 (if ctl->go)
+void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st);            // a3      (if ctl->go)
+cudaError_t gm_nl_prepare(const GmParams &P);
+int gm_nl_capacity_ok(const GmParams &P);
+void gm_launch_bonds_from_master(const GmParams &P, const GmDev &D, cudaStream_t st);
 void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
                      int lagged, cudaStream_t st);
 void gm_launch_pack(const GmParams &P, const GmDev &D, int cur, const float *pos3, const float *vel3,
@@ -106,11 +119,38 @@ void gm_launch_unpack(const GmParams &P, const GmDev &D, int cur, float *pos3, f
                       int lagged, cudaStream_t st);
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,
                                 cudaStream_t st);
-void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, cudaStream_t st);
-void gm_launch_gate(const GmDev &D, int parity, unsigned long long cond_handle, cudaStream_t st);
+void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, int parity, cudaStream_t st);
+void gm_launch_init_pad(const GmParams &P, const GmDev &D, cudaStream_t st);
 
 // ---- device helpers ---------------------------------------------------------------------------------
 #ifdef __CUDACC__
+// Does the rebuild run now?  gate = 0: forced (unless the list is already current at this time level).
+__device__ __forceinline__ bool gm_rebuild_off(const GmCtl *ctl, int gate, int parity)
+{
+    const unsigned long long m = ctl->step[parity];
+    return ctl->rebuilt_at == m || (gate && ctl->need != m);
+}
+
+// Where the current time level lives: right after a rebuild (ctl->rebuilt_at == step) the sorted copies
+// written by the sort are current; otherwise the ping-pong buffers of this parity.
+struct Src {
+    const float4 *__restrict__ pos;
+    const float4 *__restrict__ vel;
+    const float4 *__restrict__ vt;
+    const int *__restrict__ tag;
+};
+
+__device__ __forceinline__ Src current_src(const GmDev &D, int parity, unsigned long long step)
+{
+    const bool fresh = D.ctl->rebuilt_at == step;
+    Src s;
+    s.pos = fresh ? D.ref : D.pos[parity];
+    s.vel = fresh ? D.svel : D.vel;
+    s.vt = fresh ? D.svt : D.vt[parity];
+    s.tag = D.tag[D.ctl->n_rebuilds & 1ull];
+    return s;
+}
+
 // Minimum image of a - b in a periodic box (PAPER.md: Alg. 2 line 6, L458).  A direct a - b is exact
 // (Sterbenz) or rounded to half an ulp of the SMALL result when the pair does not cross the box; a
 // pair across the boundary has |a - b| ~ L, where the subtraction would round at ulp(L) -- so those

@@ -12,8 +12,8 @@ __device__ __forceinline__ float wrap_any(float x, float half, float L)
 }
 
 __global__ void __launch_bounds__(IO_BLOCK)
-k_pack(GmParams P, GmDev D, int cur, const float *__restrict__ pos3, const float *__restrict__ vel3,
-       const int *__restrict__ type, const float *__restrict__ mass)
+k_pack(const __grid_constant__ GmParams P, GmDev D, int cur, const float *__restrict__ pos3,
+       const float *__restrict__ vel3, const int *__restrict__ type, const float *__restrict__ mass)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
@@ -24,25 +24,26 @@ k_pack(GmParams P, GmDev D, int cur, const float *__restrict__ pos3, const float
     float vx = vel3[3 * i + 0], vy = vel3[3 * i + 1], vz = vel3[3 * i + 2];
     D.vel[i] = make_float4(vx, vy, vz, mass ? mass[i] : 1.0f);
     if (D.vt[0]) D.vt[cur][i] = make_float4(vx, vy, vz, __int_as_float(i));
-    D.tag[i] = i;
+    D.tag[0][i] = i;            // k_set_ctl(reset_all) selects buffer 0
     D.rtag[i] = i;
 }
 
 __global__ void __launch_bounds__(IO_BLOCK)
-k_unpack(GmParams P, GmDev D, int cur, float *__restrict__ pos3, float *__restrict__ vel3,
-         float *__restrict__ force3, int lagged)
+k_unpack(const __grid_constant__ GmParams P, GmDev D, int cur, float *__restrict__ pos3,
+         float *__restrict__ vel3, float *__restrict__ force3, int lagged)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
-    int t = D.tag[i];
+    const Src S = current_src(D, cur, D.ctl->step[cur]);
+    int t = S.tag[i];
     if (pos3) {
-        float4 p = D.pos[cur][i];
+        float4 p = S.pos[i];
         pos3[3 * t + 0] = p.x; pos3[3 * t + 1] = p.y; pos3[3 * t + 2] = p.z;
     }
     float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
     if (force3 || (vel3 && lagged)) f = D.frc[i];
     if (vel3) {
-        float4 u = D.vel[i];
+        float4 u = S.vel[i];
         if (lagged) {   // v^m = u^{m-1} + dt/2 a^m
             float h = 0.5f * P.dt / u.w;
             u.x += h * f.x; u.y += h * f.y; u.z += h * f.z;
@@ -64,30 +65,40 @@ void gm_launch_unpack(const GmParams &P, const GmDev &D, int cur, float *pos3, f
     k_unpack<<<(P.n + IO_BLOCK - 1) / IO_BLOCK, IO_BLOCK, 0, st>>>(P, D, cur, pos3, vel3, force3, lagged);
 }
 
-__global__ void k_set_ctl(GmDev D, unsigned long long step, int reset_all)
+// The far-away pad bead in slot n of every position array (NL quads are padded with index n), and
+// "no bond" (-1) in every bond table.
+__global__ void k_init_pad(const __grid_constant__ GmParams P, GmDev D)
 {
-    GmCtl *c = D.ctl;
-    c->step[0] = step;
-    c->step[1] = step;
-    c->need = ~0ull;
-    if (reset_all) {
-        c->n_rebuilds = 0; c->sum_nn = 0; c->max_nn = 0; c->err = 0; c->built = 0; c->pad = 0;
+    const float4 far = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+    const float4 zero = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = P.n + threadIdx.x; i < P.ns; i += blockDim.x) {
+        D.pos[0][i] = far; D.pos[1][i] = far; D.ref[i] = far;
+        D.vel[i] = zero; D.svel[i] = zero;
+        if (D.vt[0]) { D.vt[0][i] = zero; D.vt[1][i] = zero; D.svt[i] = zero; }
+        D.nn[i] = 0;
     }
 }
 
-void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, cudaStream_t st)
+void gm_launch_init_pad(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
-    k_set_ctl<<<1, 1, 0, st>>>(D, step, reset_all);
+    k_init_pad<<<1, 256, 0, st>>>(P, D);
 }
 
-// Gate of the conditional graph node that holds the rebuild kernels: body runs iff a rebuild is due
-// at this time level (a4).
-__global__ void k_gate(GmDev D, int parity, cudaGraphConditionalHandle h)
+__global__ void k_set_ctl(GmDev D, unsigned long long step, int reset_all, int parity)
 {
-    cudaGraphSetConditional(h, D.ctl->need == D.ctl->step[parity] ? 1u : 0u);
+    GmCtl *c = D.ctl;
+    const bool fresh = !reset_all && c->rebuilt_at == c->step[parity];
+    c->step[0] = step;
+    c->step[1] = step;
+    c->need = GM_NEVER;
+    c->rebuilt_at = fresh ? step : GM_NEVER;
+    c->go = 0;
+    if (reset_all) {
+        c->n_rebuilds = 0; c->sum_nn = 0; c->max_nn = 0; c->err = 0; c->pad = 0;
+    }
 }
 
-void gm_launch_gate(const GmDev &D, int parity, unsigned long long cond_handle, cudaStream_t st)
+void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, int parity, cudaStream_t st)
 {
-    k_gate<<<1, 1, 0, st>>>(D, parity, (cudaGraphConditionalHandle)cond_handle);
+    k_set_ctl<<<1, 1, 0, st>>>(D, step, reset_all, parity);
 }

@@ -3,62 +3,64 @@
 // that the target particle resides in)", all neighbors "within a distance that is the sum of the
 // cutoff ... r_cut, and the buffer distance, r_buffer"; table form NL[k*Np + i], NN[i]: L51, Fig. 1).
 //
-// One thread per bead, in storage (SFC) order so a warp's beads sit in a handful of adjacent cells
-// and share their candidate segments through L1.  The cell list is CSR over x-fastest linear cell
-// ids, so the three x-adjacent cells of one (y, z) row form one contiguous segment of cpos[]: nine
-// segments per bead instead of 27 (two extra pieces where the row wraps around the box).
+// Runs right after the sort of gm_sort.cu, so bead index == slot in the cell-sorted array `ref`: one
+// thread per bead, a warp owns 32 consecutive beads (a few adjacent cells of one x row), its lanes
+// read the same or adjacent candidates at every iteration and run nearly equal trip counts.  Cells run
+// along x inside a row, so the three x-adjacent cells of one (y, z) row are one contiguous run of
+// ref[]: nine runs per bead instead of 27 cells (two more where the row wraps around the box).
+//
+// The warp collects its 32 rows in shared memory (row k of lane l at [k][l]: conflict-free, and private
+// to the lane, so no synchronisation) and writes them out as whole int4 quads of its own NL tile
+// (gm_internal.cuh: entries 4q..4q+3 of a bead are one int4, the 32 int4 of a quad are contiguous):
+// coalesced 512-byte stores, and coalesced 512-byte loads in the force kernel.
 #include "gm_internal.cuh"
 
-#define NL_BLOCK 128
+extern __shared__ int nl_rows[];     // [warps per block][nl_cap][32]
 
-// One row piece: candidates cpos[s0 .. s1) against bead i.  SHIFT: the piece lies across a periodic face
-// in some dimension; the displacement is then taken relative to the two faces, (a -+ L/2) - (b +- L/2)
-// (see gm_min_image), with the bead side (ax, ay, az) prepared once per piece and the candidate side
+// One run of candidates ref[s0 .. s1) against bead i.  SHIFT: the run lies across a periodic face in
+// some dimension; the displacement is then taken relative to the two faces, (a -+ L/2) - (b +- L/2)
+// (see gm_min_image), with the bead side (ax, ay, az) prepared once per run and the candidate side
 // b + (hx, hy, hz) per candidate -- no branches in the loop.
 template <bool SHIFT>
-__device__ __forceinline__ int nl_scan_piece(const float4 *__restrict__ cpos, int s0, int s1, int i, float ax,
-                                             float ay, float az, float hx, float hy, float hz, float r_list2,
-                                             int k, int cap, int *__restrict__ col, size_t col_stride)
+__device__ __forceinline__ int nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
+                                           float ay, float az, float hx, float hy, float hz, float r_list2,
+                                           int k, int cap, int *__restrict__ row)
 {
 #pragma unroll 4
     for (int s = s0; s < s1; ++s) {
-        const float4 q = cpos[s];
+        const float4 q = __ldg(ref + s);
         float dx, dy, dz;
         if (SHIFT) { dx = ax - (q.x + hx); dy = ay - (q.y + hy); dz = az - (q.z + hz); }
         else { dx = ax - q.x; dy = ay - q.y; dz = az - q.z; }
         const float r2 = dx * dx + dy * dy + dz * dz;
-        const int j = __float_as_int(q.w);
-        if (r2 < r_list2 && j != i) {
-            if (k < cap) col[(size_t)k * col_stride] = j;
+        if (r2 < r_list2 && s != i) {
+            if (k < cap) row[k * 32] = s;
             ++k;
         }
     }
     return k;
 }
 
-// Thread s owns the bead in slot s of the cell-sorted array cpos[] (not storage bead s): the 32 beads
-// of a warp then sit in a few consecutive cells of one x row, so at every loop iteration the lanes read
-// the same or adjacent candidates (few L1 wavefronts per request) and run nearly equal trip counts.
-__global__ void __launch_bounds__(NL_BLOCK)
-k_nl_build(const __grid_constant__ GmParams P, GmDev D, int gate, int parity)
+__global__ void __launch_bounds__(128)
+k_nl_build(const __grid_constant__ GmParams P, GmDev D)
 {
-    if (gate && D.ctl->need != D.ctl->step[parity]) return;
-    const int s = blockIdx.x * blockDim.x + threadIdx.x;
-    const size_t ns = (size_t)P.ns;
+    if (!D.ctl->go) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int cap = P.nl_cap;
+    int *__restrict__ row = nl_rows + (size_t)wid * cap * 32 + lane;
     int k = 0;
-    if (s < P.n) {
-        const float4 *__restrict__ cpos = D.cpos;
+    if (i < P.n) {
+        const float4 *__restrict__ ref = D.ref;
         const int *__restrict__ cstart = D.cstart;
-        const float4 pi = cpos[s];
-        const int i = __float_as_int(pi.w);
-        int *__restrict__ col = D.nl + i;
+        const uint32_t *__restrict__ rr = D.row_rank;
+        const float4 pi = ref[i];
         const int cx = gm_cell_coord(pi.x, P.half[0], P.inv_w[0], P.nc[0]);
         const int cy = gm_cell_coord(pi.y, P.half[1], P.inv_w[1], P.nc[1]);
         const int cz = gm_cell_coord(pi.z, P.half[2], P.inv_w[2], P.nc[2]);
         const int ncx = P.nc[0], ncy = P.nc[1], ncz = P.nc[2];
         const float rl2 = P.r_list2;
-        // x pieces of a row: cells [xa0, xa1] are contiguous in cpos; a bead in an edge column also
+        // x pieces of a row: cells [xa0, xa1] are contiguous in ref; a bead in an edge column also
         // sees the single cell xb on the other side of the box
         const int xa0 = max(cx - 1, 0), xa1 = min(cx + 1, ncx - 1);
         const int xb = (cx == 0) ? ncx - 1 : ((cx == ncx - 1) ? 0 : -1);
@@ -67,9 +69,9 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D, int gate, int parity)
         if (inner) {
             for (int oz = -1; oz <= 1; ++oz)
                 for (int oy = -1; oy <= 1; ++oy) {
-                    const int row = ((cz + oz) * ncy + cy + oy) * ncx;
-                    k = nl_scan_piece<false>(cpos, cstart[row + xa0], cstart[row + xa1 + 1], i, pi.x, pi.y, pi.z,
-                                             0.f, 0.f, 0.f, rl2, k, cap, col, ns);
+                    const int r0 = (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
+                    k = nl_scan_run<false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
+                                           pi.y, pi.z, 0.f, 0.f, 0.f, rl2, k, cap, row);
                 }
         } else {
             for (int oz = -1; oz <= 1; ++oz) {
@@ -82,49 +84,83 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D, int gate, int parity)
                     float ay = pi.y, hy = 0.f;
                     if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
                     else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
-                    const int row = (z * ncy + y) * ncx;
-                    k = nl_scan_piece<true>(cpos, cstart[row + xa0], cstart[row + xa1 + 1], i, pi.x, ay, az,
-                                            0.f, hy, hz, rl2, k, cap, col, ns);
+                    const int r0 = (int)__ldg(rr + z * ncy + y) * ncx;
+                    k = nl_scan_run<true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay,
+                                          az, 0.f, hy, hz, rl2, k, cap, row);
                     if (xb >= 0)
-                        k = nl_scan_piece<true>(cpos, cstart[row + xb], cstart[row + xb + 1], i, pi.x - hxb, ay, az,
-                                                hxb, hy, hz, rl2, k, cap, col, ns);
+                        k = nl_scan_run<true>(ref, __ldg(cstart + r0 + xb), __ldg(cstart + r0 + xb + 1), i,
+                                              pi.x - hxb, ay, az, hxb, hy, hz, rl2, k, cap, row);
                 }
             }
         }
-        const int kc = min(k, cap);
-        D.nn[i] = kc;
-        D.ref[i] = make_float4(pi.x, pi.y, pi.z, 0.f);
-        atomicMax(&D.nnw[i >> 5], kc);     // tile height for the step kernel's bulk loads (cleared in k_sort_clear)
         if (k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
+        // a7 set-up: BL of this slot in index space from its tag-space row (the sort moved the beads)
+        const int sel = (int)(D.ctl->n_rebuilds & 1ull);
+        const size_t ns = (size_t)P.ns;
+        for (int b = 0; b < P.max_bonds; ++b) {
+            const int e = D.blt[sel][b * ns + i];
+            D.bl[b * ns + i] = e < 0 ? -1 : (D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK));
+        }
     }
     const int kc = min(k, cap);
+    const int nq = (kc + 3) >> 2;
+    for (int kk = kc; kk < 4 * nq; ++kk) row[kk * 32] = P.n;      // pad the last quad with the far-away bead
+    if (i < P.ns) D.nn[i] = kc;
+    int4 *__restrict__ tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
+    for (int q = 0; q < nq; ++q)
+        tile[q * 32] = make_int4(row[(4 * q) * 32], row[(4 * q + 1) * 32], row[(4 * q + 2) * 32],
+                                 row[(4 * q + 3) * 32]);
     const int m = __reduce_max_sync(0xffffffffu, kc);
     const unsigned int sum = __reduce_add_sync(0xffffffffu, (unsigned int)kc);
-    if ((threadIdx.x & 31) == 0 && sum > 0) {
-        atomicMax(&D.ctl->max_nn, m);
-        atomicAdd(&D.ctl->sum_nn, (unsigned long long)sum);
+    if (lane == 0) {
+        D.nnw[i >> 5] = m;
+        if (sum > 0) {
+            atomicMax(&D.ctl->max_nn, m);
+            atomicAdd(&D.ctl->sum_nn, (unsigned long long)sum);
+        }
     }
-    if (blockIdx.x == 0 && threadIdx.x == 0) D.ctl->built = 1;
 }
 
-void gm_launch_nl_build(const GmParams &P, const GmDev &D, const float4 *pos, int gate, int parity,
-                        cudaStream_t st)
+static int nl_warps_per_block(const GmParams &P)
 {
-    (void)pos;
-    k_nl_build<<<(P.n + NL_BLOCK - 1) / NL_BLOCK, NL_BLOCK, 0, st>>>(P, D, gate, parity);
+    const size_t per_warp = (size_t)P.nl_cap * 32 * sizeof(int);
+    int w = (int)((200u * 1024u) / per_warp);
+    return w > 4 ? 4 : w;
+}
+
+int gm_nl_capacity_ok(const GmParams &P) { return nl_warps_per_block(P) >= 1; }
+
+// Once per system (not during graph capture): opt in to more than 48 KB of dynamic shared memory.
+cudaError_t gm_nl_prepare(const GmParams &P)
+{
+    const size_t smem = (size_t)nl_warps_per_block(P) * P.nl_cap * 32 * sizeof(int);
+    if (smem > 48 * 1024)
+        return cudaFuncSetAttribute(k_nl_build, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+    return cudaSuccess;
+}
+
+void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
+{
+    const int w = nl_warps_per_block(P);
+    const size_t smem = (size_t)w * P.nl_cap * 32 * sizeof(int);
+    const int threads = w * 32;
+    k_nl_build<<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors): nn_out[tag], nl_out[tag*stride + k].
 __global__ void __launch_bounds__(256)
-k_unpack_neighbors(GmParams P, GmDev D, int *__restrict__ nn_out, int *__restrict__ nl_out, long long stride)
+k_unpack_neighbors(const __grid_constant__ GmParams P, GmDev D, int *__restrict__ nn_out,
+                   int *__restrict__ nl_out, long long stride)
 {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
-    int t = D.tag[i];
-    int nn = D.nn[i];
+    const int *__restrict__ tag = D.tag[D.ctl->n_rebuilds & 1ull];
+    const int t = tag[i];
+    const int nn = D.nn[i];
     nn_out[t] = nn;
+    const int *__restrict__ tile = reinterpret_cast<const int *>(D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31));
     for (int k = 0; k < nn && k < stride; ++k)
-        nl_out[(long long)t * stride + k] = D.tag[D.nl[(size_t)k * P.ns + i]];
+        nl_out[(long long)t * stride + k] = tag[tile[(k >> 2) * 128 + (k & 3)]];
 }
 
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,

@@ -1,60 +1,69 @@
-// gm_sort.cu -- a1 cell binning by counting sort, a2 SFC reorder (PAPER.md:L57,
-// Alg. 1 Kernel 1 L376-388 for what a cell list holds; L33/L199 for the memory sort).
+// gm_sort.cu -- a1 cell binning by counting sort, fused with a2, the space-filling-curve reorder of the
+// particle arrays (PAPER.md:L57 and Alg. 1 Kernel 1 L376-388 for what a cell list holds;
+// L33/L199 for the memory sort).
 //
-// The paper claims a slot per particle with atomicInc into a fixed-slot CL table.  Here the cell
-// list is CSR: key -> histogram -> exclusive scan -> scatter, then every cell's segment is sorted by
-// storage index so that the result (and with it the NL row order and every fp32 sum downstream)
-// is the same on every run, whatever order the histogram atomics were served in.
+// The paper claims a slot per particle with atomicInc into a fixed-slot CL table and re-sorts memory
+// now and then with SFCPACK.  Here ONE counting sort does both, at every rebuild: the sort key of a
+// bead is the rank of its cell along the curve (cells run along x inside a row; the (y, z) rows follow
+// a 2-D Hilbert curve), and all per-bead state is moved into that order.  Afterwards
+//   - the sorted position array `ref` IS the cell list (CSR: cell c = slots [cstart[c], cstart[c+1])),
+//     the three x-adjacent cells of a row are one contiguous run, and slot index == bead index, so the
+//     neighbor search (gm_nlist.cu) needs no indirection and writes whole tiles of the NL table;
+//   - the 32 beads of a warp of the force kernel sit in a few adjacent cells: their gathers hit the
+//     same cache lines and their list lengths are alike.
+// Within a cell, beads are ordered by their previous slot, so the result (and with it every fp32 sum
+// downstream) is the same on every run whatever order the histogram atomics were served in.
 //
-// One counting sort serves both uses:
-//   use_sfc_rank = 0: key = linear cell id (x fastest)  -> cstart[], cpos[]   (a1, every rebuild)
-//   use_sfc_rank = 1: key = Hilbert rank of that cell   -> permutation sorted[] (a2, every sfc_period)
+// Chain: k_gate (decide, publish ctl->go) -> k_keys (key + histogram) -> k_scan_local / k_scan_add
+// (exclusive scan -> cstart) -> k_scatter (slot lists per cell) -> k_permute (canonical slot, move state)
+// -> k_nl_build (gm_nlist.cu).
 #include "gm_internal.cuh"
 
 #define SORT_BLOCK 256
 
-__device__ __forceinline__ bool gm_gated_off(const GmCtl *ctl, int gate, int parity)
+// Decide whether the rebuild runs at this time level and publish the decision (every later kernel of
+// the chain only reads ctl->go).  With a conditional graph node the body is skipped altogether.
+__global__ void k_gate(GmDev D, int gate, int parity, cudaGraphConditionalHandle h, int use_handle)
 {
-    return gate && ctl->need != ctl->step[parity];
-}
-
-__global__ void __launch_bounds__(SORT_BLOCK)
-k_sort_clear(GmParams P, GmDev D, int use_sfc_rank, int gate, int parity)
-{
-    if (gm_gated_off(D.ctl, gate, parity)) return;
-    int stride = gridDim.x * blockDim.x;
-    for (int c = blockIdx.x * blockDim.x + threadIdx.x; c <= P.n_cells; c += stride) D.cstart[c] = 0;
-    if (!use_sfc_rank)
-        for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < P.ns / 32; c += stride) D.nnw[c] = 0;
-    if (!use_sfc_rank && blockIdx.x == 0 && threadIdx.x == 0) {
-        D.ctl->n_rebuilds += 1;
-        D.ctl->max_nn = 0;
-        D.ctl->sum_nn = 0;
+    GmCtl *c = D.ctl;
+    const int go = gm_rebuild_off(c, gate, parity) ? 0 : 1;
+    c->go = go;
+    if (go) {
+        c->rebuilt_at = c->step[parity];
+        c->n_rebuilds += 1;
+        c->max_nn = 0;
+        c->sum_nn = 0;
     }
+    if (use_handle) cudaGraphSetConditional(h, (unsigned)go);
+}
+
+void gm_launch_gate(const GmDev &D, int gate, int parity, unsigned long long cond_handle, int use_handle,
+                    cudaStream_t st)
+{
+    k_gate<<<1, 1, 0, st>>>(D, gate, parity, (cudaGraphConditionalHandle)cond_handle, use_handle);
 }
 
 __global__ void __launch_bounds__(SORT_BLOCK)
-k_sort_keys(GmParams P, GmDev D, const float4 *__restrict__ pos, int use_sfc_rank, int gate, int parity)
+k_keys(const __grid_constant__ GmParams P, GmDev D, int parity)
 {
-    if (gm_gated_off(D.ctl, gate, parity)) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!D.ctl->go) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
-    float4 p = pos[i];
+    const float4 p = D.pos[parity][i];
     int key = 0;
     if (isfinite(p.x) && isfinite(p.y) && isfinite(p.z)) {
-        int cx = gm_cell_coord(p.x, P.half[0], P.inv_w[0], P.nc[0]);
-        int cy = gm_cell_coord(p.y, P.half[1], P.inv_w[1], P.nc[1]);
-        int cz = gm_cell_coord(p.z, P.half[2], P.inv_w[2], P.nc[2]);
-        key = (cz * P.nc[1] + cy) * P.nc[0] + cx;
-        if (use_sfc_rank) key = (int)D.cell_rank[key];
+        const int cx = gm_cell_coord(p.x, P.half[0], P.inv_w[0], P.nc[0]);
+        const int cy = gm_cell_coord(p.y, P.half[1], P.inv_w[1], P.nc[1]);
+        const int cz = gm_cell_coord(p.z, P.half[2], P.inv_w[2], P.nc[2]);
+        key = (int)D.row_rank[cz * P.nc[1] + cy] * P.nc[0] + cx;
     } else {
         atomicOr(&D.ctl->err, GM_DEV_ERR_NONFINITE);
     }
     D.key[i] = key;
-    D.rank[i] = atomicAdd(&D.cstart[key], 1);     // arrival order; made canonical in k_cell_finish
+    D.rank[i] = atomicAdd(&D.ccount[key], 1);     // arrival order; made canonical in k_permute
 }
 
-// ---- exclusive scan of cstart[0 .. n_cells] (n_cells + 1 entries, the last count is 0) ----------
+// ---- exclusive scan of ccount[0 .. n_cells] into cstart (n_cells + 1 entries, the last count is 0) ----
 __device__ __forceinline__ int block_exclusive_scan(int v, int *total)
 {
     __shared__ int warp_sums[32];
@@ -85,19 +94,28 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int *total)
     return r;
 }
 
+// Block-local exclusive scan; leaves ccount zeroed for the next rebuild.
 __global__ void __launch_bounds__(GM_SCAN_BLOCK)
-k_scan_local(GmParams P, GmDev D, int gate, int parity)
+k_scan_local(const __grid_constant__ GmParams P, GmDev D)
 {
-    if (gm_gated_off(D.ctl, gate, parity)) return;
+    if (!D.ctl->go) return;
     __shared__ int total;
-    int n = P.n_cells + 1;
-    int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
+    const int n = P.n_cells + 1;
+    const int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
     int v[GM_SCAN_ITEMS], s = 0;
+    if (base + GM_SCAN_ITEMS <= n) {
+        const int4 q = *reinterpret_cast<const int4 *>(D.ccount + base);
+        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
+        *reinterpret_cast<int4 *>(D.ccount + base) = make_int4(0, 0, 0, 0);
+    } else {
 #pragma unroll
-    for (int q = 0; q < GM_SCAN_ITEMS; ++q) {
-        v[q] = (base + q < n) ? D.cstart[base + q] : 0;
-        s += v[q];
+        for (int q = 0; q < GM_SCAN_ITEMS; ++q) {
+            v[q] = (base + q < n) ? D.ccount[base + q] : 0;
+            if (base + q < n) D.ccount[base + q] = 0;
+        }
     }
+#pragma unroll
+    for (int q = 0; q < GM_SCAN_ITEMS; ++q) s += v[q];
     int off = block_exclusive_scan(s, &total);
 #pragma unroll
     for (int q = 0; q < GM_SCAN_ITEMS; ++q) {
@@ -107,144 +125,99 @@ k_scan_local(GmParams P, GmDev D, int gate, int parity)
     if (threadIdx.x == 0) D.scan_sums[blockIdx.x] = total;
 }
 
+// Each block adds the sum of the totals of the blocks before it (a few hundred at most).
 __global__ void __launch_bounds__(GM_SCAN_BLOCK)
-k_scan_sums(GmParams P, GmDev D, int n_blocks, int gate, int parity)
+k_scan_add(const __grid_constant__ GmParams P, GmDev D)
 {
-    if (gm_gated_off(D.ctl, gate, parity)) return;
-    __shared__ int total;
-    int carry = 0;
-    for (int b0 = 0; b0 < n_blocks; b0 += GM_SCAN_BLOCK) {
-        int idx = b0 + threadIdx.x;
-        int v = idx < n_blocks ? D.scan_sums[idx] : 0;
-        int off = block_exclusive_scan(v, &total);
-        if (idx < n_blocks) D.scan_sums[idx] = carry + off;
-        carry += total;
-        __syncthreads();
+    if (!D.ctl->go) return;
+    __shared__ int warp_part[32];
+    __shared__ int add_sh;
+    int part = 0;
+    for (int b = threadIdx.x; b < (int)blockIdx.x; b += GM_SCAN_BLOCK) part += D.scan_sums[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_down_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = part;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int v = warp_part[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) add_sh = v;
     }
-}
-
-__global__ void __launch_bounds__(GM_SCAN_BLOCK)
-k_scan_add(GmParams P, GmDev D, int gate, int parity)
-{
-    if (gm_gated_off(D.ctl, gate, parity)) return;
-    int n = P.n_cells + 1;
-    int add = D.scan_sums[blockIdx.x];
-    int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
+    __syncthreads();
+    const int add = add_sh;
+    const int n = P.n_cells + 1;
+    const int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
 #pragma unroll
     for (int q = 0; q < GM_SCAN_ITEMS; ++q)
         if (base + q < n) D.cstart[base + q] += add;
 }
 
 __global__ void __launch_bounds__(SORT_BLOCK)
-k_sort_scatter(GmParams P, GmDev D, int gate, int parity)
+k_scatter(const __grid_constant__ GmParams P, GmDev D)
 {
-    if (gm_gated_off(D.ctl, gate, parity)) return;
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!D.ctl->go) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
     D.sorted[D.cstart[D.key[i]] + D.rank[i]] = i;
 }
 
-// One thread per key: put the segment into ascending storage-index order (segments are a handful
-// of beads: 3 to 19 per cell in the five configs), then, for the cell list, gather the coordinates.
+// a2: thread i = old slot.  Its new slot is the start of its cell plus the number of beads of that cell
+// that had a smaller old slot (canonical order); then every per-bead array follows.
 __global__ void __launch_bounds__(SORT_BLOCK)
-k_cell_finish(GmParams P, GmDev D, const float4 *__restrict__ pos, int write_cpos, int gate, int parity)
+k_permute(const __grid_constant__ GmParams P, GmDev D, int parity)
 {
-    if (gm_gated_off(D.ctl, gate, parity)) return;
-    int c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= P.n_cells) return;
-    int b = D.cstart[c], e = D.cstart[c + 1];
-    for (int s = b + 1; s < e; ++s) {
-        int v = D.sorted[s];
-        int t = s - 1;
-        while (t >= b && D.sorted[t] > v) { D.sorted[t + 1] = D.sorted[t]; --t; }
-        D.sorted[t + 1] = v;
-    }
-    if (write_cpos)
-        for (int s = b; s < e; ++s) {
-            int idx = D.sorted[s];
-            float4 p = pos[idx];
-            D.cpos[s] = make_float4(p.x, p.y, p.z, __int_as_float(idx));
-        }
-}
-
-void gm_launch_sort_keys(const GmParams &P, const GmDev &D, const float4 *pos, int use_sfc_rank, int gate,
-                         int parity, cudaStream_t st)
-{
-    int nb = (P.n + SORT_BLOCK - 1) / SORT_BLOCK;
-    int per = GM_SCAN_BLOCK * GM_SCAN_ITEMS;
-    int nsb = (P.n_cells + 1 + per - 1) / per;
-    int ncb = (P.n_cells + 1 + SORT_BLOCK - 1) / SORT_BLOCK;
-    if (ncb > 1184) ncb = 1184;
-    k_sort_clear<<<ncb, SORT_BLOCK, 0, st>>>(P, D, use_sfc_rank, gate, parity);
-    k_sort_keys<<<nb, SORT_BLOCK, 0, st>>>(P, D, pos, use_sfc_rank, gate, parity);
-    k_scan_local<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D, gate, parity);
-    k_scan_sums<<<1, GM_SCAN_BLOCK, 0, st>>>(P, D, nsb, gate, parity);
-    k_scan_add<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D, gate, parity);
-    k_sort_scatter<<<nb, SORT_BLOCK, 0, st>>>(P, D, gate, parity);
-}
-
-void gm_launch_cell_finish(const GmParams &P, const GmDev &D, const float4 *pos, int write_cpos, int gate,
-                           int parity, cudaStream_t st)
-{
-    int nb = (P.n_cells + SORT_BLOCK - 1) / SORT_BLOCK;
-    k_cell_finish<<<nb, SORT_BLOCK, 0, st>>>(P, D, pos, write_cpos, gate, parity);
-}
-
-// ---- a2: apply the permutation sorted[new] = old to every per-bead array --------------------------
-__global__ void __launch_bounds__(SORT_BLOCK)
-k_permute4(int n, const int *__restrict__ perm, const float4 *__restrict__ src, float4 *__restrict__ dst)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) dst[i] = src[perm[i]];
-}
-
-__global__ void __launch_bounds__(SORT_BLOCK)
-k_permute_tag(int n, const int *__restrict__ perm, const int *__restrict__ src, int *__restrict__ dst)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) dst[i] = src[perm[i]];
-}
-
-__global__ void __launch_bounds__(SORT_BLOCK)
-k_set_rtag(int n, const int *__restrict__ tag_new, int *__restrict__ tag, int *__restrict__ rtag)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < n) { int t = tag_new[i]; tag[i] = t; rtag[t] = i; }
-}
-
-void gm_launch_reorder(const GmParams &P, GmDev &D, int cur, cudaStream_t st)
-{
-    int n = P.n, nb = (n + SORT_BLOCK - 1) / SORT_BLOCK;
-    size_t b4 = (size_t)n * sizeof(float4);
-    k_permute4<<<nb, SORT_BLOCK, 0, st>>>(n, D.sorted, D.pos[cur], D.tmp4);
-    cudaMemcpyAsync(D.pos[cur], D.tmp4, b4, cudaMemcpyDeviceToDevice, st);
-    k_permute4<<<nb, SORT_BLOCK, 0, st>>>(n, D.sorted, D.vel, D.tmp4);
-    cudaMemcpyAsync(D.vel, D.tmp4, b4, cudaMemcpyDeviceToDevice, st);
-    if (D.vt[0]) {
-        k_permute4<<<nb, SORT_BLOCK, 0, st>>>(n, D.sorted, D.vt[cur], D.tmp4);
-        cudaMemcpyAsync(D.vt[cur], D.tmp4, b4, cudaMemcpyDeviceToDevice, st);
-    }
-    k_permute_tag<<<nb, SORT_BLOCK, 0, st>>>(n, D.sorted, D.tag, D.tmpi);
-    k_set_rtag<<<nb, SORT_BLOCK, 0, st>>>(n, D.tmpi, D.tag, D.rtag);
-}
-
-// BL/BN in index space from the tag-space master table (the tags in column i of BL
-// are the beads bonded to i; stored under both ends).
-__global__ void __launch_bounds__(SORT_BLOCK) k_bonds_to_index(GmParams P, GmDev D)
-{
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (!D.ctl->go) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
-    int t = D.tag[i];
-    int nb = D.bn_tag[t];
-    D.bn[i] = nb;
-    for (int k = 0; k < nb; ++k) {
-        int e = D.bl_tag[(size_t)k * P.n + t];
-        D.bl[(size_t)k * P.ns + i] = D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK);
+    const int sel = (int)(D.ctl->n_rebuilds & 1ull);       // buffers this rebuild writes
+    const float4 p = D.pos[parity][i];
+    const float4 u = D.vel[i];
+    const int t = D.tag[sel ^ 1][i];
+    const int c = D.key[i];
+    const int b = D.cstart[c], e = D.cstart[c + 1];
+    int r = 0;
+    for (int s = b; s < e; ++s) r += (D.sorted[s] < i) ? 1 : 0;
+    const int d = b + r;
+    D.ref[d] = p;
+    D.svel[d] = u;
+    if (D.svt) D.svt[d] = D.vt[parity][i];
+    D.tag[sel][d] = t;
+    D.rtag[t] = d;
+    const size_t ns = (size_t)P.ns;
+    for (int k = 0; k < P.max_bonds; ++k) D.blt[sel][k * ns + d] = D.blt[sel ^ 1][k * ns + i];
+}
+
+void gm_launch_sort(const GmParams &P, const GmDev &D, int parity, cudaStream_t st)
+{
+    const int nb = (P.n + SORT_BLOCK - 1) / SORT_BLOCK;
+    const int per = GM_SCAN_BLOCK * GM_SCAN_ITEMS;
+    const int nsb = (P.n_cells + 1 + per - 1) / per;
+    k_keys<<<nb, SORT_BLOCK, 0, st>>>(P, D, parity);
+    k_scan_local<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D);
+    k_scan_add<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D);
+    k_scatter<<<nb, SORT_BLOCK, 0, st>>>(P, D);
+    k_permute<<<nb, SORT_BLOCK, 0, st>>>(P, D, parity);
+}
+
+// BL in tag space, storage order, from the tag-order master table written by gm_set_bonds
+// (column i of BL holds the beads bonded to i; each bond is stored under both ends).
+__global__ void __launch_bounds__(SORT_BLOCK) k_bonds_from_master(const __grid_constant__ GmParams P, GmDev D)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    const int sel = (int)(D.ctl->n_rebuilds & 1ull);
+    const int t = D.tag[sel][i];
+    const size_t ns = (size_t)P.ns;
+    for (int k = 0; k < P.max_bonds; ++k) {
+        const int e = D.bl_tag[k * ns + t];
+        D.blt[sel][k * ns + i] = e;
+        D.bl[k * ns + i] = e < 0 ? -1 : (D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK));
     }
 }
 
-void gm_launch_bonds_to_index(const GmParams &P, const GmDev &D, cudaStream_t st)
+void gm_launch_bonds_from_master(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     if (P.max_bonds <= 0) return;
-    k_bonds_to_index<<<(P.n + SORT_BLOCK - 1) / SORT_BLOCK, SORT_BLOCK, 0, st>>>(P, D);
+    k_bonds_from_master<<<(P.n + SORT_BLOCK - 1) / SORT_BLOCK, SORT_BLOCK, 0, st>>>(P, D);
 }

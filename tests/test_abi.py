@@ -83,16 +83,21 @@ def test_create_rejects_null_workspace_without_touching_cuda(gm):
 
 
 def test_sfc_cell_order_is_a_hilbert_permutation(gm):
-    # a permutation of the cells for any grid; on a 2^k cube consecutive cells are face neighbors
+    # a permutation of the cells for any grid; cells run along x inside a row, and on a 2^k grid
+    # consecutive (y, z) rows are edge neighbors (2-D Hilbert curve over the rows)
     for nc in ([8, 8, 8], [5, 7, 3], [13, 13, 13]):
         r = gm.gm_sfc_cell_order(nc)
         assert sorted(r.tolist()) == list(range(nc[0] * nc[1] * nc[2]))
-    r = gm.gm_sfc_cell_order([8, 8, 8])
-    inv = np.argsort(r)
-    xyz = np.stack([inv % 8, (inv // 8) % 8, inv // 64], axis=1)
-    assert (np.abs(np.diff(xyz, axis=0)).sum(axis=1) == 1).all()
-    # locality on a clipped grid: the mean jump stays close to 1 cell
-    r = gm.gm_sfc_cell_order([13, 13, 13])
-    inv = np.argsort(r)
-    xyz = np.stack([inv % 13, (inv // 13) % 13, inv // 169], axis=1)
-    assert np.abs(np.diff(xyz, axis=0)).sum(axis=1).mean() < 1.5
+        r3 = r.reshape(nc[2], nc[1], nc[0]).astype(np.int64)
+        assert (np.diff(r3, axis=2) == 1).all()            # x-adjacent cells are memory neighbors
+        assert (r3[:, :, 0] % nc[0] == 0).all()
+    r = gm.gm_sfc_cell_order([4, 8, 8]).reshape(8, 8, 4)
+    row = (r[:, :, 0] // 4).astype(np.int64)            # rank of row (z, y)
+    inv = np.argsort(row.reshape(-1))
+    zy = np.stack([inv // 8, inv % 8], axis=1)
+    assert (np.abs(np.diff(zy, axis=0)).sum(axis=1) == 1).all()
+    # locality on a clipped grid: the mean jump between consecutive rows stays close to 1 row
+    r = gm.gm_sfc_cell_order([3, 13, 13]).reshape(13, 13, 3)
+    inv = np.argsort((r[:, :, 0] // 3).reshape(-1))
+    zy = np.stack([inv // 13, inv % 13], axis=1)
+    assert np.abs(np.diff(zy, axis=0)).sum(axis=1).mean() < 1.5
