@@ -99,6 +99,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     cap = (cap + 7) / 8 * 8;
     P->nl_cap = cap;
     P->capq = cap / 4;
+    P->minq = std::min(4, P->capq);
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
     for (int t = 0; t < GM_MAX_TYPES * GM_MAX_TYPES; ++t) { P->pair[t].c0 = 0.f; P->pair[t].c1 = 0.f; P->pair[t].c2 = 0.f; P->pair[t].c3 = 0.f; }
     return GM_OK;

@@ -24,6 +24,12 @@
 #include "gm_internal.cuh"
 
 #define FORCE_BLOCK 128
+#ifndef GM_FORCE_MINB
+#define GM_FORCE_MINB 1          // minimum resident blocks per SM the step kernel is compiled for
+#endif
+#ifndef GM_LJ_NQ
+#define GM_LJ_NQ 2               // quads (of 4 list entries) per batch of the LJ gather loop
+#endif
 
 struct BeadForce {
     float fx, fy, fz;
@@ -33,16 +39,27 @@ struct BeadForce {
 
 // One list entry of the pair loop (Alg. 2: displacement, cutoff test, accumulate).  The LJ term is
 // branch-free (out-of-range entries, and the far-away pad bead, select 0).
+struct Own {                 // per-bead constants of the pair loop
+    float4 p;                // position, type
+    float ax, ay, az;        // p - hs          (MI path only)
+    float hx, hy, hz;        // copysign(L/2, p)
+    float4 vt;               // DPD: v~, tag
+    int t;                   // type
+};
+
 template <int PAIR, bool NT1, bool ENERGY, bool MI>
-__device__ __forceinline__ void pair_term(const GmParams &P, const float4 pi, const int ti, const float4 vti,
-                                          const float4 pj, const float4 vtj, const GmPair p0, uint32_t step,
-                                          float &fx, float &fy, float &fz, float &pe, float &cnt)
+__device__ __forceinline__ void pair_term(const GmParams &P, const Own &me, const float4 pj, const float4 vtj,
+                                          const GmPair p0, uint32_t step, float &fx, float &fy, float &fz,
+                                          float &pe, float &cnt)
 {
+    const float4 pi = me.p;
+    const float4 vti = me.vt;
+    const int ti = me.t;
     float dx, dy, dz;
     if (MI) {
-        dx = gm_min_image(pi.x, pj.x, P.half[0]);
-        dy = gm_min_image(pi.y, pj.y, P.half[1]);
-        dz = gm_min_image(pi.z, pj.z, P.half[2]);
+        dx = gm_min_image_signed(pi.x, me.ax, me.hx, pj.x, P.half[0]);
+        dy = gm_min_image_signed(pi.y, me.ay, me.hy, pj.y, P.half[1]);
+        dz = gm_min_image_signed(pi.z, me.az, me.hz, pj.z, P.half[2]);
     } else {
         dx = pi.x - pj.x; dy = pi.y - pj.y; dz = pi.z - pj.z;
     }
@@ -86,14 +103,31 @@ __device__ __forceinline__ int quad_get(const int4 &e, int u)
     return u == 0 ? e.x : (u == 1 ? e.y : (u == 2 ? e.z : e.w));
 }
 
-// Gather loop over row i of NL (Alg. 2), NQ quads (4 NQ list entries) per batch.
+#define GM_PRE 4      // quads of a row loaded before NN is known (GmParams::minq = min(GM_PRE, capq))
+
+__device__ __forceinline__ const int4 *nl_row(const GmParams &P, const GmDev &D, int i)
+{
+    return D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31);
+}
+
+// The first quads of row i, issued together with the other streaming loads of the bead (always written
+// by the build, padded with the far-away bead, so they do not depend on NN).
+__device__ __forceinline__ void nl_preload(const GmParams &P, const int4 *__restrict__ t, uint64_t pol,
+                                           int4 (&pre)[GM_PRE])
+{
+    const int4 pad = make_int4(P.n, P.n, P.n, P.n);
+#pragma unroll
+    for (int u = 0; u < GM_PRE; ++u) pre[u] = (u < P.minq) ? gm_ld_stream(t + u * 32, pol) : pad;
+}
+
+// Gather loop over row i of NL (Alg. 2), NQ quads (4 NQ list entries) per batch:
+// first the preloaded quads, then a software-pipelined loop over the rest of the row.
 template <int PAIR, bool NT1, bool ENERGY, bool MI>
-__device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, const Src &S, int i, const int nn,
-                                          const float4 pi, const int ti, const float4 vti,
+__device__ __forceinline__ void pair_loop(const GmParams &P, const Src &S, const int4 *__restrict__ t,
+                                          uint64_t pol, const int4 (&pre)[GM_PRE], const int nn, const Own &me,
                                           unsigned long long step, BeadForce &o)
 {
-    constexpr int NQ = (PAIR == GM_PAIR_DPD) ? 1 : 2;
-    const int4 *__restrict__ t = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31);
+    constexpr int NQ = (PAIR == GM_PAIR_DPD) ? 1 : GM_LJ_NQ;
     const int nq = (nn + 3) >> 2;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
     const GmPair p0 = P.pair[0];
@@ -101,8 +135,24 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, con
     const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
     int4 en[NQ];
 #pragma unroll
-    for (int u = 0; u < NQ; ++u) en[u] = (u < nq) ? __ldg(t + u * 32) : pad;
-    for (int q = 0; q < nq; q += NQ) {
+    for (int u = 0; u < NQ; ++u) en[u] = (GM_PRE + u < nq) ? gm_ld_stream(t + (GM_PRE + u) * 32, pol) : pad;
+#pragma unroll
+    for (int b = 0; b < GM_PRE; b += NQ) {
+        if (b < nq) {
+            float4 pj[4 * NQ], vj[4 * NQ];
+#pragma unroll
+            for (int u = 0; u < 4 * NQ; ++u) pj[u] = __ldg(S.pos + quad_get(pre[b + (u >> 2)], u & 3));
+            if (PAIR == GM_PAIR_DPD) {
+#pragma unroll
+                for (int u = 0; u < 4 * NQ; ++u) vj[u] = __ldg(S.vt + quad_get(pre[b + (u >> 2)], u & 3));
+            }
+#pragma unroll
+            for (int u = 0; u < 4 * NQ; ++u)
+                pair_term<PAIR, NT1, ENERGY, MI>(P, me, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : zero4, p0,
+                                                 (uint32_t)step, fx, fy, fz, pe, cnt);
+        }
+    }
+    for (int q = GM_PRE; q < nq; q += NQ) {
         float4 pj[4 * NQ], vj[4 * NQ];
 #pragma unroll
         for (int u = 0; u < 4 * NQ; ++u) pj[u] = __ldg(S.pos + quad_get(en[u >> 2], u & 3));
@@ -111,10 +161,10 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const GmDev &D, con
             for (int u = 0; u < 4 * NQ; ++u) vj[u] = __ldg(S.vt + quad_get(en[u >> 2], u & 3));
         }
 #pragma unroll
-        for (int u = 0; u < NQ; ++u) en[u] = (q + NQ + u < nq) ? __ldg(t + (q + NQ + u) * 32) : pad;
+        for (int u = 0; u < NQ; ++u) en[u] = (q + NQ + u < nq) ? gm_ld_stream(t + (q + NQ + u) * 32, pol) : pad;
 #pragma unroll
         for (int u = 0; u < 4 * NQ; ++u)
-            pair_term<PAIR, NT1, ENERGY, MI>(P, pi, ti, vti, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : zero4, p0,
+            pair_term<PAIR, NT1, ENERGY, MI>(P, me, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : zero4, p0,
                                              (uint32_t)step, fx, fy, fz, pe, cnt);
     }
     o.fx += fx; o.fy += fy; o.fz += fz;
@@ -172,23 +222,29 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
 }
 
 // Force on bead i at time level `step`, conservative + (DPD) dissipative/random.  vti: own v~ and tag.
+// pre / nn: the preloaded head of row i and NN[i].
 template <int PAIR, bool NT1, int BOND, bool ENERGY>
 __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const Src &S, int i,
-                                                const float4 pi, const float4 vti, unsigned long long step)
+                                                const float4 pi, const float4 vti, const int4 *__restrict__ t,
+                                                uint64_t pol, const int4 (&pre)[GM_PRE], const int nn,
+                                                unsigned long long step)
 {
     BeadForce o;
     o.fx = o.fy = o.fz = o.pe_pair = o.pe_bond = o.cnt = 0.f;
-    const int ti = __float_as_int(pi.w);
-    const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
     bond_loop<BOND, ENERGY>(P, D, S, i, pi, o);
     if (PAIR != GM_PAIR_NONE) {
+        Own me;
+        me.p = pi; me.vt = vti; me.t = __float_as_int(pi.w);
+        me.hx = copysignf(P.half[0], pi.x); me.hy = copysignf(P.half[1], pi.y); me.hz = copysignf(P.half[2], pi.z);
+        me.ax = pi.x - me.hx; me.ay = pi.y - me.hy; me.az = pi.z - me.hz;
         // A bead further than r_list + skin from every face cannot have a listed partner across the
-        // boundary (both moved < skin/2 since the build): plain differences, no image test.
+        // boundary (both moved < skin/2 since the build): plain differences, no image test.  Decided per
+        // warp so that a warp runs one of the two loops, not both.
         const float m = P.edge_margin;
         const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
                               fabsf(pi.z) < P.half[2] - m;
-        if (interior) pair_loop<PAIR, NT1, ENERGY, false>(P, D, S, i, nn, pi, ti, vti, step, o);
-        else pair_loop<PAIR, NT1, ENERGY, true>(P, D, S, i, nn, pi, ti, vti, step, o);
+        if (__all_sync(__activemask(), interior)) pair_loop<PAIR, NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o);
+        else pair_loop<PAIR, NT1, ENERGY, true>(P, S, t, pol, pre, nn, me, step, o);
     }
     return o;
 }
@@ -213,7 +269,7 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, in
 
 // ---- the per-step kernel (MODE_STEP) and the force-materialising kernel (MODE_FORCES) ---------------
 template <int PAIR, bool NT1, int BOND, int MODE>
-__global__ void __launch_bounds__(FORCE_BLOCK)
+__global__ void __launch_bounds__(FORCE_BLOCK, GM_FORCE_MINB)
 k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -227,13 +283,19 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, flo
             D.ctl->need = step + 1;
     }
     if (i >= P.n) return;
+    // every stream of this bead is requested before anything is used
+    const uint64_t pol = gm_policy_evict_first();
+    const int4 *__restrict__ t = nl_row(P, D, i);
+    int4 pre[GM_PRE];
+    if (PAIR != GM_PAIR_NONE) nl_preload(P, t, pol, pre);
     const float4 pi = S.pos[i];
-    const float4 u = S.vel[i];
+    const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
+    const float4 u = gm_ld_nol1(S.vel + i);
     float4 rf = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (MODE == GM_MODE_STEP) rf = D.ref[i];
+    if (MODE == GM_MODE_STEP) rf = gm_ld_nol1(D.ref + i);
     float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
     if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES>(P, D, S, i, pi, vti, step);
+    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES>(P, D, S, i, pi, vti, t, pol, pre, nn, step);
     const float3 a = bead_accel(P, S, i, f, u, step);
     if (MODE == GM_MODE_FORCES) {
         D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
@@ -264,10 +326,15 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
     const Src S = current_src(D, parity, step);
     double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };   // ke, pe_pair, pe_bond, px, py, pz, pairs
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += gridDim.x * blockDim.x) {
+        const uint64_t pol = gm_policy_evict_first();
+        const int4 *__restrict__ t = nl_row(P, D, i);
+        int4 pre[GM_PRE];
+        if (PAIR != GM_PAIR_NONE) nl_preload(P, t, pol, pre);
         const float4 pi = S.pos[i];
+        const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
         float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
         if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-        const BeadForce f = bead_force<PAIR, NT1, BOND, true>(P, D, S, i, pi, vti, step);
+        const BeadForce f = bead_force<PAIR, NT1, BOND, true>(P, D, S, i, pi, vti, t, pol, pre, nn, step);
         const float4 u = S.vel[i];
         float vx = u.x, vy = u.y, vz = u.z;
         if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m

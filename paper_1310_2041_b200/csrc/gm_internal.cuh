@@ -59,6 +59,7 @@ struct GmParams {
     int n, n_types, max_bonds, nl_cap;
     int ns;                        // padded bead count: n + 1 rounded up to GM_PAD (slot n is the far-away pad bead)
     int capq;                      // nl_cap / 4: int4 quads per NL row
+    int minq;                      // quads of every row that are always written (padded): min(4, capq)
     int nc[3], n_cells;
     int sfc_period;                // a rebuild (= SFC sort) is forced after this many steps without one; <= 0: never
     float box[3], half[3], inv_w[3];
@@ -162,6 +163,41 @@ __device__ __forceinline__ float gm_min_image(float a, float b, float half)
     if (d > half) d = (a - half) - (b + half);
     else if (d < -half) d = (a + half) - (b - half);
     return d;
+}
+
+// Minimum image for a bead whose own coordinate a is known: with hs = copysign(L/2, a) a partner across
+// the boundary can only lie on the far side of that face (a >= 0: a - b > L/2 only), so one magnitude
+// test selects between the plain difference and the face-relative one (a - hs) - (b + hs).
+__device__ __forceinline__ float gm_min_image_signed(float a, float a_minus_hs, float hs, float b, float half)
+{
+    const float t = a - b;
+    const float d2 = a_minus_hs - (b + hs);
+    return fabsf(t) > half ? d2 : t;
+}
+
+// Streaming loads: not kept in L1, and (with an evict-first policy) first out of L2, so that the
+// arrays that are re-read every step (positions, velocities, reference positions) stay L2-resident.
+__device__ __forceinline__ uint64_t gm_policy_evict_first()
+{
+    uint64_t p;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+
+__device__ __forceinline__ int4 gm_ld_stream(const int4 *ptr, uint64_t pol)
+{
+    int4 v;
+    asm("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.s32 {%0, %1, %2, %3}, [%4], %5;"
+        : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(ptr), "l"(pol));
+    return v;
+}
+
+__device__ __forceinline__ float4 gm_ld_nol1(const float4 *ptr)
+{
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(ptr));
+    return v;
 }
 
 __device__ __forceinline__ float gm_wrap(float x, float half, float L)

@@ -33,10 +33,8 @@ __device__ __forceinline__ int nl_scan_run(const float4 *__restrict__ ref, int s
         if (SHIFT) { dx = ax - (q.x + hx); dy = ay - (q.y + hy); dz = az - (q.z + hz); }
         else { dx = ax - q.x; dy = ay - q.y; dz = az - q.z; }
         const float r2 = dx * dx + dy * dy + dz * dz;
-        if (r2 < r_list2 && s != i) {
-            if (k < cap) row[k * 32] = s;
-            ++k;
-        }
+        row[min(k, cap - 1) * 32] = s;           // branch-free append: the slot is kept only on a hit
+        k += (r2 < r_list2 && s != i) ? 1 : 0;
     }
     return k;
 }
@@ -103,8 +101,10 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
         }
     }
     const int kc = min(k, cap);
-    const int nq = (kc + 3) >> 2;
-    for (int kk = kc; kk < 4 * nq; ++kk) row[kk * 32] = P.n;      // pad the last quad with the far-away bead
+    // whole quads, at least minq of them (the force kernel loads those before it knows NN), padded with
+    // the far-away bead
+    const int nq = max((kc + 3) >> 2, P.minq);
+    for (int kk = kc; kk < 4 * nq; ++kk) row[kk * 32] = P.n;
     if (i < P.ns) D.nn[i] = kc;
     int4 *__restrict__ tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
     for (int q = 0; q < nq; ++q)

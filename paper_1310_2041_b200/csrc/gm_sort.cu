@@ -23,9 +23,8 @@
 
 // Decide whether the rebuild runs at this time level and publish the decision (every later kernel of
 // the chain only reads ctl->go).  With a conditional graph node the body is skipped altogether.
-__global__ void k_gate(GmDev D, int gate, int parity, cudaGraphConditionalHandle h, int use_handle)
+__device__ __forceinline__ int gate_decide(GmCtl *c, int gate, int parity)
 {
-    GmCtl *c = D.ctl;
     const int go = gm_rebuild_off(c, gate, parity) ? 0 : 1;
     c->go = go;
     if (go) {
@@ -34,13 +33,21 @@ __global__ void k_gate(GmDev D, int gate, int parity, cudaGraphConditionalHandle
         c->max_nn = 0;
         c->sum_nn = 0;
     }
-    if (use_handle) cudaGraphSetConditional(h, (unsigned)go);
+    return go;
+}
+
+__global__ void k_gate(GmDev D, int gate, int parity) { gate_decide(D.ctl, gate, parity); }
+
+__global__ void k_gate_cond(GmDev D, int gate, int parity, cudaGraphConditionalHandle h)
+{
+    cudaGraphSetConditional(h, (unsigned)gate_decide(D.ctl, gate, parity));
 }
 
 void gm_launch_gate(const GmDev &D, int gate, int parity, unsigned long long cond_handle, int use_handle,
                     cudaStream_t st)
 {
-    k_gate<<<1, 1, 0, st>>>(D, gate, parity, (cudaGraphConditionalHandle)cond_handle, use_handle);
+    if (use_handle) k_gate_cond<<<1, 1, 0, st>>>(D, gate, parity, (cudaGraphConditionalHandle)cond_handle);
+    else k_gate<<<1, 1, 0, st>>>(D, gate, parity);
 }
 
 __global__ void __launch_bounds__(SORT_BLOCK)
