@@ -24,8 +24,11 @@
 #include "gm_internal.cuh"
 
 #define FORCE_BLOCK 128
-#ifndef GM_FORCE_MINB
-#define GM_FORCE_MINB 1          // minimum resident blocks per SM the step kernel is compiled for
+#ifndef STEP_BLOCK
+#define STEP_BLOCK 128           // beads per CTA of the step kernel
+#endif
+#ifndef STEP_MINB
+#define STEP_MINB 7              // minimum resident CTAs per SM the step kernel is compiled for (72 registers)
 #endif
 #ifndef GM_LJ_NQ
 #define GM_LJ_NQ 2               // quads (of 4 list entries) per batch of the LJ gather loop
@@ -267,22 +270,12 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, in
     return a;
 }
 
-// ---- the per-step kernel (MODE_STEP) and the force-materialising kernel (MODE_FORCES) ---------------
+// ---- the per-step work of one bead (MODE_STEP) / its materialised force (MODE_FORCES) -----------------
 template <int PAIR, bool NT1, int BOND, int MODE>
-__global__ void __launch_bounds__(FORCE_BLOCK, GM_FORCE_MINB)
-k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
+__device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, const Src &S, const int i,
+                                          const unsigned long long step, const int parity, const float kick,
+                                          const float kick_vt)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const unsigned long long step = D.ctl->step[parity];
-    const Src S = current_src(D, parity, step);
-    if (MODE == GM_MODE_STEP && blockIdx.x == 0 && threadIdx.x == 0) {
-        D.ctl->step[parity ^ 1] = step + 1;
-        // a2: at most sfc_period steps between two sorts
-        if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
-            step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
-            D.ctl->need = step + 1;
-    }
-    if (i >= P.n) return;
     // every stream of this bead is requested before anything is used
     const uint64_t pol = gm_policy_evict_first();
     const int4 *__restrict__ t = nl_row(P, D, i);
@@ -315,6 +308,38 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, flo
     const float dy = gm_min_image(y, rf.y, P.half[1]);
     const float dz = gm_min_image(z, rf.z, P.half[2]);
     if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) D.ctl->need = step + 1;
+}
+
+// gm_compute_forces: one block per 128 beads.
+template <int PAIR, bool NT1, int BOND>
+__global__ void __launch_bounds__(FORCE_BLOCK)
+k_force(const __grid_constant__ GmParams P, GmDev D, int parity)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned long long step = D.ctl->step[parity];
+    const Src S = current_src(D, parity, step);
+    if (i >= P.n) return;
+    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES>(P, D, S, i, step, parity, 0.f, 0.f);
+}
+
+// The step kernel (a4..a8).  A CTA owns STEP_BLOCK consecutive beads: storage order is cell order along
+// the curve, so its warps work side by side on a few adjacent (y, z) rows of cells and share the neighbor
+// positions they gather through the SM's L1.
+template <int PAIR, bool NT1, int BOND>
+__global__ void __launch_bounds__(STEP_BLOCK, STEP_MINB)
+k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
+{
+    const unsigned long long step = D.ctl->step[parity];
+    const Src S = current_src(D, parity, step);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        D.ctl->step[parity ^ 1] = step + 1;
+        // a2: at most sfc_period steps between two sorts
+        if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
+            step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
+            D.ctl->need = step + 1;
+    }
+    const int i = blockIdx.x * STEP_BLOCK + threadIdx.x;
+    if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP>(P, D, S, i, step, parity, kick, kick_vt);
 }
 
 // ---- a9 energies: grid-stride, fp64 accumulation, per-block partials in fixed order ----------------
@@ -378,10 +403,10 @@ static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int pari
                            int lagged, cudaStream_t st)
 {
     int nb = (P.n + FORCE_BLOCK - 1) / FORCE_BLOCK;
-    if (mode == GM_MODE_STEP)
-        k_force<PAIR, NT1, BOND, GM_MODE_STEP><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
-    else if (mode == GM_MODE_FORCES)
-        k_force<PAIR, NT1, BOND, GM_MODE_FORCES><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+    if (mode == GM_MODE_STEP) {
+        k_step<PAIR, NT1, BOND><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+    } else if (mode == GM_MODE_FORCES)
+        k_force<PAIR, NT1, BOND><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity);
     else {
         int g = nb < GM_ESUM_BLOCKS ? nb : GM_ESUM_BLOCKS;
         k_energy<PAIR, NT1, BOND><<<g, FORCE_BLOCK, 0, st>>>(P, D, parity, lagged);
