@@ -9,34 +9,65 @@
 // along x inside a row, so the three x-adjacent cells of one (y, z) row are one contiguous run of
 // ref[]: nine runs per bead instead of 27 cells (two more where the row wraps around the box).
 //
-// The warp collects its 32 rows in shared memory (row k of lane l at [k][l]: conflict-free, and private
-// to the lane, so no synchronisation) and writes them out as whole int4 quads of its own NL tile
-// (gm_internal.cuh: entries 4q..4q+3 of a bead are one int4, the 32 int4 of a quad are contiguous):
-// coalesced 512-byte stores, and coalesced 512-byte loads in the force kernel.
+// Hits are staged in a small lane-private shared-memory ring (NL_STAGE entries per lane, column l of
+// [NL_STAGE][32]: conflict-free and private to the lane, so no synchronisation); candidates are scanned in
+// chunks of NL_CHUNK, and after a chunk every lane that holds 16 or more staged entries writes four whole
+// int4 quads of its NL row (gm_internal.cuh: entries 4q..4q+3 of a bead are one int4; the 32 int4 of a
+// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 16 KB per CTA
+// whatever the row capacity, which leaves the rest of the SM's 228 KB to L1 for the candidate loads.
 #include "gm_internal.cuh"
 
-extern __shared__ int nl_rows[];     // [warps per block][nl_cap][32]
+#define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + NL_CHUNK)
+#define NL_CHUNK 16          // candidates scanned between two flush checks
+#define NL_WARPS 4
+
+struct NlRow {
+    int *ring;               // this lane's column of the ring: ring[(k & (NL_STAGE-1)) * 32]
+    int4 *tile;              // this lane's int4 column of its NL tile: tile[q * 32]
+    int k;                   // hits so far
+    int flushed;             // entries already written to the tile (multiple of 16)
+    int cap;
+};
+
+// write entries [flushed, flushed + 16) of the row (whole quads) from the ring to the tile
+__device__ __forceinline__ void nl_flush16(NlRow &r)
+{
+    if (r.flushed + 16 <= r.cap) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int e = r.flushed + 4 * q;
+            r.tile[(e >> 2) * 32] = make_int4(r.ring[((e + 0) & (NL_STAGE - 1)) * 32], r.ring[((e + 1) & (NL_STAGE - 1)) * 32],
+                                              r.ring[((e + 2) & (NL_STAGE - 1)) * 32], r.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+        }
+    }
+    r.flushed += 16;
+}
 
 // One run of candidates ref[s0 .. s1) against bead i.  SHIFT: the run lies across a periodic face in
 // some dimension; the displacement is then taken relative to the two faces, (a -+ L/2) - (b +- L/2)
 // (see gm_min_image), with the bead side (ax, ay, az) prepared once per run and the candidate side
-// b + (hx, hy, hz) per candidate -- no branches in the loop.
+// b + (hx, hy, hz) per candidate -- no branches in the chunk loop.
 template <bool SHIFT>
-__device__ __forceinline__ int nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
-                                           float ay, float az, float hx, float hy, float hz, float r_list2,
-                                           int k, int cap, int *__restrict__ row)
+__device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
+                                            float ay, float az, float hx, float hy, float hz, float r_list2,
+                                            NlRow &r)
 {
+    for (int c0 = s0; c0 < s1; c0 += NL_CHUNK) {
+        const int c1 = min(c0 + NL_CHUNK, s1);
+        int k = r.k;
 #pragma unroll 4
-    for (int s = s0; s < s1; ++s) {
-        const float4 q = __ldg(ref + s);
-        float dx, dy, dz;
-        if (SHIFT) { dx = ax - (q.x + hx); dy = ay - (q.y + hy); dz = az - (q.z + hz); }
-        else { dx = ax - q.x; dy = ay - q.y; dz = az - q.z; }
-        const float r2 = dx * dx + dy * dy + dz * dz;
-        row[min(k, cap - 1) * 32] = s;           // branch-free append: the slot is kept only on a hit
-        k += (r2 < r_list2 && s != i) ? 1 : 0;
+        for (int s = c0; s < c1; ++s) {
+            const float4 q = __ldg(ref + s);
+            float dx, dy, dz;
+            if (SHIFT) { dx = ax - (q.x + hx); dy = ay - (q.y + hy); dz = az - (q.z + hz); }
+            else { dx = ax - q.x; dy = ay - q.y; dz = az - q.z; }
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            r.ring[(k & (NL_STAGE - 1)) * 32] = s;      // branch-free append: the slot is kept only on a hit
+            k += (r2 < r_list2 && s != i) ? 1 : 0;
+        }
+        r.k = k;
+        if (k - r.flushed >= 16) nl_flush16(r);
     }
-    return k;
 }
 
 __global__ void __launch_bounds__(128)
@@ -45,9 +76,12 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     if (!D.ctl->go) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    __shared__ int nl_ring[NL_WARPS][NL_STAGE][32];
+    NlRow row;
+    row.ring = &nl_ring[wid][0][lane];
+    row.tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
+    row.k = 0; row.flushed = 0; row.cap = P.nl_cap;
     const int cap = P.nl_cap;
-    int *__restrict__ row = nl_rows + (size_t)wid * cap * 32 + lane;
-    int k = 0;
     if (i < P.n) {
         const float4 *__restrict__ ref = D.ref;
         const int *__restrict__ cstart = D.cstart;
@@ -68,8 +102,8 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
             for (int oz = -1; oz <= 1; ++oz)
                 for (int oy = -1; oy <= 1; ++oy) {
                     const int r0 = (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
-                    k = nl_scan_run<false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
-                                           pi.y, pi.z, 0.f, 0.f, 0.f, rl2, k, cap, row);
+                    nl_scan_run<false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, pi.y,
+                                       pi.z, 0.f, 0.f, 0.f, rl2, row);
                 }
         } else {
             for (int oz = -1; oz <= 1; ++oz) {
@@ -83,15 +117,15 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
                     if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
                     else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
                     const int r0 = (int)__ldg(rr + z * ncy + y) * ncx;
-                    k = nl_scan_run<true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay,
-                                          az, 0.f, hy, hz, rl2, k, cap, row);
+                    nl_scan_run<true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
+                                      0.f, hy, hz, rl2, row);
                     if (xb >= 0)
-                        k = nl_scan_run<true>(ref, __ldg(cstart + r0 + xb), __ldg(cstart + r0 + xb + 1), i,
-                                              pi.x - hxb, ay, az, hxb, hy, hz, rl2, k, cap, row);
+                        nl_scan_run<true>(ref, __ldg(cstart + r0 + xb), __ldg(cstart + r0 + xb + 1), i, pi.x - hxb,
+                                          ay, az, hxb, hy, hz, rl2, row);
                 }
             }
         }
-        if (k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
+        if (row.k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
         // a7 set-up: BL of this slot in index space from its tag-space row (the sort moved the beads)
         const int sel = (int)(D.ctl->n_rebuilds & 1ull);
         const size_t ns = (size_t)P.ns;
@@ -100,16 +134,17 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
             D.bl[b * ns + i] = e < 0 ? -1 : (D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK));
         }
     }
-    const int kc = min(k, cap);
-    // whole quads, at least minq of them (the force kernel loads those before it knows NN), padded with
-    // the far-away bead
+    // the tail of the row: whole quads, at least minq of them in all (the force kernel loads those before
+    // it knows NN), padded with the far-away bead
+    const int kc = min(row.k, cap);
     const int nq = max((kc + 3) >> 2, P.minq);
-    for (int kk = kc; kk < 4 * nq; ++kk) row[kk * 32] = P.n;
+    for (int e = max(kc, row.flushed); e < 4 * nq; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = P.n;
+    for (int q = row.flushed >> 2; q < nq; ++q) {
+        const int e = 4 * q;
+        row.tile[q * 32] = make_int4(row.ring[((e + 0) & (NL_STAGE - 1)) * 32], row.ring[((e + 1) & (NL_STAGE - 1)) * 32],
+                                     row.ring[((e + 2) & (NL_STAGE - 1)) * 32], row.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+    }
     if (i < P.ns) D.nn[i] = kc;
-    int4 *__restrict__ tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
-    for (int q = 0; q < nq; ++q)
-        tile[q * 32] = make_int4(row[(4 * q) * 32], row[(4 * q + 1) * 32], row[(4 * q + 2) * 32],
-                                 row[(4 * q + 3) * 32]);
     const int m = __reduce_max_sync(0xffffffffu, kc);
     const unsigned int sum = __reduce_add_sync(0xffffffffu, (unsigned int)kc);
     if (lane == 0) {
@@ -121,30 +156,14 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     }
 }
 
-static int nl_warps_per_block(const GmParams &P)
-{
-    const size_t per_warp = (size_t)P.nl_cap * 32 * sizeof(int);
-    int w = (int)((200u * 1024u) / per_warp);
-    return w > 4 ? 4 : w;
-}
+int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 4 == 0; }
 
-int gm_nl_capacity_ok(const GmParams &P) { return nl_warps_per_block(P) >= 1; }
-
-// Once per system (not during graph capture): opt in to more than 48 KB of dynamic shared memory.
-cudaError_t gm_nl_prepare(const GmParams &P)
-{
-    const size_t smem = (size_t)nl_warps_per_block(P) * P.nl_cap * 32 * sizeof(int);
-    if (smem > 48 * 1024)
-        return cudaFuncSetAttribute(k_nl_build, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-    return cudaSuccess;
-}
+cudaError_t gm_nl_prepare(const GmParams &P) { (void)P; return cudaSuccess; }
 
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
-    const int w = nl_warps_per_block(P);
-    const size_t smem = (size_t)w * P.nl_cap * 32 * sizeof(int);
-    const int threads = w * 32;
-    k_nl_build<<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
+    const int threads = NL_WARPS * 32;
+    k_nl_build<<<(P.ns + threads - 1) / threads, threads, 0, st>>>(P, D);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors): nn_out[tag], nl_out[tag*stride + k].
