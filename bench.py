@@ -257,7 +257,7 @@ def main():
     bytes_step = bytes_kernel + w.n * (80 + 4 * nbar_l) / m_interval
     achieved = bytes_kernel / (k_ms * 1e-3) / 1e9
     ms_ts = ms / n_ts
-    roof = {"bound": "hbm", "kernel": "k_force<STEP> (fused a4+a5+a7+a8)", "achieved": achieved, "peak": hbm_gbs,
+    roof = {"bound": "hbm", "kernel": "k_step (fused a4+a5+a7+a8)", "achieved": achieved, "peak": hbm_gbs,
             "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None, "peak_source": peak_src,
             "kernel_ms": k_ms, "algorithmic_bytes_per_launch": bytes_kernel,
             "kernel_share_of_step": k_ms / ms_ts,

@@ -1,0 +1,138 @@
+"""Full-size and long-run GPU-vs-oracle parity (run with -m gpu on a B200).
+
+  * BASELINE.json configs[2] ("C3", the 1,000,000-bead Kremer-Grest melt bench.py times), in the launch
+    configuration bench.py uses (CUDA graphs with the rebuild inside a conditional node): neighbor sets,
+    per-bead forces and the 10-step trajectory against the fp64 cell-list oracle on ALL beads (the
+    oracle's O(N) mode finishes a step of C3 in about 0.1 s; its agreement with the O(N^2) definition is
+    pinned in tests/test_oracle_pins.py).
+  * Long runs (north_star: "energy drift and <Rg^2>/bond-length statistics must agree within a stated
+    1 %"): C1 for its full 1,000 NVE steps, a scaled C2 under the Langevin
+    thermostat, a scaled C4 under DPD.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def gm():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1310_2041_b200 import gm as g
+    g.lib()
+    return g
+
+
+@pytest.fixture(scope="module")
+def c3():
+    return make_config("C3")
+
+
+def test_c3_full_neighbor_sets(gm, c3):
+    w = c3
+    s = gm.System(w)
+    s.build_neighbors()
+    nn, nl = s.neighbors()
+    st = s.stats()
+    assert st["max_nn"] == nn.max() and st["sum_nn"] == nn.sum() and st["dev_err"] == 0
+    n = w.n
+    rl = float(np.float32(np.max(w.pair["rc"]))) + float(np.float32(w.r_skin))
+    inner = orc.neighbor_pairs(w.pos, w.box, rl - 1e-6, True)
+    outer = orc.neighbor_pairs(w.pos, w.box, rl + 1e-6, True)
+    mask = np.arange(nl.shape[1])[None, :] < nn[:, None]
+    rows = np.broadcast_to(np.arange(n)[:, None], nl.shape)[mask].astype(np.int64)
+    cols = nl[mask].astype(np.int64)
+    assert (rows != cols).all()
+    key = rows * n + cols
+    assert len(np.unique(key)) == len(key)                       # no duplicates
+    assert np.array_equal(np.sort(key), np.sort(cols * n + rows))  # FULL list: (i,j) and (j,i)
+    half = key[rows < cols]
+    k_in = inner[:, 0].astype(np.int64) * n + inner[:, 1]
+    k_out = outer[:, 0].astype(np.int64) * n + outer[:, 1]
+    assert np.isin(k_in, half).all(), "GPU list misses a pair inside r_list - 1e-6"
+    assert np.isin(half, k_out).all(), "GPU list holds a pair outside r_list + 1e-6"
+    s.close()
+
+
+def test_c3_full_forces_and_10_step_trajectory(gm, c3):
+    w = c3
+    s = gm.System(w)                      # default flags: graphs + conditional rebuild node, as in bench.py
+    o = orc.Oracle(w, use_cells=True)
+    s.compute_forces()
+    F = s.get_particles(False, False, True)[2]
+    Fo = o.compute_forces().copy()
+    frms = np.sqrt((Fo ** 2).sum(axis=1).mean())
+    err = np.abs(F - Fo).max()
+    assert err <= 1e-4 * frms, f"max|dF| = {err:.3e} > 1e-4 F_rms = {1e-4 * frms:.3e}"
+    e = s.energies()
+    assert e["n_pairs"] == o.last[2]
+    assert e["pe_pair"] == pytest.approx(o.last[0], rel=1e-5)
+    assert e["pe_bond"] == pytest.approx(o.last[1], rel=1e-5)
+    s.step(10)
+    o.run(10)
+    pos = s.get_particles(True, False, False)[0]
+    d = pos.astype(np.float64) - o.pos
+    d -= o.box * np.rint(d / o.box)
+    rms = np.sqrt((d ** 2).sum(axis=1).mean())
+    assert rms <= 1e-4, f"RMS position difference after 10 steps = {rms:.3e} sigma"
+    assert s.stats()["dev_err"] == 0
+    s.close()
+
+
+def _observables(pos, w):
+    b = orc.bond_lengths(pos, w.box, w.bonds)
+    rg2 = orc.chain_rg2(pos, w.box, w.chain_len)
+    return b.mean(), b.var(), rg2.mean()
+
+
+def _long_run(gm, w, n_steps, every):
+    s = gm.System(w)
+    o = orc.Oracle(w, use_cells=True)
+    o.compute_forces()
+    rows_g, rows_o = [], []
+    for _ in range(n_steps // every):
+        s.step(every)
+        o.run(every)
+        e = s.energies()
+        pos = s.get_particles(True, False, False)[0]
+        rows_g.append((e["etot"] / w.n, e["ke"] / w.n, e["T"]) + _observables(pos, w))
+        pe_pair, pe_bond, _ = o.potential()
+        ke = o.kinetic()
+        rows_o.append(((ke + pe_pair + pe_bond) / w.n, ke / w.n, o.temperature()) + _observables(o.pos, w))
+    assert s.stats()["dev_err"] == 0
+    s.close()
+    return np.array(rows_g), np.array(rows_o)
+
+
+def test_c1_full_1000_steps_nve_statistics(gm):
+    w = make_config("C1")
+    g, o = _long_run(gm, w, 1000, 100)
+    # (i) run-averaged mean bond length and <Rg^2> within 1 %
+    assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)
+    # (ii) NVE: total energy per bead stays within 1 % of the mean kinetic energy per bead, in both runs
+    for r in (g, o):
+        assert np.abs(r[:, 0] - r[0, 0]).max() <= 0.01 * r[:, 1].mean()
+    # the two runs hold the same energy per bead to the same level
+    assert np.abs(g[:, 0] - o[:, 0]).max() <= 0.01 * o[:, 1].mean()
+
+
+def test_c2_scaled_langevin_temperature_statistics(gm):
+    w = make_config("C2", scale=0.4)          # 16^3 lattice, 4096 beads, LJ 2.5 + Langevin (same noise keys)
+    g, o = _long_run(gm, w, 600, 100)
+    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)     # (iii) run-averaged T within 1 %
+    assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)
+
+
+def test_c4_scaled_dpd_temperature_statistics(gm):
+    w = make_config("C4", scale=0.1)          # 10^3 box, 3000 beads, DPD + GW-VV (same pair-noise keys)
+    g, o = _long_run(gm, w, 300, 50)
+    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)
+    assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)
