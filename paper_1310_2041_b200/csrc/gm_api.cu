@@ -93,7 +93,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     int cap = c->nl_row_capacity;
     if (cap <= 0) {
         double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
-        cap = (int)(1.5 * nbar) + 32;
+        cap = (int)(2.0 * nbar) + 48;     // random-walk DPD starts (C4) reach ~3x the mean in places
     }
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
     cap = (cap + 7) / 8 * 8;
