@@ -299,14 +299,12 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
         D.vt[parity ^ 1][i] = make_float4(u.x + kick_vt * a.x, u.y + kick_vt * a.y, u.z + kick_vt * a.z, vti.w);
     const float ux = u.x + kick * a.x, uy = u.y + kick * a.y, uz = u.z + kick * a.z;
     D.vel[i] = make_float4(ux, uy, uz, u.w);
-    const float x = gm_wrap(pi.x + P.dt * ux, P.half[0], P.box[0]);
-    const float y = gm_wrap(pi.y + P.dt * uy, P.half[1], P.box[1]);
-    const float z = gm_wrap(pi.z + P.dt * uz, P.half[2], P.box[2]);
+    // positions are NOT wrapped here: between two rebuilds a bead may sit up to skin/2 outside the box (the
+    // sort wraps it back), so that every listed pair keeps the periodic image it had at the build
+    const float x = pi.x + P.dt * ux, y = pi.y + P.dt * uy, z = pi.z + P.dt * uz;
     D.pos[parity ^ 1][i] = make_float4(x, y, z, pi.w);
-    // a4: displacement since the last NL build
-    const float dx = gm_min_image(x, rf.x, P.half[0]);
-    const float dy = gm_min_image(y, rf.y, P.half[1]);
-    const float dz = gm_min_image(z, rf.z, P.half[2]);
+    // a4: displacement since the last NL build (ref holds the wrapped position the bead had then)
+    const float dx = x - rf.x, dy = y - rf.y, dz = z - rf.z;
     if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) D.ctl->need = step + 1;
 }
 

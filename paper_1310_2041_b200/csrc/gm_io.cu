@@ -37,8 +37,10 @@ k_unpack(const __grid_constant__ GmParams P, GmDev D, int cur, float *__restrict
     const Src S = current_src(D, cur, D.ctl->step[cur]);
     int t = S.tag[i];
     if (pos3) {
-        float4 p = S.pos[i];
-        pos3[3 * t + 0] = p.x; pos3[3 * t + 1] = p.y; pos3[3 * t + 2] = p.z;
+        float4 p = S.pos[i];     // may sit up to skin/2 outside the box between rebuilds: wrapped on the way out
+        pos3[3 * t + 0] = gm_wrap(p.x, P.half[0], P.box[0]);
+        pos3[3 * t + 1] = gm_wrap(p.y, P.half[1], P.box[1]);
+        pos3[3 * t + 2] = gm_wrap(p.z, P.half[2], P.box[2]);
     }
     float4 f = make_float4(0.f, 0.f, 0.f, 0.f);
     if (force3 || (vel3 && lagged)) f = D.frc[i];

@@ -56,9 +56,12 @@ k_keys(const __grid_constant__ GmParams P, GmDev D, int parity)
     if (!D.ctl->go) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
-    const float4 p = D.pos[parity][i];
+    float4 p = D.pos[parity][i];
     int key = 0;
     if (isfinite(p.x) && isfinite(p.y) && isfinite(p.z)) {
+        // the step kernel leaves positions unwrapped between rebuilds (at most skin/2 outside the box)
+        p.x = gm_wrap(p.x, P.half[0], P.box[0]); p.y = gm_wrap(p.y, P.half[1], P.box[1]);
+        p.z = gm_wrap(p.z, P.half[2], P.box[2]);
         const int cx = gm_cell_coord(p.x, P.half[0], P.inv_w[0], P.nc[0]);
         const int cy = gm_cell_coord(p.y, P.half[1], P.inv_w[1], P.nc[1]);
         const int cz = gm_cell_coord(p.z, P.half[2], P.inv_w[2], P.nc[2]);
@@ -178,7 +181,9 @@ k_permute(const __grid_constant__ GmParams P, GmDev D, int parity)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= P.n) return;
     const int sel = (int)(D.ctl->n_rebuilds & 1ull);       // buffers this rebuild writes
-    const float4 p = D.pos[parity][i];
+    float4 p = D.pos[parity][i];
+    p.x = gm_wrap(p.x, P.half[0], P.box[0]); p.y = gm_wrap(p.y, P.half[1], P.box[1]);
+    p.z = gm_wrap(p.z, P.half[2], P.box[2]);
     const float4 u = D.vel[i];
     const int t = D.tag[sel ^ 1][i];
     const int c = D.key[i];
