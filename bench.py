@@ -163,6 +163,9 @@ def main():
     ap.add_argument("--no-cond-nodes", action="store_true",
                     help="gate the rebuild with early-exit kernels instead of a conditional graph node "
                          "(ncu cannot profile kernel nodes of graphs that hold conditional nodes)")
+    ap.add_argument("--skin", type=float, default=None,
+                    help="override the config's neighbor skin (a tuning knob that never changes results; "
+                         "BASELINE.json gives none for C4)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -171,6 +174,8 @@ def main():
 
     from workloads import make_config
     w = make_config(args.config, scale=args.scale)
+    if args.skin is not None:
+        w.r_skin = float(args.skin)
     if args.impl == "reference":
         run_reference(args, w)
         return
