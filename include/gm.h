@@ -90,7 +90,10 @@ typedef struct {
 
 enum {
     GM_FLAG_NO_GRAPH = 1,            /* launch every kernel directly (debugging)                   */
-    GM_FLAG_NO_COND_NODES = 2        /* gate the rebuild with early-exit kernels instead of a CUDA conditional graph node */
+    GM_FLAG_NO_COND_NODES = 2,       /* gate the rebuild with early-exit kernels instead of a CUDA conditional graph node */
+    GM_FLAG_STEP_SUBWARP = 4         /* step kernel variant for long neighbor lists: 8 lanes share a bead, partial
+                                        forces summed by warp shuffles (same results up to fp32 summation order;
+                                        measured slower than one thread per bead on B200 -- kept for comparison) */
 };
 
 /* Bytes of device workspace gm_create needs for this configuration (all of the library's device

@@ -98,6 +98,9 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
     cap = (cap + 7) / 8 * 8;
     P->nl_cap = cap;
+    // lanes per bead of the step kernel: 8 lanes sharing a bead (shuffle reduction) measured SLOWER than one
+    // thread per bead on every config, so it is opt-in
+    P->step_subw = (c->flags & GM_FLAG_STEP_SUBWARP) ? 8 : 1;
     P->capq = cap / 4;
     P->minq = std::min(4, P->capq);
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;

@@ -340,6 +340,85 @@ k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, floa
     if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP>(P, D, S, i, step, parity, kick, kick_vt);
 }
 
+// The step kernel for LONG neighbor lists (n_l of 80-100: LJ with r_c = 2.5, configs C2/C5): SUBW lanes share
+// one bead.  Lane `sub` of the group walks quads sub, sub + SUBW, ... of the bead's NL row (two quads, eight
+// gathers, in flight per iteration), the partial forces are summed with xor-shuffles inside the group, and
+// lane 0 of the group adds the bonds and integrates.  With one thread per bead a 64,000-bead system is
+// 2,000 warps -- half a wave on 148 SMs, each thread walking ~90 dependent gathers; with 8 lanes per bead it is
+// 16,000 warps of ~11 gathers per lane.  Still no atomics: a bead's force is owned by one group.
+template <int PAIR, bool NT1, int BOND, int SUBW>
+__global__ void __launch_bounds__(STEP_BLOCK)
+k_step_sub(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
+{
+    const unsigned long long step = D.ctl->step[parity];
+    const Src S = current_src(D, parity, step);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        D.ctl->step[parity ^ 1] = step + 1;
+        if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
+            step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
+            D.ctl->need = step + 1;
+    }
+    const long long gt = (long long)blockIdx.x * STEP_BLOCK + threadIdx.x;
+    const int i = (int)(gt / SUBW), sub = (int)(gt % SUBW);
+    const bool valid = i < P.n;
+    const int ic = valid ? i : 0;                       // idle groups shadow bead 0 and write nothing
+    const uint64_t pol = gm_policy_evict_first();
+    const int4 *__restrict__ t = nl_row(P, D, ic);
+    const float4 pi = S.pos[ic];
+    const int nq = valid ? (D.nn[ic] + 3) >> 2 : 0;
+    float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (PAIR == GM_PAIR_DPD) vti = S.vt[ic];
+    Own me;
+    me.p = pi; me.vt = vti; me.t = __float_as_int(pi.w);
+    me.hx = copysignf(P.half[0], pi.x); me.hy = copysignf(P.half[1], pi.y); me.hz = copysignf(P.half[2], pi.z);
+    me.ax = pi.x - me.hx; me.ay = pi.y - me.hy; me.az = pi.z - me.hz;
+    const GmPair p0 = P.pair[0];
+    const int4 pad = make_int4(P.n, P.n, P.n, P.n);
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
+    if (PAIR != GM_PAIR_NONE) {
+        int4 ea = (sub < nq) ? gm_ld_stream(t + sub * 32, pol) : pad;
+        int4 eb = (sub + SUBW < nq) ? gm_ld_stream(t + (sub + SUBW) * 32, pol) : pad;
+        for (int q = sub; q < nq; q += 2 * SUBW) {
+            float4 pj[8], vj[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) pj[u] = __ldg(S.pos + quad_get(u < 4 ? ea : eb, u & 3));
+            if (PAIR == GM_PAIR_DPD) {
+#pragma unroll
+                for (int u = 0; u < 8; ++u) vj[u] = __ldg(S.vt + quad_get(u < 4 ? ea : eb, u & 3));
+            }
+            ea = (q + 2 * SUBW < nq) ? gm_ld_stream(t + (q + 2 * SUBW) * 32, pol) : pad;
+            eb = (q + 3 * SUBW < nq) ? gm_ld_stream(t + (q + 3 * SUBW) * 32, pol) : pad;
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                pair_term<PAIR, NT1, false, true>(P, me, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : zero4, p0,
+                                                  (uint32_t)step, fx, fy, fz, pe, cnt);
+        }
+    }
+#pragma unroll
+    for (int o = SUBW >> 1; o > 0; o >>= 1) {
+        fx += __shfl_xor_sync(0xffffffffu, fx, o);
+        fy += __shfl_xor_sync(0xffffffffu, fy, o);
+        fz += __shfl_xor_sync(0xffffffffu, fz, o);
+    }
+    if (!valid || sub != 0) return;
+    BeadForce f;
+    f.fx = 0.f; f.fy = 0.f; f.fz = 0.f; f.pe_pair = 0.f; f.pe_bond = 0.f; f.cnt = 0.f;
+    bond_loop<BOND, false>(P, D, S, i, pi, f);
+    f.fx += fx; f.fy += fy; f.fz += fz;
+    const float4 u = gm_ld_nol1(S.vel + i);
+    const float4 rf = gm_ld_nol1(D.ref + i);
+    const float3 a = bead_accel(P, S, i, f, u, step);
+    if (PAIR == GM_PAIR_DPD)
+        D.vt[parity ^ 1][i] = make_float4(u.x + kick_vt * a.x, u.y + kick_vt * a.y, u.z + kick_vt * a.z, vti.w);
+    const float ux = u.x + kick * a.x, uy = u.y + kick * a.y, uz = u.z + kick * a.z;
+    D.vel[i] = make_float4(ux, uy, uz, u.w);
+    const float x = pi.x + P.dt * ux, y = pi.y + P.dt * uy, z = pi.z + P.dt * uz;
+    D.pos[parity ^ 1][i] = make_float4(x, y, z, pi.w);
+    const float dx = x - rf.x, dy = y - rf.y, dz = z - rf.z;
+    if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) D.ctl->need = step + 1;
+}
+
 // ---- a9 energies: grid-stride, fp64 accumulation, per-block partials in fixed order ----------------
 template <int PAIR, bool NT1, int BOND>
 __global__ void __launch_bounds__(FORCE_BLOCK)
@@ -402,7 +481,12 @@ static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int pari
 {
     int nb = (P.n + FORCE_BLOCK - 1) / FORCE_BLOCK;
     if (mode == GM_MODE_STEP) {
-        k_step<PAIR, NT1, BOND><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+        if (P.step_subw == 8 && PAIR != GM_PAIR_NONE) {
+            const long long nt = (long long)P.n * 8;
+            k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + STEP_BLOCK - 1) / STEP_BLOCK), STEP_BLOCK, 0, st>>>(
+                P, D, parity, kick, kick_vt);
+        } else
+            k_step<PAIR, NT1, BOND><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
     } else if (mode == GM_MODE_FORCES)
         k_force<PAIR, NT1, BOND><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity);
     else {

@@ -22,7 +22,7 @@ GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_
 GM_PAIR = {"none": 0, "lj": 1, "dpd": 2}
 GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
 GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
-GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES = 1, 2
+GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP = 1, 2, 4
 
 SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_bond_params",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",

@@ -192,6 +192,13 @@ def test_trajectory_c1_40_steps_spans_rebuilds(gm):
     s.close()
 
 
+def test_subwarp_step_variant_matches_oracle(gm):
+    """GM_FLAG_STEP_SUBWARP: 8 lanes per bead with a shuffle reduction (long-list variant)."""
+    trajectory_parity(gm, make_config("C2", scale=0.5), flags=gm.GM_FLAG_STEP_SUBWARP)
+    trajectory_parity(gm, make_config("C4", scale=0.12), flags=gm.GM_FLAG_STEP_SUBWARP)
+    trajectory_parity(gm, make_config("C1"), flags=gm.GM_FLAG_STEP_SUBWARP)
+
+
 def test_launch_modes_are_bit_identical(gm):
     """Direct launches, graphs with early-exit gating and graphs with conditional nodes run the
     same kernels on the same data: trajectories agree bit for bit (and so does a repeated run)."""
