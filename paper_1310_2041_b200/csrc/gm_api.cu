@@ -56,7 +56,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
-    P->ns = (P->n + 1 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slot n: the far-away pad bead
+    P->ns = (P->n + 4 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+3 (at least): far-away pad beads
     P->sfc_period = c->sfc_period;
     P->n_types = c->n_types;
     P->max_bonds = c->max_bonds_per_particle;

@@ -57,7 +57,7 @@ struct GmPair { float c0, c1, c2, c3; };
 // Constants of one system, passed to kernels by value (constant bank).
 struct GmParams {
     int n, n_types, max_bonds, nl_cap;
-    int ns;                        // padded bead count: n + 1 rounded up to GM_PAD (slot n is the far-away pad bead)
+    int ns;                        // padded bead count: n + 4 rounded up to GM_PAD (slots n.. are far-away pad beads)
     int capq;                      // nl_cap / 4: int4 quads per NL row
     int minq;                      // quads of every row that are always written (padded): min(4, capq)
     int nc[3], n_cells;

@@ -10,19 +10,19 @@
 // ref[]: nine runs per bead instead of 27 cells (two more where the row wraps around the box).
 //
 // Hits are staged in a small lane-private shared-memory ring (NL_STAGE entries per lane, column l of
-// [NL_STAGE][32]: conflict-free and private to the lane, so no synchronisation); candidates are scanned in
-// chunks of NL_CHUNK, and after a chunk every lane that holds 16 or more staged entries writes four whole
+// [NL_STAGE][32]: conflict-free and private to the lane, so no synchronisation); candidates are scanned
+// four at a time, and after each four every lane that holds 16 or more staged entries writes four whole
 // int4 quads of its NL row (gm_internal.cuh: entries 4q..4q+3 of a bead are one int4; the 32 int4 of a
-// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 16 KB per CTA
+// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 20 KB per CTA
 // whatever the row capacity, which leaves the rest of the SM's 228 KB to L1 for the candidate loads.
 #include "gm_internal.cuh"
 
-#define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + NL_CHUNK)
-#define NL_CHUNK 16          // candidates scanned between two flush checks
+#define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 4)
 #define NL_WARPS 4
 
 struct NlRow {
     int *ring;               // this lane's column of the ring: ring[(k & (NL_STAGE-1)) * 32]
+    uint32_t lb;             // shared-memory byte address of ring[0] (the warp's ring is 4 KB-aligned)
     int4 *tile;              // this lane's int4 column of its NL tile: tile[q * 32]
     int k;                   // hits so far
     int flushed;             // entries already written to the tile (multiple of 16)
@@ -43,30 +43,62 @@ __device__ __forceinline__ void nl_flush16(NlRow &r)
     r.flushed += 16;
 }
 
-// One run of candidates ref[s0 .. s1) against bead i.  SHIFT: the run lies across a periodic face in
-// some dimension; the displacement is then taken relative to the two faces, (a -+ L/2) - (b +- L/2)
-// (see gm_min_image), with the bead side (ax, ay, az) prepared once per run and the candidate side
-// b + (hx, hy, hz) per candidate -- no branches in the chunk loop.
-template <bool SHIFT>
+// ring[(k & (NL_STAGE-1)) * 32] = v with k kept as the byte offset kb = 128 k: the address is
+// (kb & mask) | lb, one LOP3 (the warp's ring is 4 KB-aligned, so the two terms share no bits)
+__device__ __forceinline__ void nl_ring_put(uint32_t kb, uint32_t lb, int v)
+{
+    asm volatile("{\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %1, %2, 0xEA;\n\tst.shared.b32 [t], %3;\n\t}"
+                 :: "r"(kb), "n"((NL_STAGE - 1) * 128), "r"(lb), "r"(v) : "memory");
+}
+
+// kb += 128 if candidate u of this trip is inside the run (u < left), inside r_list and (SELF) not bead i:
+// two or three predicate-setting compares and one predicated add (written in PTX: the compiler otherwise
+// builds the increment from three selects).
+template <bool SELF>
+__device__ __forceinline__ void nl_count_hit(uint32_t &kb, float r2, float r_list2, int left, int u, int s, int i)
+{
+    if (SELF)
+        asm("{\n\t.reg .pred v, p;\n\tsetp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
+            "setp.ne.and.s32 p, %5, %6, p;\n\t@p add.u32 %0, %0, 128;\n\t}"
+            : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u), "r"(s), "r"(i));
+    else
+        asm("{\n\t.reg .pred v, p;\n\tsetp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
+            "@p add.u32 %0, %0, 128;\n\t}"
+            : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u));
+}
+
+// One run of candidates ref[s0 .. s1) against bead i, four at a time, every one predicated on s < s1 (the
+// runs of C3 hold ~9 candidates: no remainder loop, and the lanes of a warp make ceil(len / 4) trips).
+// SHIFT: the run lies across a periodic face in some dimension; the displacement is then taken relative to
+// the two faces, (a -+ L/2) - (b +- L/2) (see gm_min_image), with the bead side (ax, ay, az) prepared once
+// per run and the candidate side b + (hx, hy, hz) per candidate.  SELF: the run holds bead i itself.
+// The hit counter is kept as a byte offset into the lane's ring column (128 bytes per entry), so the
+// branch-free append costs one LOP3, one STS and one predicated add.
+template <bool SHIFT, bool SELF>
 __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
                                             float ay, float az, float hx, float hy, float hz, float r_list2,
                                             NlRow &r)
 {
-    for (int c0 = s0; c0 < s1; c0 += NL_CHUNK) {
-        const int c1 = min(c0 + NL_CHUNK, s1);
-        int k = r.k;
-#pragma unroll 4
-        for (int s = c0; s < c1; ++s) {
-            const float4 q = __ldg(ref + s);
+    uint32_t kb = (uint32_t)r.k * 128u;
+    for (int s = s0; s < s1; s += 4) {
+        // loads past the end of the run stay inside the array (per-bead arrays carry >= 4 pad slots after
+        // bead n - 1, GmParams::ns); what they return is masked by the `left` test
+        float4 q[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) q[u] = __ldg(ref + s + u);
+        const int left = s1 - s;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
             float dx, dy, dz;
-            if (SHIFT) { dx = ax - (q.x + hx); dy = ay - (q.y + hy); dz = az - (q.z + hz); }
-            else { dx = ax - q.x; dy = ay - q.y; dz = az - q.z; }
+            if (SHIFT) { dx = ax - (q[u].x + hx); dy = ay - (q[u].y + hy); dz = az - (q[u].z + hz); }
+            else { dx = ax - q[u].x; dy = ay - q[u].y; dz = az - q[u].z; }
             const float r2 = dx * dx + dy * dy + dz * dz;
-            r.ring[(k & (NL_STAGE - 1)) * 32] = s;      // branch-free append: the slot is kept only on a hit
-            k += (r2 < r_list2 && s != i) ? 1 : 0;
+            nl_ring_put(kb, r.lb, s + u);      // the slot is kept only on a hit
+            nl_count_hit<SELF>(kb, r2, r_list2, left, u, s + u, i);
         }
-        r.k = k;
-        if (k - r.flushed >= 16) nl_flush16(r);
+        // at most 4 new entries per trip: flush as soon as 16 are staged (ring of 32)
+        r.k = (int)(kb >> 7);
+        if (r.k - r.flushed >= 16) nl_flush16(r);
     }
 }
 
@@ -76,9 +108,14 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     if (!D.ctl->go) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    __shared__ int nl_ring[NL_WARPS][NL_STAGE][32];
+    // [NL_WARPS][NL_STAGE][32] ints, 4 KB per warp, aligned by hand to 4 KB in the shared window (nl_ring_put
+    // ORs the entry offset into the lane's base address); the launch asks for 4 KB of slack
+    extern __shared__ int nl_ring_raw[];
+    const uint32_t raw = (uint32_t)__cvta_generic_to_shared(nl_ring_raw);
+    int *nl_ring = nl_ring_raw + (((raw + 4095u) & ~4095u) - raw) / 4;
     NlRow row;
-    row.ring = &nl_ring[wid][0][lane];
+    row.ring = nl_ring + wid * (NL_STAGE * 32) + lane;
+    row.lb = (uint32_t)__cvta_generic_to_shared(row.ring);
     row.tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
     row.k = 0; row.flushed = 0; row.cap = P.nl_cap;
     const int cap = P.nl_cap;
@@ -102,8 +139,12 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
             for (int oz = -1; oz <= 1; ++oz)
                 for (int oy = -1; oy <= 1; ++oy) {
                     const int r0 = (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
-                    nl_scan_run<false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, pi.y,
-                                       pi.z, 0.f, 0.f, 0.f, rl2, row);
+                    if (oz == 0 && oy == 0)
+                        nl_scan_run<false, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
+                                                 pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
+                    else
+                        nl_scan_run<false, false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
+                                                  pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
                 }
         } else {
             for (int oz = -1; oz <= 1; ++oz) {
@@ -117,10 +158,10 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
                     if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
                     else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
                     const int r0 = (int)__ldg(rr + z * ncy + y) * ncx;
-                    nl_scan_run<true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
+                    nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
                                       0.f, hy, hz, rl2, row);
                     if (xb >= 0)
-                        nl_scan_run<true>(ref, __ldg(cstart + r0 + xb), __ldg(cstart + r0 + xb + 1), i, pi.x - hxb,
+                        nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xb), __ldg(cstart + r0 + xb + 1), i, pi.x - hxb,
                                           ay, az, hxb, hy, hz, rl2, row);
                 }
             }
@@ -163,7 +204,7 @@ cudaError_t gm_nl_prepare(const GmParams &P) { (void)P; return cudaSuccess; }
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     const int threads = NL_WARPS * 32;
-    k_nl_build<<<(P.ns + threads - 1) / threads, threads, 0, st>>>(P, D);
+    k_nl_build<<<(P.ns + threads - 1) / threads, threads, NL_WARPS * NL_STAGE * 32 * 4 + 4096, st>>>(P, D);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors): nn_out[tag], nl_out[tag*stride + k].
