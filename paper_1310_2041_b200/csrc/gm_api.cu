@@ -71,12 +71,24 @@ static gm_status derive(const gm_config *c, GmParams *P)
         if (P->nc[d] > 1024) P->nc[d] = 1024;
         vol *= c->box[d];
     }
+    // x only: cells r_list / sx wide, searched sx to either side (the run of a (y, z) row shrinks from 3 to
+    // 2 + 1/sx list radii); sx grows with the number of beads per r_list^3 cell
+    {
+        const double per_cell = (double)P->n / ((double)P->nc[0] * P->nc[1] * P->nc[2]);
+        int sx = per_cell >= 12.0 ? 4 : (per_cell >= 2.0 ? 2 : 1);
+        if (const char *e = getenv("GM_XDIV")) sx = std::max(1, std::min(8, atoi(e)));
+        P->sx = sx;
+        if (sx > 1) {
+            P->nc[0] = (int)std::floor((double)c->box[0] * sx / (r_list * 1.0001));
+            if (P->nc[0] > 4096) { P->sx = 1; P->nc[0] = 1024; }
+        }
+    }
     // sparse boxes: no more cells than a few per bead (wider cells stay correct)
     while ((long long)P->nc[0] * P->nc[1] * P->nc[2] > 8ll * P->n + 64) {
         int d = 0;
         if (P->nc[1] > P->nc[d]) d = 1;
         if (P->nc[2] > P->nc[d]) d = 2;
-        if (P->nc[d] <= 3) break;
+        if (P->nc[d] <= 3 * (d == 0 ? P->sx : 1)) break;
         P->nc[d] -= 1;
     }
     P->n_cells = P->nc[0] * P->nc[1] * P->nc[2];

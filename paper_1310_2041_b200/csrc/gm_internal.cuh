@@ -61,6 +61,7 @@ struct GmParams {
     int capq;                      // nl_cap / 4: int4 quads per NL row
     int minq;                      // quads of every row that are always written (padded): min(4, capq)
     int nc[3], n_cells;
+    int sx;                        // cells are r_list / sx wide in x: the search reaches sx cells to either side
     int step_subw;                 // lanes per bead of the step kernel: 1 (short lists), 4 or 8 (long lists)
     int sfc_period;                // a rebuild (= SFC sort) is forced after this many steps without one; <= 0: never
     float box[3], half[3], inv_w[3];

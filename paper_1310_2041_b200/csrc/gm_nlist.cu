@@ -6,8 +6,10 @@
 // Runs right after the sort of gm_sort.cu, so bead index == slot in the cell-sorted array `ref`: one
 // thread per bead, a warp owns 32 consecutive beads (a few adjacent cells of one x row), its lanes
 // read the same or adjacent candidates at every iteration and run nearly equal trip counts.  Cells run
-// along x inside a row, so the three x-adjacent cells of one (y, z) row are one contiguous run of
-// ref[]: nine runs per bead instead of 27 cells (two more where the row wraps around the box).
+// along x inside a row, so the x-adjacent cells of one (y, z) row are one contiguous run of
+// ref[]: nine runs per bead instead of 27 cells (more where the row wraps around the box).  Cells are
+// r_list wide in y and z but r_list / sx in x (GmParams::sx): a run then spans (2 + 1/sx) r_list instead
+// of 3 r_list -- fewer candidates per bead at no extra runs.
 //
 // Hits are staged in a small lane-private shared-memory ring (NL_STAGE entries per lane, column l of
 // [NL_STAGE][32]: conflict-free and private to the lane, so no synchronisation); candidates are scanned
@@ -18,7 +20,9 @@
 #include "gm_internal.cuh"
 
 #define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 4)
+#ifndef NL_WARPS
 #define NL_WARPS 4
+#endif
 
 struct NlRow {
     int *ring;               // this lane's column of the ring: ring[(k & (NL_STAGE-1)) * 32]
@@ -43,28 +47,27 @@ __device__ __forceinline__ void nl_flush16(NlRow &r)
     r.flushed += 16;
 }
 
-// ring[(k & (NL_STAGE-1)) * 32] = v with k kept as the byte offset kb = 128 k: the address is
-// (kb & mask) | lb, one LOP3 (the warp's ring is 4 KB-aligned, so the two terms share no bits)
-__device__ __forceinline__ void nl_ring_put(uint32_t kb, uint32_t lb, int v)
-{
-    asm volatile("{\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %1, %2, 0xEA;\n\tst.shared.b32 [t], %3;\n\t}"
-                 :: "r"(kb), "n"((NL_STAGE - 1) * 128), "r"(lb), "r"(v) : "memory");
-}
-
-// kb += 128 if candidate u of this trip is inside the run (u < left), inside r_list and (SELF) not bead i:
-// two or three predicate-setting compares and one predicated add (written in PTX: the compiler otherwise
-// builds the increment from three selects).
+// Append candidate slot s to the lane's ring column if it is inside the run (u < left), inside r_list and
+// (SELF) not bead i: ring[(k & (NL_STAGE-1)) * 32] = s; k += 1, with k kept as the byte offset kb = 128 k.
+// The address is (kb & mask) | lb, one LOP3 (the warp's ring is 4 KB-aligned, so the two terms share no
+// bits); store and increment are predicated on the hit (written in PTX: the compiler otherwise builds the
+// increment from three selects).
 template <bool SELF>
-__device__ __forceinline__ void nl_count_hit(uint32_t &kb, float r2, float r_list2, int left, int u, int s, int i)
+__device__ __forceinline__ void nl_append(uint32_t &kb, uint32_t lb, float r2, float r_list2, int left, int u,
+                                          int s, int i)
 {
     if (SELF)
-        asm("{\n\t.reg .pred v, p;\n\tsetp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
-            "setp.ne.and.s32 p, %5, %6, p;\n\t@p add.u32 %0, %0, 128;\n\t}"
-            : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u), "r"(s), "r"(i));
+        asm volatile("{\n\t.reg .pred v, p;\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %7, %8, 0xEA;\n\t"
+                     "setp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
+                     "setp.ne.and.s32 p, %5, %6, p;\n\t@p st.shared.b32 [t], %5;\n\t@p add.u32 %0, %0, 128;\n\t}"
+                     : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u), "r"(s), "r"(i),
+                       "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
     else
-        asm("{\n\t.reg .pred v, p;\n\tsetp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
-            "@p add.u32 %0, %0, 128;\n\t}"
-            : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u));
+        asm volatile("{\n\t.reg .pred v, p;\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %7, %8, 0xEA;\n\t"
+                     "setp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
+                     "@p st.shared.b32 [t], %5;\n\t@p add.u32 %0, %0, 128;\n\t}"
+                     : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u), "r"(s), "r"(i),
+                       "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
 }
 
 // One run of candidates ref[s0 .. s1) against bead i, four at a time, every one predicated on s < s1 (the
@@ -72,8 +75,6 @@ __device__ __forceinline__ void nl_count_hit(uint32_t &kb, float r2, float r_lis
 // SHIFT: the run lies across a periodic face in some dimension; the displacement is then taken relative to
 // the two faces, (a -+ L/2) - (b +- L/2) (see gm_min_image), with the bead side (ax, ay, az) prepared once
 // per run and the candidate side b + (hx, hy, hz) per candidate.  SELF: the run holds bead i itself.
-// The hit counter is kept as a byte offset into the lane's ring column (128 bytes per entry), so the
-// branch-free append costs one LOP3, one STS and one predicated add.
 template <bool SHIFT, bool SELF>
 __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
                                             float ay, float az, float hx, float hy, float hz, float r_list2,
@@ -93,8 +94,7 @@ __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int 
             if (SHIFT) { dx = ax - (q[u].x + hx); dy = ay - (q[u].y + hy); dz = az - (q[u].z + hz); }
             else { dx = ax - q[u].x; dy = ay - q[u].y; dz = az - q[u].z; }
             const float r2 = dx * dx + dy * dy + dz * dz;
-            nl_ring_put(kb, r.lb, s + u);      // the slot is kept only on a hit
-            nl_count_hit<SELF>(kb, r2, r_list2, left, u, s + u, i);
+            nl_append<SELF>(kb, r.lb, r2, r_list2, left, u, s + u, i);
         }
         // at most 4 new entries per trip: flush as soon as 16 are staged (ring of 32)
         r.k = (int)(kb >> 7);
@@ -102,7 +102,10 @@ __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int 
     }
 }
 
-__global__ void __launch_bounds__(128)
+#ifndef NL_MINB
+#define NL_MINB 1
+#endif
+__global__ void __launch_bounds__(NL_WARPS * 32, NL_MINB)
 k_nl_build(const __grid_constant__ GmParams P, GmDev D)
 {
     if (!D.ctl->go) return;
@@ -129,12 +132,16 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
         const int cz = gm_cell_coord(pi.z, P.half[2], P.inv_w[2], P.nc[2]);
         const int ncx = P.nc[0], ncy = P.nc[1], ncz = P.nc[2];
         const float rl2 = P.r_list2;
-        // x pieces of a row: cells [xa0, xa1] are contiguous in ref; a bead in an edge column also
-        // sees the single cell xb on the other side of the box
-        const int xa0 = max(cx - 1, 0), xa1 = min(cx + 1, ncx - 1);
-        const int xb = (cx == 0) ? ncx - 1 : ((cx == ncx - 1) ? 0 : -1);
-        const float hxb = (cx == 0) ? -P.half[0] : P.half[0];       // candidate side of the wrapped x piece
-        const bool inner = cx > 0 && cx < ncx - 1 && cy > 0 && cy < ncy - 1 && cz > 0 && cz < ncz - 1;
+        // x pieces of a row: cells [xa0, xa1] are contiguous in ref (cells are r_list / sx wide in x, so the
+        // run reaches sx cells to either side); a bead within sx cells of a face also sees the cells
+        // [xb0, xb1] on the other side of the box
+        const int sx = P.sx;
+        const int xa0 = max(cx - sx, 0), xa1 = min(cx + sx, ncx - 1);
+        const int xb0 = (cx < sx) ? ncx - (sx - cx) : 0;
+        const int xb1 = (cx < sx) ? ncx - 1 : cx + sx - ncx;
+        const bool has_xb = cx < sx || cx + sx > ncx - 1;
+        const float hxb = (cx < sx) ? -P.half[0] : P.half[0];       // candidate side of the wrapped x piece
+        const bool inner = cx >= sx && cx + sx <= ncx - 1 && cy > 0 && cy < ncy - 1 && cz > 0 && cz < ncz - 1;
         if (inner) {
             for (int oz = -1; oz <= 1; ++oz)
                 for (int oy = -1; oy <= 1; ++oy) {
@@ -160,8 +167,8 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
                     const int r0 = (int)__ldg(rr + z * ncy + y) * ncx;
                     nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
                                       0.f, hy, hz, rl2, row);
-                    if (xb >= 0)
-                        nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xb), __ldg(cstart + r0 + xb + 1), i, pi.x - hxb,
+                    if (has_xb)
+                        nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xb0), __ldg(cstart + r0 + xb1 + 1), i, pi.x - hxb,
                                           ay, az, hxb, hy, hz, rl2, row);
                 }
             }
