@@ -56,7 +56,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
-    P->ns = (P->n + 4 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+3 (at least): far-away pad beads
+    P->ns = (P->n + 8 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+7 (at least): far-away pad beads
     P->sfc_period = c->sfc_period;
     P->n_types = c->n_types;
     P->max_bonds = c->max_bonds_per_particle;
@@ -75,9 +75,12 @@ static gm_status derive(const gm_config *c, GmParams *P)
     // 2 + 1/sx list radii); sx grows with the number of beads per r_list^3 cell
     {
         const double per_cell = (double)P->n / ((double)P->nc[0] * P->nc[1] * P->nc[2]);
-        int sx = per_cell >= 12.0 ? 4 : (per_cell >= 2.0 ? 2 : 1);
+        int sx = per_cell >= 6.0 ? 4 : (per_cell >= 2.0 ? 3 : (per_cell >= 1.0 ? 2 : 1));   // measured: C3 3, C2/C4/C5 4
         if (const char *e = getenv("GM_XDIV")) sx = std::max(1, std::min(8, atoi(e)));
         P->sx = sx;
+        // mean candidates per run of a (y, z) row: (2 sx + 1) cells of per_cell / sx beads
+        P->nl_trip = per_cell * (2.0 * sx + 1.0) / sx >= 16.0 ? 8 : 4;
+        if (const char *e = getenv("GM_NLTRIP")) P->nl_trip = atoi(e) == 8 ? 8 : 4;
         if (sx > 1) {
             P->nc[0] = (int)std::floor((double)c->box[0] * sx / (r_list * 1.0001));
             if (P->nc[0] > 4096) { P->sx = 1; P->nc[0] = 1024; }

@@ -57,10 +57,11 @@ struct GmPair { float c0, c1, c2, c3; };
 // Constants of one system, passed to kernels by value (constant bank).
 struct GmParams {
     int n, n_types, max_bonds, nl_cap;
-    int ns;                        // padded bead count: n + 4 rounded up to GM_PAD (slots n.. are far-away pad beads)
+    int ns;                        // padded bead count: n + 8 rounded up to GM_PAD (slots n.. are far-away pad beads)
     int capq;                      // nl_cap / 4: int4 quads per NL row
     int minq;                      // quads of every row that are always written (padded): min(4, capq)
     int nc[3], n_cells;
+    int nl_trip;                   // candidates the NL build loads together: 4 (short runs) or 8
     int sx;                        // cells are r_list / sx wide in x: the search reaches sx cells to either side
     int step_subw;                 // lanes per bead of the step kernel: 1 (short lists), 4 or 8 (long lists)
     int sfc_period;                // a rebuild (= SFC sort) is forced after this many steps without one; <= 0: never

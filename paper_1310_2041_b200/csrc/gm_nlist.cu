@@ -75,37 +75,36 @@ __device__ __forceinline__ void nl_append(uint32_t &kb, uint32_t lb, float r2, f
 // SHIFT: the run lies across a periodic face in some dimension; the displacement is then taken relative to
 // the two faces, (a -+ L/2) - (b +- L/2) (see gm_min_image), with the bead side (ax, ay, az) prepared once
 // per run and the candidate side b + (hx, hy, hz) per candidate.  SELF: the run holds bead i itself.
-template <bool SHIFT, bool SELF>
+template <int TRIP, bool SHIFT, bool SELF>
 __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
                                             float ay, float az, float hx, float hy, float hz, float r_list2,
                                             NlRow &r)
 {
     uint32_t kb = (uint32_t)r.k * 128u;
-    for (int s = s0; s < s1; s += 4) {
-        // loads past the end of the run stay inside the array (per-bead arrays carry >= 4 pad slots after
+    for (int s = s0; s < s1; s += TRIP) {
+        // loads past the end of the run stay inside the array (per-bead arrays carry >= 8 pad slots after
         // bead n - 1, GmParams::ns); what they return is masked by the `left` test
-        float4 q[4];
+        float4 q[TRIP];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) q[u] = __ldg(ref + s + u);
+        for (int u = 0; u < TRIP; ++u) q[u] = __ldg(ref + s + u);
         const int left = s1 - s;
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < TRIP; ++u) {
             float dx, dy, dz;
             if (SHIFT) { dx = ax - (q[u].x + hx); dy = ay - (q[u].y + hy); dz = az - (q[u].z + hz); }
             else { dx = ax - q[u].x; dy = ay - q[u].y; dz = az - q[u].z; }
             const float r2 = dx * dx + dy * dy + dz * dz;
             nl_append<SELF>(kb, r.lb, r2, r_list2, left, u, s + u, i);
         }
-        // at most 4 new entries per trip: flush as soon as 16 are staged (ring of 32)
+        // at most TRIP <= 8 new entries per trip: flush as soon as 16 are staged (ring of 32)
         r.k = (int)(kb >> 7);
         if (r.k - r.flushed >= 16) nl_flush16(r);
     }
 }
 
-#ifndef NL_MINB
-#define NL_MINB 1
-#endif
-__global__ void __launch_bounds__(NL_WARPS * 32, NL_MINB)
+// TRIP: candidates loaded together (4: runs of ~10 candidates, C1/C3; 8: runs of 20 and more, C2/C4/C5)
+template <int TRIP>
+__global__ void __launch_bounds__(NL_WARPS * 32)
 k_nl_build(const __grid_constant__ GmParams P, GmDev D)
 {
     if (!D.ctl->go) return;
@@ -147,10 +146,10 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
                 for (int oy = -1; oy <= 1; ++oy) {
                     const int r0 = (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
                     if (oz == 0 && oy == 0)
-                        nl_scan_run<false, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
+                        nl_scan_run<TRIP, false, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
                                                  pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
                     else
-                        nl_scan_run<false, false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
+                        nl_scan_run<TRIP, false, false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
                                                   pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
                 }
         } else {
@@ -165,10 +164,10 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
                     if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
                     else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
                     const int r0 = (int)__ldg(rr + z * ncy + y) * ncx;
-                    nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
+                    nl_scan_run<TRIP, true, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
                                       0.f, hy, hz, rl2, row);
                     if (has_xb)
-                        nl_scan_run<true, true>(ref, __ldg(cstart + r0 + xb0), __ldg(cstart + r0 + xb1 + 1), i, pi.x - hxb,
+                        nl_scan_run<TRIP, true, true>(ref, __ldg(cstart + r0 + xb0), __ldg(cstart + r0 + xb1 + 1), i, pi.x - hxb,
                                           ay, az, hxb, hy, hz, rl2, row);
                 }
             }
@@ -211,7 +210,9 @@ cudaError_t gm_nl_prepare(const GmParams &P) { (void)P; return cudaSuccess; }
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     const int threads = NL_WARPS * 32;
-    k_nl_build<<<(P.ns + threads - 1) / threads, threads, NL_WARPS * NL_STAGE * 32 * 4 + 4096, st>>>(P, D);
+    const int smem = NL_WARPS * NL_STAGE * 32 * 4 + 4096;
+    if (P.nl_trip == 8) k_nl_build<8><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
+    else k_nl_build<4><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors): nn_out[tag], nl_out[tag*stride + k].
