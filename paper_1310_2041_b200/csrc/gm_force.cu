@@ -175,6 +175,74 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const Src &S, const
     o.cnt = cnt;
 }
 
+// DPD gather loop with per-lane compaction (a6).  A list slot costs ~12 instructions to test against r_c but
+// ~100 to evaluate (ten Philox rounds), and only ~37 % of the slots of a skin-padded list are inside r_c (C4):
+// evaluated slot by slot, a warp pays the Philox rounds for a slot whenever ANY of its lanes is in range, i.e.
+// always.  So pass 1 walks the row, tests r^2 and appends the in-range partner indices to a lane-private
+// shared-memory column; pass 2 evaluates two compacted partners per trip -- the warp makes max-over-lanes
+// (in-range count) / 2 trips instead of NN / 1.  The column holds GM_CPT_ROWS entries; it is drained early if
+// it could overflow.  col: this thread's column, entries GM_CPT_STRIDE ints apart.
+#define GM_CPT_ROWS 32
+#define GM_CPT_STRIDE 128
+// the compaction columns of a CTA of GM_CPT_STRIDE threads (DPD kernels only)
+#define GM_CPT_DECL(PAIR) __shared__ int gm_cpt[(PAIR) == GM_PAIR_DPD ? GM_CPT_ROWS * GM_CPT_STRIDE : 1]
+template <bool NT1, bool ENERGY, bool MI>
+__device__ __forceinline__ void pair_loop_dpd(const GmParams &P, const Src &S, const int4 *__restrict__ t,
+                                              uint64_t pol, const int4 (&pre)[GM_PRE], const int nn, const Own &me,
+                                              unsigned long long step, BeadForce &o, int *__restrict__ col)
+{
+    const int nq = (nn + 3) >> 2;
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
+    const GmPair p0 = P.pair[0];
+    int k = 0;
+    auto scan_quad = [&](const int4 e) {
+        float4 pj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pj[u] = __ldg(S.pos + quad_get(e, u));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float dx, dy, dz;
+            if (MI) {
+                dx = gm_min_image_signed(me.p.x, me.ax, me.hx, pj[u].x, P.half[0]);
+                dy = gm_min_image_signed(me.p.y, me.ay, me.hy, pj[u].y, P.half[1]);
+                dz = gm_min_image_signed(me.p.z, me.az, me.hz, pj[u].z, P.half[2]);
+            } else {
+                dx = me.p.x - pj[u].x; dy = me.p.y - pj[u].y; dz = me.p.z - pj[u].z;
+            }
+            const float r2 = dx * dx + dy * dy + dz * dz;
+            const float cut = NT1 ? p0.c0 : P.pair[me.t * P.n_types + __float_as_int(pj[u].w)].c0;
+            col[k * GM_CPT_STRIDE] = quad_get(e, u);       // kept only if in range
+            k += (r2 < cut) ? 1 : 0;
+        }
+    };
+    auto drain = [&]() {
+        for (int c = 0; c < k; c += 2) {
+            const int j0 = col[c * GM_CPT_STRIDE];
+            const int j1 = (c + 1 < k) ? col[(c + 1) * GM_CPT_STRIDE] : P.n;     // the far-away pad bead
+            const float4 q0 = __ldg(S.pos + j0), q1 = __ldg(S.pos + j1);
+            const float4 w0 = __ldg(S.vt + j0), w1 = __ldg(S.vt + j1);
+            pair_term<GM_PAIR_DPD, NT1, ENERGY, MI>(P, me, q0, w0, p0, (uint32_t)step, fx, fy, fz, pe, cnt);
+            pair_term<GM_PAIR_DPD, NT1, ENERGY, MI>(P, me, q1, w1, p0, (uint32_t)step, fx, fy, fz, pe, cnt);
+        }
+        k = 0;
+    };
+    const int4 pad = make_int4(P.n, P.n, P.n, P.n);
+    int4 en = (GM_PRE < nq) ? gm_ld_stream(t + GM_PRE * 32, pol) : pad;
+#pragma unroll
+    for (int b = 0; b < GM_PRE; ++b)
+        if (b < nq) scan_quad(pre[b]);
+    for (int q = GM_PRE; q < nq; ++q) {
+        const int4 e = en;
+        en = (q + 1 < nq) ? gm_ld_stream(t + (q + 1) * 32, pol) : pad;
+        if (k > GM_CPT_ROWS - 4) drain();
+        scan_quad(e);
+    }
+    drain();
+    o.fx += fx; o.fy += fy; o.fz += fz;
+    o.pe_pair = 0.5f * pe;
+    o.cnt = cnt;
+}
+
 // Bond partners of bead i from column i of BL (Fig. 2), two at a time; -1 = no bond.
 template <int BOND, bool ENERGY>
 __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, const Src &S, int i, const float4 pi,
@@ -230,7 +298,7 @@ template <int PAIR, bool NT1, int BOND, bool ENERGY>
 __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const Src &S, int i,
                                                 const float4 pi, const float4 vti, const int4 *__restrict__ t,
                                                 uint64_t pol, const int4 (&pre)[GM_PRE], const int nn,
-                                                unsigned long long step)
+                                                unsigned long long step, int *__restrict__ col)
 {
     BeadForce o;
     o.fx = o.fy = o.fz = o.pe_pair = o.pe_bond = o.cnt = 0.f;
@@ -246,7 +314,10 @@ __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &
         const float m = P.edge_margin;
         const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
                               fabsf(pi.z) < P.half[2] - m;
-        if (__all_sync(__activemask(), interior)) pair_loop<PAIR, NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o);
+        if (PAIR == GM_PAIR_DPD) {
+            if (__all_sync(__activemask(), interior)) pair_loop_dpd<NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o, col);
+            else pair_loop_dpd<NT1, ENERGY, true>(P, S, t, pol, pre, nn, me, step, o, col);
+        } else if (__all_sync(__activemask(), interior)) pair_loop<PAIR, NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o);
         else pair_loop<PAIR, NT1, ENERGY, true>(P, S, t, pol, pre, nn, me, step, o);
     }
     return o;
@@ -274,7 +345,7 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, in
 template <int PAIR, bool NT1, int BOND, int MODE>
 __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, const Src &S, const int i,
                                           const unsigned long long step, const int parity, const float kick,
-                                          const float kick_vt)
+                                          const float kick_vt, int *__restrict__ col)
 {
     // every stream of this bead is requested before anything is used
     const uint64_t pol = gm_policy_evict_first();
@@ -288,7 +359,7 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
     if (MODE == GM_MODE_STEP) rf = gm_ld_nol1(D.ref + i);
     float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
     if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES>(P, D, S, i, pi, vti, t, pol, pre, nn, step);
+    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col);
     const float3 a = bead_accel(P, S, i, f, u, step);
     if (MODE == GM_MODE_FORCES) {
         D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
@@ -316,8 +387,9 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned long long step = D.ctl->step[parity];
     const Src S = current_src(D, parity, step);
+    GM_CPT_DECL(PAIR);
     if (i >= P.n) return;
-    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES>(P, D, S, i, step, parity, 0.f, 0.f);
+    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES>(P, D, S, i, step, parity, 0.f, 0.f, gm_cpt + threadIdx.x);
 }
 
 // The step kernel (a4..a8).  A CTA owns STEP_BLOCK consecutive beads: storage order is cell order along
@@ -337,7 +409,8 @@ k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, floa
             D.ctl->need = step + 1;
     }
     const int i = blockIdx.x * STEP_BLOCK + threadIdx.x;
-    if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP>(P, D, S, i, step, parity, kick, kick_vt);
+    GM_CPT_DECL(PAIR);
+    if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP>(P, D, S, i, step, parity, kick, kick_vt, gm_cpt + threadIdx.x);
 }
 
 // The step kernel for LONG neighbor lists (n_l of 80-100: LJ with r_c = 2.5, configs C2/C5): SUBW lanes share
@@ -426,6 +499,7 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
 {
     const unsigned long long step = D.ctl->step[parity];
     const Src S = current_src(D, parity, step);
+    GM_CPT_DECL(PAIR);
     double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };   // ke, pe_pair, pe_bond, px, py, pz, pairs
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += gridDim.x * blockDim.x) {
         const uint64_t pol = gm_policy_evict_first();
@@ -436,7 +510,7 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
         const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
         float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
         if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-        const BeadForce f = bead_force<PAIR, NT1, BOND, true>(P, D, S, i, pi, vti, t, pol, pre, nn, step);
+        const BeadForce f = bead_force<PAIR, NT1, BOND, true>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x);
         const float4 u = S.vel[i];
         float vx = u.x, vy = u.y, vz = u.z;
         if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m
