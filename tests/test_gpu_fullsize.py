@@ -140,4 +140,10 @@ def test_c4_scaled_dpd_temperature_statistics(gm):
     g, o = g[30:], o[30:]
     assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)
     assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)
-    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)
+    # <Rg^2> of 300 ten-bead chains: a run average over 1200 steps still carries a standard error of about 1 %
+    # (chain shapes relax over hundreds of steps), estimated here from four block means of each run; the two
+    # averages must agree within 1 % or three standard errors of their difference, whichever is larger
+    def block_se(x):
+        return np.std([b.mean() for b in np.array_split(x, 4)], ddof=1) / 2.0
+    tol = max(0.01 * o[:, 5].mean(), 3.0 * np.hypot(block_se(g[:, 5]), block_se(o[:, 5])))
+    assert abs(g[:, 5].mean() - o[:, 5].mean()) <= tol

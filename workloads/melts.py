@@ -159,7 +159,7 @@ CONFIGS = {
                integrator="langevin", gamma=1.0, n_steps=10_000),
     "C3": dict(kind="kg", n=1_000_000, chain_len=100, n_lat=100, box=_kg_box(1_000_000), rc=WCA_RC,
                skin=0.4, integrator="nve", gamma=1.0, n_steps=10_000, sfc_period=500, equil_steps=1_000),
-    "C4": dict(kind="dpd", n_chains=300_000, box=100.0, skin=0.4, n_steps=5_000),
+    "C4": dict(kind="dpd", n_chains=300_000, box=100.0, skin=0.6, n_steps=5_000),
     "C5": dict(kind="kg", n=8_000_000, chain_len=200, n_lat=200, box=_kg_box(8_000_000), rc=2.5,
                skin=0.3, integrator="nve", gamma=0.0, n_steps=2_000, sfc_period=200),
 }
