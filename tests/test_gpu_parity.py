@@ -115,6 +115,35 @@ def forces_parity(gm, w, steps_before=0, tol=1e-4):
     return frms
 
 
+@pytest.mark.parametrize("xdiv,trip", [(1, 4), (2, 8), (3, 4), (4, 8), (8, 4)])
+def test_cell_refinement_and_scan_width_do_not_change_the_list_or_the_forces(gm, monkeypatch, xdiv, trip):
+    # a3: cells r_list / sx wide in x and 4 or 8 candidates per trip are exact accelerations (DESIGN.md c-12);
+    # the overrides are read by gm_create.  Non-cubic box with beads on the faces, then C1 forces.
+    monkeypatch.setenv("GM_XDIV", str(xdiv))
+    monkeypatch.setenv("GM_NLTRIP", str(trip))
+    w = make_random_box(3000, [9.0, 13.5, 17.25], seed=6)
+    w.pos[:50, 0] = -4.5                                       # exactly on the lower face
+    w.pos[50:100, 1] = np.nextafter(np.float32(6.75), np.float32(0))   # last value below the upper face
+    w.pos[100:120] = w.pos[120:140]                            # coincident beads
+    check_neighbor_sets(gm, w, use_cells=False)
+    forces_parity(gm, make_config("C1"), steps_before=12)
+
+
+def test_forces_dense_dpd_exercises_the_early_drain_of_the_compaction_column(gm):
+    # a6: rho = 9 puts ~38 partners inside r_c = 1, more than the 28 the compaction column holds before it
+    # is drained (pair_loop_dpd); 2 types, harmonic bonds, velocities set so the dissipative term is live
+    rng = np.random.default_rng(21)
+    box, n = 7.0, 3087
+    pos = rng.uniform(-0.5 * box, 0.5 * box, (n, 3)).astype(np.float32)
+    vel = rng.normal(0, 1, (n, 3)).astype(np.float32)
+    typ = (np.arange(n) % 2).astype(np.int32)
+    bonds = np.stack([np.arange(0, n - 1, 3), np.arange(1, n, 3)], axis=1)
+    w = custom(pos, box, vel=vel, typ=typ, bonds=bonds, pair_style="dpd", a=np.array([[25.0, 40.0], [40.0, 25.0]]),
+               rc=1.0, bond_style="harmonic", k=4.0, r0=0.0, integrator="gwvv", dt=0.04, gamma=4.5, r_skin=0.3,
+               n_types=2)
+    forces_parity(gm, w)
+
+
 def test_forces_c1_wca_fene(gm):
     forces_parity(gm, make_config("C1"))
 
