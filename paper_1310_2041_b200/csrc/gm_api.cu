@@ -110,6 +110,11 @@ static gm_status derive(const gm_config *c, GmParams *P)
         double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
         cap = (int)(2.0 * nbar) + 48;     // random-walk DPD starts (C4) reach ~3x the mean in places
     }
+    {
+        const double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
+        P->step_wide = nbar >= 40.0 ? 1 : 0;       // measured: C1/C3 (13) narrow, C2/C5 (78) wide
+        if (const char *e = getenv("GM_STEP_WIDE")) P->step_wide = atoi(e) != 0;
+    }
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
     cap = (cap + 7) / 8 * 8;
     P->nl_cap = cap;

@@ -25,13 +25,20 @@
 
 #define FORCE_BLOCK 128
 #ifndef STEP_BLOCK
-#define STEP_BLOCK 128           // beads per CTA of the step kernel
+#define STEP_BLOCK 32            // beads per CTA of the short-list step kernel: one warp
 #endif
 #ifndef STEP_MINB
-#define STEP_MINB 7              // minimum resident CTAs per SM the step kernel is compiled for (72 registers)
+#define STEP_MINB 32             // resident CTAs per SM of the short-list step kernel (<= 64 registers, 32 warps)
+#endif
+#ifndef WIDE_BLOCK
+#define WIDE_BLOCK 128           // long lists and DPD: CTAs of 128 beads,
+#define WIDE_MINB 7              //   7 resident per SM (72 registers)
+#endif
+#ifndef SUB_BLOCK
+#define SUB_BLOCK 128            // threads per CTA of the sub-warp step kernel
 #endif
 #ifndef GM_LJ_NQ
-#define GM_LJ_NQ 2               // quads (of 4 list entries) per batch of the LJ gather loop
+#define GM_LJ_NQ 1               // quads (of 4 list entries) per batch of the LJ gather loop
 #endif
 
 struct BeadForce {
@@ -125,12 +132,12 @@ __device__ __forceinline__ void nl_preload(const GmParams &P, const int4 *__rest
 
 // Gather loop over row i of NL (Alg. 2), NQ quads (4 NQ list entries) per batch:
 // first the preloaded quads, then a software-pipelined loop over the rest of the row.
-template <int PAIR, bool NT1, bool ENERGY, bool MI>
+template <int PAIR, bool NT1, bool ENERGY, bool MI, int NQL>
 __device__ __forceinline__ void pair_loop(const GmParams &P, const Src &S, const int4 *__restrict__ t,
                                           uint64_t pol, const int4 (&pre)[GM_PRE], const int nn, const Own &me,
                                           unsigned long long step, BeadForce &o)
 {
-    constexpr int NQ = (PAIR == GM_PAIR_DPD) ? 1 : GM_LJ_NQ;
+    constexpr int NQ = (PAIR == GM_PAIR_DPD) ? 1 : NQL;
     const int nq = (nn + 3) >> 2;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
     const GmPair p0 = P.pair[0];
@@ -181,16 +188,16 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const Src &S, const
 // always.  So pass 1 walks the row, tests r^2 and appends the in-range partner indices to a lane-private
 // shared-memory column; pass 2 evaluates two compacted partners per trip -- the warp makes max-over-lanes
 // (in-range count) / 2 trips instead of NN / 1.  The column holds GM_CPT_ROWS entries; it is drained early if
-// it could overflow.  col: this thread's column, entries GM_CPT_STRIDE ints apart.
+// it could overflow.  col: this thread's column, entries `stride` (= blockDim.x) ints apart.
 #define GM_CPT_ROWS 32
-#define GM_CPT_STRIDE 128
-// the compaction columns of a CTA of GM_CPT_STRIDE threads (DPD kernels only)
-#define GM_CPT_DECL(PAIR) __shared__ int gm_cpt[(PAIR) == GM_PAIR_DPD ? GM_CPT_ROWS * GM_CPT_STRIDE : 1]
+// the compaction columns of a CTA of NT threads (DPD kernels only); entry k of thread t is gm_cpt[k * NT + t]
+#define GM_CPT_DECL(PAIR, NT) __shared__ int gm_cpt[(PAIR) == GM_PAIR_DPD ? GM_CPT_ROWS * (NT) : 1]
 template <bool NT1, bool ENERGY, bool MI>
 __device__ __forceinline__ void pair_loop_dpd(const GmParams &P, const Src &S, const int4 *__restrict__ t,
                                               uint64_t pol, const int4 (&pre)[GM_PRE], const int nn, const Own &me,
                                               unsigned long long step, BeadForce &o, int *__restrict__ col)
 {
+    const int stride = (int)blockDim.x;
     const int nq = (nn + 3) >> 2;
     float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
     const GmPair p0 = P.pair[0];
@@ -211,14 +218,14 @@ __device__ __forceinline__ void pair_loop_dpd(const GmParams &P, const Src &S, c
             }
             const float r2 = dx * dx + dy * dy + dz * dz;
             const float cut = NT1 ? p0.c0 : P.pair[me.t * P.n_types + __float_as_int(pj[u].w)].c0;
-            col[k * GM_CPT_STRIDE] = quad_get(e, u);       // kept only if in range
+            col[k * stride] = quad_get(e, u);       // kept only if in range
             k += (r2 < cut) ? 1 : 0;
         }
     };
     auto drain = [&]() {
         for (int c = 0; c < k; c += 2) {
-            const int j0 = col[c * GM_CPT_STRIDE];
-            const int j1 = (c + 1 < k) ? col[(c + 1) * GM_CPT_STRIDE] : P.n;     // the far-away pad bead
+            const int j0 = col[c * stride];
+            const int j1 = (c + 1 < k) ? col[(c + 1) * stride] : P.n;     // the far-away pad bead
             const float4 q0 = __ldg(S.pos + j0), q1 = __ldg(S.pos + j1);
             const float4 w0 = __ldg(S.vt + j0), w1 = __ldg(S.vt + j1);
             pair_term<GM_PAIR_DPD, NT1, ENERGY, MI>(P, me, q0, w0, p0, (uint32_t)step, fx, fy, fz, pe, cnt);
@@ -294,7 +301,7 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
 
 // Force on bead i at time level `step`, conservative + (DPD) dissipative/random.  vti: own v~ and tag.
 // pre / nn: the preloaded head of row i and NN[i].
-template <int PAIR, bool NT1, int BOND, bool ENERGY>
+template <int PAIR, bool NT1, int BOND, bool ENERGY, int NQL>
 __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const Src &S, int i,
                                                 const float4 pi, const float4 vti, const int4 *__restrict__ t,
                                                 uint64_t pol, const int4 (&pre)[GM_PRE], const int nn,
@@ -317,8 +324,8 @@ __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &
         if (PAIR == GM_PAIR_DPD) {
             if (__all_sync(__activemask(), interior)) pair_loop_dpd<NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o, col);
             else pair_loop_dpd<NT1, ENERGY, true>(P, S, t, pol, pre, nn, me, step, o, col);
-        } else if (__all_sync(__activemask(), interior)) pair_loop<PAIR, NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o);
-        else pair_loop<PAIR, NT1, ENERGY, true>(P, S, t, pol, pre, nn, me, step, o);
+        } else if (__all_sync(__activemask(), interior)) pair_loop<PAIR, NT1, ENERGY, false, NQL>(P, S, t, pol, pre, nn, me, step, o);
+        else pair_loop<PAIR, NT1, ENERGY, true, NQL>(P, S, t, pol, pre, nn, me, step, o);
     }
     return o;
 }
@@ -342,7 +349,7 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, in
 }
 
 // ---- the per-step work of one bead (MODE_STEP) / its materialised force (MODE_FORCES) -----------------
-template <int PAIR, bool NT1, int BOND, int MODE>
+template <int PAIR, bool NT1, int BOND, int MODE, int NQL>
 __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, const Src &S, const int i,
                                           const unsigned long long step, const int parity, const float kick,
                                           const float kick_vt, int *__restrict__ col)
@@ -359,7 +366,7 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
     if (MODE == GM_MODE_STEP) rf = gm_ld_nol1(D.ref + i);
     float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
     if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col);
+    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES, NQL>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col);
     const float3 a = bead_accel(P, S, i, f, u, step);
     if (MODE == GM_MODE_FORCES) {
         D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
@@ -387,16 +394,20 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const unsigned long long step = D.ctl->step[parity];
     const Src S = current_src(D, parity, step);
-    GM_CPT_DECL(PAIR);
+    GM_CPT_DECL(PAIR, FORCE_BLOCK);
     if (i >= P.n) return;
-    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES>(P, D, S, i, step, parity, 0.f, 0.f, gm_cpt + threadIdx.x);
+    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES, GM_LJ_NQ>(P, D, S, i, step, parity, 0.f, 0.f, gm_cpt + threadIdx.x);
 }
 
-// The step kernel (a4..a8).  A CTA owns STEP_BLOCK consecutive beads: storage order is cell order along
-// the curve, so its warps work side by side on a few adjacent (y, z) rows of cells and share the neighbor
-// positions they gather through the SM's L1.
-template <int PAIR, bool NT1, int BOND>
-__global__ void __launch_bounds__(STEP_BLOCK, STEP_MINB)
+// The step kernel (a4..a8).  A CTA owns BLOCK consecutive beads: storage order is cell order along the curve,
+// so neighboring CTAs work side by side on a few adjacent (y, z) rows of cells and share the neighbor positions
+// they gather through the SM's L1.  Two shapes, chosen by the mean list length (GmParams::step_wide):
+//   short lists (C1/C3, n_l ~ 13): CTAs of ONE warp, 32 resident per SM (<= 64 registers), gather batches of one
+//     quad -- a warp's slot is free the moment it is done instead of waiting for the slowest of four
+//     (measured on C3: 48.2 -> 42.8 us);
+//   long lists (C2/C5, n_l ~ 90) and DPD: CTAs of 128, 7 resident per SM, batches of two quads.
+template <int PAIR, bool NT1, int BOND, int BLOCK, int MINB, int NQL>
+__global__ void __launch_bounds__(BLOCK, MINB)
 k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
 {
     const unsigned long long step = D.ctl->step[parity];
@@ -408,9 +419,9 @@ k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, floa
             step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
             D.ctl->need = step + 1;
     }
-    const int i = blockIdx.x * STEP_BLOCK + threadIdx.x;
-    GM_CPT_DECL(PAIR);
-    if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP>(P, D, S, i, step, parity, kick, kick_vt, gm_cpt + threadIdx.x);
+    const int i = blockIdx.x * BLOCK + threadIdx.x;
+    GM_CPT_DECL(PAIR, BLOCK);
+    if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP, NQL>(P, D, S, i, step, parity, kick, kick_vt, gm_cpt + threadIdx.x);
 }
 
 // The step kernel for LONG neighbor lists (n_l of 80-100: LJ with r_c = 2.5, configs C2/C5): SUBW lanes share
@@ -420,7 +431,7 @@ k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, floa
 // 2,000 warps -- half a wave on 148 SMs, each thread walking ~90 dependent gathers; with 8 lanes per bead it is
 // 16,000 warps of ~11 gathers per lane.  Still no atomics: a bead's force is owned by one group.
 template <int PAIR, bool NT1, int BOND, int SUBW>
-__global__ void __launch_bounds__(STEP_BLOCK)
+__global__ void __launch_bounds__(SUB_BLOCK)
 k_step_sub(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, float kick_vt)
 {
     const unsigned long long step = D.ctl->step[parity];
@@ -431,7 +442,7 @@ k_step_sub(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, 
             step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
             D.ctl->need = step + 1;
     }
-    const long long gt = (long long)blockIdx.x * STEP_BLOCK + threadIdx.x;
+    const long long gt = (long long)blockIdx.x * SUB_BLOCK + threadIdx.x;
     const int i = (int)(gt / SUBW), sub = (int)(gt % SUBW);
     const bool valid = i < P.n;
     const int ic = valid ? i : 0;                       // idle groups shadow bead 0 and write nothing
@@ -499,7 +510,7 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
 {
     const unsigned long long step = D.ctl->step[parity];
     const Src S = current_src(D, parity, step);
-    GM_CPT_DECL(PAIR);
+    GM_CPT_DECL(PAIR, FORCE_BLOCK);
     double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };   // ke, pe_pair, pe_bond, px, py, pz, pairs
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += gridDim.x * blockDim.x) {
         const uint64_t pol = gm_policy_evict_first();
@@ -510,7 +521,7 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
         const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
         float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
         if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-        const BeadForce f = bead_force<PAIR, NT1, BOND, true>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x);
+        const BeadForce f = bead_force<PAIR, NT1, BOND, true, GM_LJ_NQ>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x);
         const float4 u = S.vel[i];
         float vx = u.x, vy = u.y, vz = u.z;
         if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m
@@ -557,10 +568,14 @@ static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int pari
     if (mode == GM_MODE_STEP) {
         if (P.step_subw == 8 && PAIR != GM_PAIR_NONE) {
             const long long nt = (long long)P.n * 8;
-            k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + STEP_BLOCK - 1) / STEP_BLOCK), STEP_BLOCK, 0, st>>>(
+            k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + SUB_BLOCK - 1) / SUB_BLOCK), SUB_BLOCK, 0, st>>>(
                 P, D, parity, kick, kick_vt);
-        } else
-            k_step<PAIR, NT1, BOND><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(P, D, parity, kick, kick_vt);
+        } else if (P.step_wide || PAIR == GM_PAIR_DPD)
+            k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, 2><<<(P.n + WIDE_BLOCK - 1) / WIDE_BLOCK, WIDE_BLOCK, 0, st>>>(
+                P, D, parity, kick, kick_vt);
+        else if constexpr (PAIR != GM_PAIR_DPD)
+            k_step<PAIR, NT1, BOND, STEP_BLOCK, STEP_MINB, GM_LJ_NQ><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(
+                P, D, parity, kick, kick_vt);
     } else if (mode == GM_MODE_FORCES)
         k_force<PAIR, NT1, BOND><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity);
     else {

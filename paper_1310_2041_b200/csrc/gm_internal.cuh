@@ -63,6 +63,7 @@ struct GmParams {
     int nc[3], n_cells;
     int nl_trip;                   // candidates the NL build loads together: 4 (short runs) or 8
     int sx;                        // cells are r_list / sx wide in x: the search reaches sx cells to either side
+    int step_wide;                 // step kernel shape: 0 = one-warp CTAs (short lists), 1 = CTAs of 128 (long lists)
     int step_subw;                 // lanes per bead of the step kernel: 1 (short lists), 4 or 8 (long lists)
     int sfc_period;                // a rebuild (= SFC sort) is forced after this many steps without one; <= 0: never
     float box[3], half[3], inv_w[3];
