@@ -34,6 +34,9 @@
 #define WIDE_BLOCK 128           // long lists and DPD: CTAs of 128 beads,
 #define WIDE_MINB 7              //   7 resident per SM (72 registers)
 #endif
+#ifndef WIDE_NQ
+#define WIDE_NQ 2                //   gather batches of two quads
+#endif
 #ifndef SUB_BLOCK
 #define SUB_BLOCK 128            // threads per CTA of the sub-warp step kernel
 #endif
@@ -571,7 +574,7 @@ static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int pari
             k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + SUB_BLOCK - 1) / SUB_BLOCK), SUB_BLOCK, 0, st>>>(
                 P, D, parity, kick, kick_vt);
         } else if (P.step_wide || PAIR == GM_PAIR_DPD)
-            k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, 2><<<(P.n + WIDE_BLOCK - 1) / WIDE_BLOCK, WIDE_BLOCK, 0, st>>>(
+            k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, WIDE_NQ><<<(P.n + WIDE_BLOCK - 1) / WIDE_BLOCK, WIDE_BLOCK, 0, st>>>(
                 P, D, parity, kick, kick_vt);
         else if constexpr (PAIR != GM_PAIR_DPD)
             k_step<PAIR, NT1, BOND, STEP_BLOCK, STEP_MINB, GM_LJ_NQ><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(
