@@ -145,6 +145,22 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
+def max_over_ranks(ms: float, world: int, device) -> float:
+    """Device-timed milliseconds of the slowest rank (replicas only: no data-path collective)."""
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        t = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms
+
+
+def whole_job_value(world: int, timesteps_per_rank: int, ms: float) -> float:
+    """Whole-job timesteps/s of `world` independent replicas that each ran timesteps_per_rank in (max) ms."""
+    return world * timesteps_per_rank / (ms * 1e-3)
+
+
 def describe(w) -> str:
     rc = float(np.max(w.pair["rc"]))
     return (f"{w.name}: {w.n} beads, chains of {w.chain_len}, box {float(w.box[0]):.3f}, {w.pair_style} rc={rc:.4f}, "
@@ -234,12 +250,9 @@ def main():
     ms = e0.elapsed_time(e1)
     clk = clocks.stop()
     st2 = s.stats()
-    if world > 1:
-        t = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, world, dev)
     n_ts = args.steps * inner
-    tps = world * n_ts / (ms * 1e-3)
+    tps = whole_job_value(world, n_ts, ms)
     rebuilds = st2["rebuilds"] - st1["rebuilds"]
     reorders = st2["reorders"] - st1["reorders"]
     nbar_l = st2["sum_nn"] / w.n
