@@ -261,9 +261,10 @@ def main():
     pairs_in_rc = en["n_pairs"]
 
     # kernels launched inside the timed region: per timestep the gate + the fused force/integrate kernel;
-    # per rebuild 6 (keys, 2 scan, scatter, permute = SFC sort of all particle arrays, NL build)
+    # per rebuild 6 (keys, 2 scan, scatter, permute = SFC sort of all particle arrays, NL build), 7 with bonds
+    # (BL remap to the new bead indices)
 
-    launches = n_ts * 2 + rebuilds * 6
+    launches = n_ts * 2 + rebuilds * (7 if len(w.bonds) else 6)
 
     # ---- the dominant kernel alone: CUDA events around every launch (gm_step_timed) ----------------
     n_prof = min(inner, 200)

@@ -173,13 +173,6 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
             }
         }
         if (row.k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
-        // a7 set-up: BL of this slot in index space from its tag-space row (the sort moved the beads)
-        const int sel = (int)(D.ctl->n_rebuilds & 1ull);
-        const size_t ns = (size_t)P.ns;
-        for (int b = 0; b < P.max_bonds; ++b) {
-            const int e = D.blt[sel][b * ns + i];
-            D.bl[b * ns + i] = e < 0 ? -1 : (D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK));
-        }
     }
     // the tail of the row: whole quads, at least minq of them in all (the force kernel loads those before
     // it knows NN), padded with the far-away bead
@@ -203,6 +196,23 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     }
 }
 
+// a7 set-up: BL of every slot in index space from its tag-space row (the sort moved the beads).  A kernel of
+// its own (full occupancy, a dozen registers): at the end of k_nl_build the dependent blt -> rtag -> store chain
+// kept every warp's slot for two more memory latencies.
+__global__ void __launch_bounds__(256)
+k_bl_remap(const __grid_constant__ GmParams P, GmDev D)
+{
+    if (!D.ctl->go) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= P.n) return;
+    const int sel = (int)(D.ctl->n_rebuilds & 1ull);
+    const size_t ns = (size_t)P.ns;
+    for (int b = 0; b < P.max_bonds; ++b) {
+        const int e = D.blt[sel][b * ns + i];
+        D.bl[b * ns + i] = e < 0 ? -1 : (D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK));
+    }
+}
+
 int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 4 == 0; }
 
 cudaError_t gm_nl_prepare(const GmParams &P) { (void)P; return cudaSuccess; }
@@ -210,6 +220,7 @@ cudaError_t gm_nl_prepare(const GmParams &P) { (void)P; return cudaSuccess; }
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     const int threads = NL_WARPS * 32;
+    if (P.max_bonds > 0) k_bl_remap<<<(P.n + 255) / 256, 256, 0, st>>>(P, D);
     const int smem = NL_WARPS * NL_STAGE * 32 * 4 + 4096;
     if (P.nl_trip == 8) k_nl_build<8><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
     else k_nl_build<4><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);

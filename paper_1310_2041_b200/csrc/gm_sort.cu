@@ -16,7 +16,7 @@
 //
 // Chain: k_gate (decide, publish ctl->go) -> k_keys (key + histogram) -> k_scan_local / k_scan_add
 // (exclusive scan -> cstart) -> k_scatter (slot lists per cell) -> k_permute (canonical slot, move state)
-// -> k_nl_build (gm_nlist.cu).
+// -> k_bl_remap, k_nl_build (gm_nlist.cu).
 #include "gm_internal.cuh"
 
 #define SORT_BLOCK 256
