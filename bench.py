@@ -322,7 +322,7 @@ def main():
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cores = os.cpu_count() or 1
         t1, _ = oracle_timesteps(w, 1, cores)
-        k = int(max(2, min(50, 15.0 / max(t1, 1e-3))))
+        k = int(max(2, min(200, 15.0 / max(t1, 1e-3))))       # about 15 s of CPU work
         tt, thr = oracle_timesteps(w, k, cores)
         cpu = {"value": k / tt, "unit": "timesteps/s", "cores": thr, "kind": "oracle",
                "sample": f"{k} MD timesteps of {w.name} (N={w.n}) from the start state, fp64 cell-list oracle, OpenMP over beads"}
