@@ -20,6 +20,7 @@
 #include "gm_internal.cuh"
 
 #define SORT_BLOCK 256
+static_assert(GM_SCAN_ITEMS == 4, "the scan kernels move one int4 per thread");
 
 // Decide whether the rebuild runs at this time level and publish the decision (every later kernel of
 // the chain only reads ctl->go).  With a conditional graph node the body is skipped altogether.
@@ -127,10 +128,14 @@ k_scan_local(const __grid_constant__ GmParams P, GmDev D)
 #pragma unroll
     for (int q = 0; q < GM_SCAN_ITEMS; ++q) s += v[q];
     int off = block_exclusive_scan(s, &total);
+    if (base + GM_SCAN_ITEMS <= n) {          // one 16-byte store per thread (cstart is 256-byte aligned)
+        *reinterpret_cast<int4 *>(D.cstart + base) = make_int4(off, off + v[0], off + v[0] + v[1], off + v[0] + v[1] + v[2]);
+    } else {
 #pragma unroll
-    for (int q = 0; q < GM_SCAN_ITEMS; ++q) {
-        if (base + q < n) D.cstart[base + q] = off;
-        off += v[q];
+        for (int q = 0; q < GM_SCAN_ITEMS; ++q) {
+            if (base + q < n) D.cstart[base + q] = off;
+            off += v[q];
+        }
     }
     if (threadIdx.x == 0) D.scan_sums[blockIdx.x] = total;
 }
@@ -158,9 +163,15 @@ k_scan_add(const __grid_constant__ GmParams P, GmDev D)
     const int add = add_sh;
     const int n = P.n_cells + 1;
     const int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
+    if (base + GM_SCAN_ITEMS <= n) {
+        int4 c = *reinterpret_cast<const int4 *>(D.cstart + base);
+        c.x += add; c.y += add; c.z += add; c.w += add;
+        *reinterpret_cast<int4 *>(D.cstart + base) = c;
+    } else {
 #pragma unroll
-    for (int q = 0; q < GM_SCAN_ITEMS; ++q)
-        if (base + q < n) D.cstart[base + q] += add;
+        for (int q = 0; q < GM_SCAN_ITEMS; ++q)
+            if (base + q < n) D.cstart[base + q] += add;
+    }
 }
 
 __global__ void __launch_bounds__(SORT_BLOCK)
