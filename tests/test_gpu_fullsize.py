@@ -5,7 +5,7 @@
     per-bead forces and the 10-step trajectory against the fp64 cell-list oracle on ALL beads (the
     oracle's O(N) mode finishes a step of C3 in about 0.1 s; its agreement with the O(N^2) definition is
     pinned in tests/test_oracle_pins.py).
-  * configs[3] ("C4", 3,000,000-bead DPD melt) and configs[4] ("C5", 8,000,000-bead LJ 2.5 melt) at full size:
+  * configs[1] ("C2", 64,000 beads, Langevin), configs[3] ("C4", 3,000,000-bead DPD melt) and configs[4] ("C5", 8,000,000-bead LJ 2.5 melt) at full size:
     forces on all beads, energies, and a few steps of trajectory.
   * Long runs (north_star: "energy drift and <Rg^2>/bond-length statistics must agree within a stated
     1 %"): C1 for its full 1,000 NVE steps, a scaled C2 under the Langevin
@@ -139,6 +139,11 @@ def _full_size_forces_and_steps(gm, name, n_steps):
     st = s.stats()
     assert st["dev_err"] == 0 and st["max_nn"] <= st["nl_row_capacity"]
     s.close()
+
+
+def test_c2_full_64k_bead_lj25_langevin_forces_and_steps(gm):
+    # configs[1]: 64,000 beads, LJ r_c = 2.5 + FENE, Langevin thermostat (drag + Philox per-bead noise)
+    _full_size_forces_and_steps(gm, "C2", 10)
 
 
 def test_c4_full_3m_bead_dpd_forces_and_steps(gm):
