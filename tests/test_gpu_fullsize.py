@@ -195,6 +195,18 @@ def test_c1_full_1000_steps_nve_statistics(gm):
     assert np.abs(g[:, 0] - o[:, 0]).max() <= 0.01 * o[:, 1].mean()
 
 
+def test_c3_full_200_steps_nve_statistics(gm, c3):
+    # shortened oracle run at full size.  10,000 chains of 100: the run averages carry standard
+    # errors far below the 1 % bar; 200 steps span ~25 rebuilds (each one a full SFC sort of every array).
+    g, o = _long_run(gm, c3, 200, 50)
+    assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)      # mean bond length
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)      # <Rg^2>
+    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)      # temperature
+    for r in (g, o):                                                      # NVE drift against the kinetic energy
+        assert np.abs(r[:, 0] - r[0, 0]).max() <= 0.01 * r[:, 1].mean()
+    assert np.abs(g[:, 0] - o[:, 0]).max() <= 0.01 * o[:, 1].mean()
+
+
 def test_c2_scaled_langevin_temperature_statistics(gm):
     w = make_config("C2", scale=0.4)          # 16^3 lattice, 4096 beads, LJ 2.5 + Langevin (same noise keys)
     g, o = _long_run(gm, w, 600, 100)
