@@ -112,7 +112,8 @@ static gm_status derive(const gm_config *c, GmParams *P)
     }
     {
         const double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
-        P->step_wide = nbar >= 40.0 ? 1 : 0;       // measured: C1/C3 (13) narrow, C2/C5 (78) wide
+        // measured: C1/C3 (n_l 13) narrow; C5 (78, 8M beads) wide; C2 (78, 64k beads: less than one wave) narrow
+        P->step_wide = (nbar >= 40.0 && P->n > 262144) ? 1 : 0;
         if (const char *e = getenv("GM_STEP_WIDE")) P->step_wide = atoi(e) != 0;
     }
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
