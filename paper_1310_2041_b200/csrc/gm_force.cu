@@ -554,13 +554,16 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
     }
 }
 
-__global__ void k_energy_final(GmDev D, int n_blocks)
+// Second stage: warp q sums quantity q over the block partials -- lane l takes blocks l, l + 32, ... in
+// order, then a fixed xor-shuffle tree: the order of the additions depends on nothing but n_blocks.
+__global__ void __launch_bounds__(7 * 32) k_energy_final(GmDev D, int n_blocks)
 {
-    if (threadIdx.x < 7) {
-        double v = 0.0;
-        for (int b = 0; b < n_blocks; ++b) v += D.esum[(size_t)b * 8 + threadIdx.x];
-        D.esum[(size_t)GM_ESUM_BLOCKS * 8 + threadIdx.x] = v;
-    }
+    const int q = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    double v = 0.0;
+    for (int b = lane; b < n_blocks; b += 32) v += D.esum[(size_t)b * 8 + q];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane == 0) D.esum[(size_t)GM_ESUM_BLOCKS * 8 + q] = v;
 }
 
 template <int PAIR, bool NT1, int BOND>
@@ -584,7 +587,7 @@ static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int pari
     else {
         int g = nb < GM_ESUM_BLOCKS ? nb : GM_ESUM_BLOCKS;
         k_energy<PAIR, NT1, BOND><<<g, FORCE_BLOCK, 0, st>>>(P, D, parity, lagged);
-        k_energy_final<<<1, 32, 0, st>>>(D, g);
+        k_energy_final<<<1, 7 * 32, 0, st>>>(D, g);
     }
 }
 
