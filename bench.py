@@ -283,10 +283,13 @@ def main():
             "whole_step": {"algorithmic_bytes_per_timestep": bytes_step, "achieved": bytes_step / (ms_ts * 1e-3) / 1e9,
                            "frac": bytes_step / (ms_ts * 1e-3) / 1e9 / hbm_gbs,
                            "frac_of_nominal_8TBs": bytes_step / (ms_ts * 1e-3) / 1e9 / 8000.0}}
-    tr = os.path.join(ROOT, "profiles", "traffic_r01.json")     # dram bytes/launch from the ncu --set full capture
+    tr = os.path.join(ROOT, "profiles", "traffic_r01.csv")      # dram bytes/launch of k_step from the ncu capture
     if os.path.exists(tr):
+        import csv
         with open(tr) as f:
-            roof["traffic"] = json.load(f).get(args.config)
+            for row in csv.DictReader(f):
+                if row["config"] == args.config:
+                    roof["traffic"] = float(row["dram_bytes_per_launch"])
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------------
     e2e = None
