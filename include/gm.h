@@ -51,7 +51,9 @@ enum {
     GM_ERR_STATE = -2,               /* call order: e.g. gm_step before gm_set_particles          */
     GM_ERR_CUDA = -3,                /* a CUDA runtime call failed; message has the CUDA string   */
     GM_ERR_WORKSPACE_TOO_SMALL = -4,
-    GM_ERR_BOX_TOO_SMALL = -5,       /* box_d < 3 (r_cut_max + r_skin) in some dimension (27-cell search) */
+    GM_ERR_BOX_TOO_SMALL = -5,       /* box_d < 3.0003 (r_cut_max + r_skin) in some dimension (27-cell search with a
+                                        1e-4 margin for the fp32 cell assignment), or r_cut_max + 2 r_skin >= box_d / 2
+                                        (one minimum-image test per listed pair) */
     GM_ERR_NEIGHBOR_OVERFLOW = -6,   /* a bead has more neighbors than nl_row_capacity            */
     GM_ERR_BOND_OVERSTRETCH = -7,    /* FENE bond with r >= R0                                    */
     GM_ERR_NONFINITE = -8            /* a coordinate became NaN/Inf                               */
@@ -69,7 +71,7 @@ typedef struct {
     uint32_t struct_size;
     int32_t device;                  /* CUDA device ordinal                                        */
     void *stream;                    /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy default */
-    int64_t n_particles;             /* N >= 1, < 2^31                                             */
+    int64_t n_particles;             /* N >= 1, < 2^28 (bond rows pack the partner index in 28 bits) */
     int32_t n_types;                 /* 1..GM_MAX_TYPES                                            */
     int32_t max_bonds_per_particle;  /* rows of the BL table (Fig. 2); 0 = no bonds  */
     float box[3];                    /* cuboid edge lengths                                        */
@@ -85,7 +87,11 @@ typedef struct {
                                         neighbor rebuild sorts; > 0 forces a rebuild after this many steps) */
     int32_t nl_row_capacity;         /* rows of the NL table; 0 = choose from density              */
     int32_t flags;                   /* GM_FLAG_*                                                  */
-    int32_t reserved;
+    /* Tuning overrides, 0 = choose from the geometry.  They never change results (exact accelerations). */
+    int32_t x_cell_div;              /* 1..8: cells are (r_cut_max + r_skin) / x_cell_div wide in x (DESIGN.md c-12)  */
+    int32_t nl_scan_trip;            /* 4 or 8: candidates the neighbor search loads together                         */
+    int32_t step_shape;              /* 1: one-warp CTAs (short lists), 2: CTAs of 128 (long lists)                    */
+    int32_t reserved;                /* must be 0                                                                      */
 } gm_config;
 
 enum {

@@ -41,9 +41,11 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if p.returncode != 0:
             sys.stderr.write(out)
             raise RuntimeError(f"nvcc failed on {src}")
-    # resource usage of every kernel (registers, spills, shared memory); compile times dropped so that the
-    # file only changes when the code does
-    with open(os.path.join(CSRC, "ptxas.log"), "w") as f:
+    # resource usage of every kernel (registers, spills, shared memory): a build log, kept out of the tree's
+    # history (_work/ is git-ignored)
+    logdir = os.path.join(os.path.dirname(HERE), "_work")
+    os.makedirs(logdir, exist_ok=True)
+    with open(os.path.join(logdir, "ptxas.log"), "w") as f:
         f.write("\n".join(l for out in log for l in out.splitlines() if "Compile time" not in l) + "\n")
     if verbose:
         print("\n".join(log))

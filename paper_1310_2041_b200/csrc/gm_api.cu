@@ -55,6 +55,9 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (c->integrator < GM_NVE || c->integrator > GM_DPD_GWVV) return GM_ERR_INVALID_ARG;
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
+    if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
+        c->step_shape < 0 || c->step_shape > 2 || c->reserved != 0)
+        return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
     P->ns = (P->n + 8 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+7 (at least): far-away pad beads
     P->sfc_period = c->sfc_period;
@@ -68,6 +71,9 @@ static gm_status derive(const gm_config *c, GmParams *P)
         // cell width >= r_list with a 1e-4 relative margin for the fp32 cell assignment (reading c-12)
         P->nc[d] = (int)std::floor((double)c->box[d] / (r_list * 1.0001));
         if (P->nc[d] < 3) return GM_ERR_BOX_TOO_SMALL;
+        // one |a - b| > L/2 test per listed pair (gm_min_image_signed) and the plain differences of the search
+        // pick the right image only while r_list + r_skin < L/2 (a listed pair drifts by at most r_skin)
+        if (!(r_list + (double)c->r_skin < 0.5 * (double)c->box[d])) return GM_ERR_BOX_TOO_SMALL;
         if (P->nc[d] > 1024) P->nc[d] = 1024;
         vol *= c->box[d];
     }
@@ -76,11 +82,11 @@ static gm_status derive(const gm_config *c, GmParams *P)
     {
         const double per_cell = (double)P->n / ((double)P->nc[0] * P->nc[1] * P->nc[2]);
         int sx = per_cell >= 6.0 ? 4 : (per_cell >= 2.0 ? 3 : (per_cell >= 1.0 ? 2 : 1));   // measured: C3 3, C2/C4/C5 4
-        if (const char *e = getenv("GM_XDIV")) sx = std::max(1, std::min(8, atoi(e)));
+        if (c->x_cell_div > 0) sx = c->x_cell_div;
         P->sx = sx;
         // mean candidates per run of a (y, z) row: (2 sx + 1) cells of per_cell / sx beads
         P->nl_trip = per_cell * (2.0 * sx + 1.0) / sx >= 16.0 ? 8 : 4;
-        if (const char *e = getenv("GM_NLTRIP")) P->nl_trip = atoi(e) == 8 ? 8 : 4;
+        if (c->nl_scan_trip > 0) P->nl_trip = c->nl_scan_trip;
         if (sx > 1) {
             P->nc[0] = (int)std::floor((double)c->box[0] * sx / (r_list * 1.0001));
             if (P->nc[0] > 4096) { P->sx = 1; P->nc[0] = 1024; }
@@ -114,7 +120,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
         const double nbar = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
         // measured: C1/C3 (n_l 13) narrow; C5 (78, 8M beads) wide; C2 (78, 64k beads: less than one wave) narrow
         P->step_wide = (nbar >= 40.0 && P->n > 262144) ? 1 : 0;
-        if (const char *e = getenv("GM_STEP_WIDE")) P->step_wide = atoi(e) != 0;
+        if (c->step_shape > 0) P->step_wide = c->step_shape == 2;
     }
     if ((long long)cap > (long long)P->n) cap = std::max(1, P->n - 1 + (P->n == 1));
     cap = (cap + 7) / 8 * 8;
@@ -267,7 +273,6 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     cudaError_t e = cudaSetDevice(cfg->device);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st2, cudaStreamNonBlocking);
-    if (e == cudaSuccess) e = gm_nl_prepare(P);
     if (e == cudaSuccess) {
         std::vector<uint32_t> rr;
         sfc_row_order(P.nc[1], P.nc[2], rr);
@@ -376,10 +381,11 @@ extern "C" gm_status gm_set_particles(gm_system *s, const float *pos3, const flo
         CU(cudaMemcpyAsync(st + 9 * n, type, n * 4, cudaMemcpyHostToDevice, s->st));
         if (mass) CU(cudaMemcpyAsync(st + 10 * n, mass, n * 4, cudaMemcpyHostToDevice, s->st));
         dp = st; dv = st + 3 * n; dt = (const int *)(st + 9 * n); dm = mass ? st + 10 * n : nullptr;
+        CU(cudaStreamSynchronize(s->st));      // "copies inputs in": the caller may reuse (pinned) buffers at once
     }
     s->cur = 0;
+    gm_launch_set_ctl(s->D, 0, 1, 0, s->st);             // clears the latched device errors: before the pack
     gm_launch_pack(s->P, s->D, 0, dp, dv, dt, dm, s->st);
-    gm_launch_set_ctl(s->D, 0, 1, 0, s->st);
     CU(cudaGetLastError());
     s->step = 0;
     s->have_particles = true;
@@ -672,6 +678,7 @@ extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, f
 // ---- results ----------------------------------------------------------------------------------------
 static gm_status dev_error(gm_system *s, const GmCtl &c)
 {
+    if (c.err & GM_DEV_ERR_BAD_INPUT) return fail(s, GM_ERR_INVALID_ARG, "gm_set_particles: a type outside [0, n_types) or a mass <= 0%s");
     if (c.err & GM_DEV_ERR_NONFINITE) return fail(s, GM_ERR_NONFINITE, "a coordinate became non-finite%s");
     if (c.err & GM_DEV_ERR_OVERSTRETCH) return fail(s, GM_ERR_BOND_OVERSTRETCH, "a FENE bond reached r >= R0%s");
     if (c.err & GM_DEV_ERR_OVERFLOW) return fail(s, GM_ERR_NEIGHBOR_OVERFLOW, "a neighbor row exceeded nl_row_capacity%s");
@@ -739,27 +746,33 @@ extern "C" gm_status gm_get_neighbors(gm_system *s, int32_t *nn, int32_t *nl_tag
     if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_get_neighbors: no particles set%s");
     if (!nn || !nl_tags || row_stride < 1) return fail(s, GM_ERR_INVALID_ARG, "gm_get_neighbors: bad arguments%s");
     CU(cudaSetDevice(s->cfg.device));
-    if (!s->nl_valid) { gm_status r = ensure_list(s); if (r != GM_OK) return r; }
+    {   // gated rebuild: a no-op when the list is current at this time level (a4)
+        gm_status r = ensure_list(s);
+        if (r != GM_OK) return r;
+    }
     GmCtl c;
     gm_status r = sync_and_check(s, &c);
     if (r != GM_OK) return r;
     if (row_stride < c.max_nn) return fail(s, GM_ERR_INVALID_ARG, "gm_get_neighbors: row_stride < max nn%s");
-    const size_t n = (size_t)s->P.n;
+    const int n = s->P.n;
     if (on_device) {
-        gm_launch_unpack_neighbors(s->P, s->D, nn, nl_tags, row_stride, s->st);
+        gm_launch_unpack_neighbors(s->P, s->D, nn, nl_tags, row_stride, 0, n, s->st);
         CU(cudaGetLastError());
         return GM_OK;
     }
-    // validation path: a temporary device image of the tag-space table
-    int *tmp = nullptr;
-    CU(cudaMalloc(&tmp, n * 4 * (size_t)(row_stride + 1)));
-    gm_launch_unpack_neighbors(s->P, s->D, tmp, tmp + n, row_stride, s->st);
-    cudaError_t e = cudaGetLastError();
-    if (e == cudaSuccess) e = cudaMemcpyAsync(nn, tmp, n * 4, cudaMemcpyDeviceToHost, s->st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(nl_tags, tmp + n, n * 4 * (size_t)row_stride, cudaMemcpyDeviceToHost, s->st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
-    cudaFree(tmp);
-    if (e != cudaSuccess) return fail(s, GM_ERR_CUDA, "CUDA: %s", cudaGetErrorString(e));
+    // host output: tag ranges that fit the I/O staging area of the workspace (11 ns floats), one range at a time
+    int *st = reinterpret_cast<int *>(s->D.stage);
+    const long long rows_fit = (long long)((size_t)s->P.ns * 11 / (size_t)(row_stride + 1));
+    if (rows_fit < 1) return fail(s, GM_ERR_INVALID_ARG, "gm_get_neighbors: row_stride too large for the staging area%s");
+    for (long long t0 = 0; t0 < n; t0 += rows_fit) {
+        const int t1 = (int)std::min<long long>(n, t0 + rows_fit);
+        const size_t m = (size_t)(t1 - t0);
+        gm_launch_unpack_neighbors(s->P, s->D, st, st + m, row_stride, (int)t0, t1, s->st);
+        CU(cudaGetLastError());
+        CU(cudaMemcpyAsync(nn + t0, st, m * 4, cudaMemcpyDeviceToHost, s->st));
+        CU(cudaMemcpyAsync(nl_tags + t0 * row_stride, st + m, m * 4 * (size_t)row_stride, cudaMemcpyDeviceToHost, s->st));
+        CU(cudaStreamSynchronize(s->st));
+    }
     return GM_OK;
 }
 

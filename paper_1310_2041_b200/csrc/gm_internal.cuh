@@ -35,7 +35,7 @@
 #define GM_NEVER (~0ull)
 
 // latched device error bits (GmCtl::err)
-enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE = 4 };
+enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE = 4, GM_DEV_ERR_BAD_INPUT = 8 };
 
 // Small device control block (one per system).
 struct GmCtl {
@@ -113,7 +113,6 @@ void gm_launch_gate(const GmDev &D, int gate, int parity, unsigned long long con
                     cudaStream_t st);                                                  // decides, publishes ctl->go
 void gm_launch_sort(const GmParams &P, const GmDev &D, int parity, cudaStream_t st);    // a1 + a2 (if ctl->go)
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st);            // a3      (if ctl->go)
-cudaError_t gm_nl_prepare(const GmParams &P);
 int gm_nl_capacity_ok(const GmParams &P);
 void gm_launch_bonds_from_master(const GmParams &P, const GmDev &D, cudaStream_t st);
 void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
@@ -123,7 +122,7 @@ void gm_launch_pack(const GmParams &P, const GmDev &D, int cur, const float *pos
 void gm_launch_unpack(const GmParams &P, const GmDev &D, int cur, float *pos3, float *vel3, float *force3,
                       int lagged, cudaStream_t st);
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,
-                                cudaStream_t st);
+                                int t0, int t1, cudaStream_t st);
 void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, int parity, cudaStream_t st);
 void gm_launch_init_pad(const GmParams &P, const GmDev &D, cudaStream_t st);
 

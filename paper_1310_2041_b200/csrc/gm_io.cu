@@ -20,9 +20,18 @@ k_pack(const __grid_constant__ GmParams P, GmDev D, int cur, const float *__rest
     float x = wrap_any(pos3[3 * i + 0], P.half[0], P.box[0]);
     float y = wrap_any(pos3[3 * i + 1], P.half[1], P.box[1]);
     float z = wrap_any(pos3[3 * i + 2], P.half[2], P.box[2]);
-    D.pos[cur][i] = make_float4(x, y, z, __int_as_float(type[i]));
+    // a type outside [0, n_types) would index the pair table out of bounds, a mass <= 0 has no acceleration:
+    // latched, reported as GM_ERR_INVALID_ARG by the next synchronising call; the bead is stored as type 0, mass 1
+    int ty = type[i];
+    float m = mass ? mass[i] : 1.0f;
+    if (ty < 0 || ty >= P.n_types || !(m > 0.0f) || !isfinite(m)) {
+        atomicOr(&D.ctl->err, GM_DEV_ERR_BAD_INPUT);
+        ty = (ty < 0 || ty >= P.n_types) ? 0 : ty;
+        m = (m > 0.0f && isfinite(m)) ? m : 1.0f;
+    }
+    D.pos[cur][i] = make_float4(x, y, z, __int_as_float(ty));
     float vx = vel3[3 * i + 0], vy = vel3[3 * i + 1], vz = vel3[3 * i + 2];
-    D.vel[i] = make_float4(vx, vy, vz, mass ? mass[i] : 1.0f);
+    D.vel[i] = make_float4(vx, vy, vz, m);
     if (D.vt[0]) D.vt[cur][i] = make_float4(vx, vy, vz, __int_as_float(i));
     D.tag[0][i] = i;            // k_set_ctl(reset_all) selects buffer 0
     D.rtag[i] = i;

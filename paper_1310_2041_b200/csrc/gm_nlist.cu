@@ -215,8 +215,6 @@ k_bl_remap(const __grid_constant__ GmParams P, GmDev D)
 
 int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 4 == 0; }
 
-cudaError_t gm_nl_prepare(const GmParams &P) { (void)P; return cudaSuccess; }
-
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     const int threads = NL_WARPS * 32;
@@ -226,24 +224,26 @@ void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
     else k_nl_build<4><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
 }
 
-// Neighbor list in tag space for the boundary (gm_get_neighbors): nn_out[tag], nl_out[tag*stride + k].
+// Neighbor list in tag space for the boundary (gm_get_neighbors), tags [t0, t1): nn_out[tag - t0],
+// nl_out[(tag - t0) * stride + k].  One thread per tag.
 __global__ void __launch_bounds__(256)
 k_unpack_neighbors(const __grid_constant__ GmParams P, GmDev D, int *__restrict__ nn_out,
-                   int *__restrict__ nl_out, long long stride)
+                   int *__restrict__ nl_out, long long stride, int t0, int t1)
 {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= P.n) return;
+    const int t = t0 + blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= t1) return;
     const int *__restrict__ tag = D.tag[D.ctl->n_rebuilds & 1ull];
-    const int t = tag[i];
+    const int i = D.rtag[t];
     const int nn = D.nn[i];
-    nn_out[t] = nn;
+    nn_out[t - t0] = nn;
     const int *__restrict__ tile = reinterpret_cast<const int *>(D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31));
     for (int k = 0; k < nn && k < stride; ++k)
-        nl_out[(long long)t * stride + k] = tag[tile[(k >> 2) * 128 + (k & 3)]];
+        nl_out[(long long)(t - t0) * stride + k] = tag[tile[(k >> 2) * 128 + (k & 3)]];
 }
 
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,
-                                cudaStream_t st)
+                                int t0, int t1, cudaStream_t st)
 {
-    k_unpack_neighbors<<<(P.n + 255) / 256, 256, 0, st>>>(P, D, nn_out, nl_out, stride);
+    if (t1 <= t0) return;
+    k_unpack_neighbors<<<(t1 - t0 + 255) / 256, 256, 0, st>>>(P, D, nn_out, nl_out, stride, t0, t1);
 }

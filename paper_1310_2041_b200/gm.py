@@ -39,6 +39,7 @@ class gm_config(C.Structure):
         ("pair_style", C.c_int32), ("bond_style", C.c_int32), ("integrator", C.c_int32),
         ("kT", C.c_float), ("gamma", C.c_float), ("lam", C.c_float),
         ("sfc_period", C.c_int32), ("nl_row_capacity", C.c_int32), ("flags", C.c_int32),
+        ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
         ("reserved", C.c_int32),
     ]
 
@@ -217,7 +218,7 @@ class System:
     """
 
     def __init__(self, w, device: int = 0, flags: int = 0, nl_row_capacity: int = 0, sfc_period=None,
-                 load: bool = True):
+                 load: bool = True, tune: dict | None = None):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1310_2041_b200 needs a CUDA device (there is no CPU fallback)")
@@ -251,6 +252,8 @@ class System:
         cfg.sfc_period = int(w.sfc_period if sfc_period is None else sfc_period)
         cfg.nl_row_capacity = int(nl_row_capacity)
         cfg.flags = int(flags)
+        for k, v in (tune or {}).items():       # gm_config tuning overrides: x_cell_div, nl_scan_trip, step_shape
+            setattr(cfg, k, int(v))
         self.cfg = cfg
         nbytes = gm_query_workspace(cfg)
         self.workspace_bytes = nbytes

@@ -40,8 +40,8 @@ def gpu_pair_set(nn, nl):
     return out
 
 
-def check_neighbor_sets(gm, w, use_cells=True):
-    s = gm.System(w)
+def check_neighbor_sets(gm, w, use_cells=True, tune=None):
+    s = gm.System(w, tune=tune)
     s.build_neighbors()
     nn, nl = s.neighbors()
     st = s.stats()
@@ -90,8 +90,8 @@ def test_neighbor_sets_noncubic_random_with_beads_on_faces(gm):
     check_neighbor_sets(gm, w, use_cells=False)
 
 
-def forces_parity(gm, w, steps_before=0, tol=1e-4):
-    s = gm.System(w)
+def forces_parity(gm, w, steps_before=0, tol=1e-4, tune=None):
+    s = gm.System(w, tune=tune)
     o = orc.Oracle(w)
     if steps_before:
         s.step(steps_before)
@@ -116,17 +116,16 @@ def forces_parity(gm, w, steps_before=0, tol=1e-4):
 
 
 @pytest.mark.parametrize("xdiv,trip", [(1, 4), (2, 8), (3, 4), (4, 8), (8, 4)])
-def test_cell_refinement_and_scan_width_do_not_change_the_list_or_the_forces(gm, monkeypatch, xdiv, trip):
+def test_cell_refinement_and_scan_width_do_not_change_the_list_or_the_forces(gm, xdiv, trip):
     # a3: cells r_list / sx wide in x and 4 or 8 candidates per trip are exact accelerations (DESIGN.md c-12);
-    # the overrides are read by gm_create.  Non-cubic box with beads on the faces, then C1 forces.
-    monkeypatch.setenv("GM_XDIV", str(xdiv))
-    monkeypatch.setenv("GM_NLTRIP", str(trip))
+    # the overrides are gm_config fields.  Non-cubic box with beads on the faces, then C1 forces.
+    tune = dict(x_cell_div=xdiv, nl_scan_trip=trip)
     w = make_random_box(3000, [9.0, 13.5, 17.25], seed=6)
     w.pos[:50, 0] = -4.5                                       # exactly on the lower face
     w.pos[50:100, 1] = np.nextafter(np.float32(6.75), np.float32(0))   # last value below the upper face
     w.pos[100:120] = w.pos[120:140]                            # coincident beads
-    check_neighbor_sets(gm, w, use_cells=False)
-    forces_parity(gm, make_config("C1"), steps_before=12)
+    check_neighbor_sets(gm, w, use_cells=False, tune=tune)
+    forces_parity(gm, make_config("C1"), steps_before=12, tune=tune)
 
 
 def test_forces_dense_dpd_exercises_the_early_drain_of_the_compaction_column(gm):
