@@ -399,3 +399,108 @@ def test_dpd_temperature_and_momentum():
         Ts.append(o.temperature())
     assert np.abs(o.momentum() - p0).max() < 1e-9         # pairwise noise conserves momentum exactly
     assert np.mean(Ts) == pytest.approx(1.0, rel=0.06)    # GW-VV at dt = 0.04, lambda = 0.65
+
+
+def test_dpd_temperature_long_average():
+    """Fluctuation-dissipation through <T> (sigma_R^2 = 2 gamma kT, reading c-3) on a longer average: 2,058 beads,
+    220 readings over 2,200 steps after a 300-step transient.  One reading of N beads scatters by sqrt(2/3N) = 1.8 %;
+    readings 10 steps apart are nearly independent (DPD velocity correlations die within ~0.3 tau = 8 steps), so the mean
+    is good to ~0.15 %; the integrator's own offset at dt = 0.04, lambda = 0.65 stays below 1 %, so the window is
+    1.5 % (was 6 %): a wrong noise amplitude (sigma_R^2 = gamma kT or 4 gamma kT) gives 0.5 or 2.0, a missing 1/sqrt(dt)
+    gives 0.04, uniform noise without the sqrt(3) gives 1/3."""
+    w = make_config("C4", scale=0.0882)                   # 8.82^3 box: 205 chains, 2,050 beads, rho = 3
+    o = orc.Oracle(w, n_threads=4)
+    o.compute_forces()
+    o.run(300)
+    Ts = []
+    for _ in range(220):
+        o.run(10)
+        Ts.append(o.temperature())
+    T = float(np.mean(Ts))
+    assert T == pytest.approx(1.0, rel=0.015), T
+
+
+# ---- GW-VV predictor/corrector (reading c-6; PAPER.md:L135) ------------------------------------------
+def _dpd_conservative(seed, dt, integrator):
+    """Soft-sphere fluid with the DPD conservative force only (gamma = 0, kT = 0): Hamiltonian."""
+    w = make_random_box(600, (6.0, 6.0, 6.0), seed=seed, kT=1.0)
+    w.pair_style = "dpd"; w.pair = dict(a=np.full((1, 1), 25.0, np.float32), rc=np.ones((1, 1), np.float32))
+    w.integrator = integrator; w.gamma = 0.0; w.kT = 0.0; w.lam = 0.65; w.dt = dt
+    o = orc.Oracle(w, use_cells=False)
+    o.P.dt = dt                                           # exact fp64 time step
+    return o
+
+
+def test_gwvv_without_thermostat_is_velocity_verlet():
+    """With gamma = 0 the force does not see v~, and GW-VV (r += dt v + dt^2/2 f; v += dt/2 (f + f')) IS velocity
+    Verlet: the ORC_GWVV branch of orc_run must reproduce the ORC_NVE branch (pinned by P2, P5, P6) to fp64
+    round-off.  A missing dt^2/2 f drift, v += dt f' or a corrector without the old force all break this."""
+    a = _dpd_conservative(31, 0.01, "nve")
+    b = _dpd_conservative(31, 0.01, "gwvv")
+    a.compute_forces(); b.compute_forces()
+    a.run(200); b.run(200)
+    d = a.pos - b.pos; d -= a.box * np.rint(d / a.box)
+    # round-off (1e-16) grows along the chaotic trajectory to ~3e-10 by t = 2; a wrong scheme differs by O(dt^2) = 1e-4
+    assert np.abs(d).max() < 1e-8 and np.abs(a.vel - b.vel).max() < 1e-8
+    assert np.abs(a.vel).max() > 0.5                      # the run did move
+
+
+def test_gwvv_energy_error_is_second_order():
+    """Same Hamiltonian system through the GW-VV branch: halving dt quarters the energy error."""
+    def rms(dt, n):
+        o = _dpd_conservative(32, dt, "gwvv")
+        o.compute_forces()
+        es = []
+        for _ in range(n):
+            o.run(1)
+            es.append(o.kinetic() + o.potential()[0])
+        es = np.array(es)
+        return float(np.sqrt(np.mean((es - es.mean()) ** 2)))
+    e1, e2 = rms(0.02, 100), rms(0.01, 200)
+    assert 3.0 < e1 / e2 < 5.0, (e1, e2)
+
+
+def test_gwvv_two_bead_step_depends_on_lambda(golden):
+    """tests/golden/closed_forms.txt: one GW-VV step of two approaching beads under the dissipative force alone,
+    worked by hand for lambda = 0.65.  Pins v~ = v + lambda dt f (lambda = 0.5 gives f' = -1.2448 instead of
+    -1.2272), the dt^2/2 f drift and the dt/2 (f + f') corrector."""
+    g = G(golden)
+
+    def one_step(lam):
+        w = custom([[-0.25, 0, 0], [0.25, 0, 0]], 20.0, vel=[[0.5, 0, 0], [-0.5, 0, 0]], pair_style="dpd", a=0.0,
+                   rc=1.0, integrator="gwvv", dt=0.04, kT=0.0, gamma=4.5, lam=lam)
+        o = orc.Oracle(w, use_cells=False)
+        o.P.dt = 0.04; o.P.lam = lam                      # exact fp64 parameters (the workload carries fp32)
+        o.compute_forces()
+        assert o.frc[0, 0] == pytest.approx(-1.125, abs=1e-14) and o.frc[1, 0] == pytest.approx(1.125, abs=1e-14)
+        o.run(1)
+        return o
+    o = one_step(0.65)
+    assert o.frc[0, 0] == pytest.approx(g["gwvv_two_bead_f1"], abs=1e-11)
+    assert o.frc[1, 0] == pytest.approx(-g["gwvv_two_bead_f1"], abs=1e-11)
+    assert o.vel[0, 0] == pytest.approx(g["gwvv_two_bead_v1"], abs=1e-12)
+    assert o.vel[1, 0] == pytest.approx(-g["gwvv_two_bead_v1"], abs=1e-12)
+    assert o.pos[0, 0] == pytest.approx(g["gwvv_two_bead_x1"], abs=1e-14)
+    assert np.abs(o.pos[:, 1:]).max() == 0.0 and np.abs(o.vel[:, 1:]).max() == 0.0
+    o = one_step(0.5)                                     # the pin must tell lambda = 0.5 from 0.65
+    assert abs(o.frc[0, 0] - g["gwvv_two_bead_f1"]) > 1e-2
+    assert abs(o.vel[0, 0] - g["gwvv_two_bead_v1"]) > 1e-4
+
+
+# ---- O8 observables ---------------------------------------------------------------------------------
+def test_rod_radius_of_gyration_and_bond_lengths(golden):
+    """chain_rg2 / bond_lengths on straight rods that cross the periodic faces: Rg^2 = (n^2 - 1) a^2 / 12."""
+    g = G(golden)
+    n, a, box = 10, 0.9, np.array([5.0, 6.0, 7.0])
+    rng = np.random.default_rng(3)
+    pos = []
+    for _ in range(7):                                    # 7 rods, random origins and directions
+        e = rng.normal(size=3); e /= np.linalg.norm(e)
+        r0 = rng.uniform(-0.5, 0.5, 3) * box
+        pos.append(r0 + a * np.arange(n)[:, None] * e)
+    pos = np.concatenate(pos)
+    pos -= box * np.floor(pos / box + 0.5)                # wrapped into the box: the rods are cut by the faces
+    rg2 = orc.chain_rg2(pos, box, n)
+    assert rg2.shape == (7,) and np.allclose(rg2, g["rod_rg2_n10_a0p9"], rtol=1e-12)
+    bonds = np.array([[c * n + k, c * n + k + 1] for c in range(7) for k in range(n - 1)])
+    assert np.allclose(orc.bond_lengths(pos, box, bonds), a, rtol=1e-12)
