@@ -216,19 +216,119 @@ def test_c2_scaled_langevin_temperature_statistics(gm):
 
 
 def test_c4_scaled_dpd_temperature_statistics(gm):
-    w = make_config("C4", scale=0.1)          # 10^3 box, 3000 beads, DPD + GW-VV (same pair-noise keys)
+    w = make_config("C4", scale=0.3)          # 30^3 box, 81,000 beads = 8,100 chains, DPD + GW-VV (same pair-noise keys)
     # fp32 and fp64 trajectories decorrelate after ~50 steps, so the two runs are independent samples of the
-    # same ensemble: one temperature reading of 3000 beads scatters by sqrt(2 / 3N) = 1.5 %.  The 1 % bar is
-    # put on run averages whose standard error is well below it: 120 readings, 10 steps apart, after the
-    # first 300 steps (the random-walk start relaxes from T = 1.39).
+    # same ensemble.  The 1 % bar is put on run averages whose standard error is well below it: 120 readings, 10
+    # steps apart, after the first 300 steps (the random-walk start relaxes from T = 1.39).  One temperature reading
+    # of 81,000 beads scatters by sqrt(2 / 3N) = 0.3 %; one <Rg^2> reading of 8,100 ten-bead chains by ~0.5 %
+    # (relative spread of a chain's Rg^2 ~ 0.5), the run average over ~5 chain relaxation times by ~0.25 %.
     g, o = _long_run(gm, w, 1500, 10)
     g, o = g[30:], o[30:]
-    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)
+    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)      # temperature
+    assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)      # mean bond length
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)      # <Rg^2>, plain 1 %
+
+
+# ---- full size, full length (north_star: "Over long runs, energy drift and <Rg^2>/bond-length statistics must
+#      agree within a stated 1 %"; SURVEY.md 8(c) gates (i)-(iii)) ------------------------------------------------
+def _gpu_drift(s, w, n_steps, every):
+    """|E(t) - E(0)| / N against the mean kinetic energy per bead, GPU only, sampled every `every` steps."""
+    e0 = s.energies()["etot"] / w.n
+    de, ke = [], []
+    for _ in range(n_steps // every):
+        s.step(every)
+        e = s.energies()
+        de.append(e["etot"] / w.n - e0)
+        ke.append(e["ke"] / w.n)
+    assert s.stats()["dev_err"] == 0
+    return np.abs(np.array(de)).max(), float(np.mean(ke))
+
+
+def test_c3_full_length_10000_steps_nve_drift(gm, c3):
+    # exactly what bench.py times: 1,000 Langevin steps of equilibration, then the config's 10,000 NVE steps
+    # (~1,280 rebuilds, each a full SFC sort); energy sampled every 500 steps
+    import copy
+    w = copy.copy(c3)
+    w.integrator = "langevin"
+    s = gm.System(w)
+    s.step(c3.equil_steps)
+    s.set_integrator("nve", c3.kT, 0.0)
+    drift, ke = _gpu_drift(s, c3, 10000, 500)
+    assert drift <= 0.01 * ke, f"C3: |dE|/N = {drift:.3e} vs <KE>/N = {ke:.3f}"
+    assert s.stats()["rebuilds"] > 1000
+    s.close()
+
+
+def test_c5_full_2000_steps_drift_and_40_oracle_steps_statistics(gm):
+    w = make_config("C5")
+    g, o = _long_run(gm, w, 40, 20)           # 8M beads, 40,000 chains: oracle ~3 s per step
+    assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)      # mean bond length
+    assert g[:, 4].mean() == pytest.approx(o[:, 4].mean(), rel=0.01)      # bond length variance
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)      # <Rg^2>
+    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)      # temperature
+    assert np.abs(g[:, 0] - o[:, 0]).max() <= 0.01 * o[:, 1].mean()       # same energy per bead
+    s = gm.System(w)                          # the config's full 2,000 NVE steps (~500 rebuilds), GPU only
+    drift, ke = _gpu_drift(s, w, 2000, 100)
+    assert drift <= 0.01 * ke, f"C5: |dE|/N = {drift:.3e} vs <KE>/N = {ke:.3f}"
+    s.close()
+
+
+def test_c4_full_100_steps_dpd_statistics(gm):
+    # 3,000,000 beads, 300,000 chains: one reading of T, bond length or <Rg^2> is good to < 0.1 %, so the 1 % bar
+    # is resolved by every single reading; both runs relax from the same random-walk start
+    w = make_config("C4")
+    g, o = _long_run(gm, w, 100, 25)
+    for col in (2, 3, 5):                     # temperature, mean bond length, <Rg^2>: reading by reading
+        assert np.allclose(g[:, col], o[:, col], rtol=0.01), (col, g[:, col], o[:, col])
+    assert g[:, 4].mean() == pytest.approx(o[:, 4].mean(), rel=0.01)
+
+
+def test_c2_full_1000_steps_langevin_statistics(gm):
+    w = make_config("C2")                     # 64,000 beads, LJ 2.5 + FENE, Langevin (same per-bead noise keys)
+    g, o = _long_run(gm, w, 1000, 100)
+    assert g[:, 2].mean() == pytest.approx(o[:, 2].mean(), rel=0.01)      # (iii) run-averaged T
     assert g[:, 3].mean() == pytest.approx(o[:, 3].mean(), rel=0.01)
-    # <Rg^2> of 300 ten-bead chains: a run average over 1200 steps still carries a standard error of about 1 %
-    # (chain shapes relax over hundreds of steps), estimated here from four block means of each run; the two
-    # averages must agree within 1 % or three standard errors of their difference, whichever is larger
-    def block_se(x):
-        return np.std([b.mean() for b in np.array_split(x, 4)], ddof=1) / 2.0
-    tol = max(0.01 * o[:, 5].mean(), 3.0 * np.hypot(block_se(g[:, 5]), block_se(o[:, 5])))
-    assert abs(g[:, 5].mean() - o[:, 5].mean()) <= tol
+    assert g[:, 5].mean() == pytest.approx(o[:, 5].mean(), rel=0.01)
+
+
+# ---- restart (SURVEY.md 5): n steps + gm_get_particles / gm_set_particles / gm_set_step + n steps vs 2n steps ----
+def _restart(gm, w, n, with_set_step=True):
+    a = gm.System(w)
+    a.step(2 * n)
+    pa, va, _ = a.get_particles(True, True, False)
+    a.close()
+    b = gm.System(w)
+    b.step(n)
+    pb, vb, _ = b.get_particles(True, True, False)
+    b.set_particles(pb, vb, w.type, w.mass)
+    if with_set_step:
+        gm.gm_set_step(b.h, n)
+    b.step(n)
+    pb2, vb2, _ = b.get_particles(True, True, False)
+    assert b.stats()["steps"] == (2 * n if with_set_step else n)
+    b.close()
+    d = pa.astype(np.float64) - pb2
+    d -= w.box * np.rint(d / w.box)
+    return float(np.sqrt((d ** 2).sum(axis=1).mean())), float(np.abs(va - vb2).max())
+
+
+def test_restart_nve_is_roundoff_equal(gm):
+    # NOT bit-identical, and why: (1) the library stores half-step velocities; gm_get_particles completes them to
+    # v^n = u + dt/2 a and the first step after gm_set_particles kicks by dt/2 again, where the uninterrupted run
+    # kicks once by dt (two fp32 roundings instead of one); (2) gm_set_particles enters the beads in tag order, so the
+    # next sort orders the beads of a cell differently and the fp32 force sums run in another order.  Both are
+    # round-off: ~1e-7 sigma after 50 steps.
+    w = make_config("C1")
+    rms, dv = _restart(gm, w, 50)
+    assert rms <= 5e-6 and dv <= 1e-3
+
+
+def test_restart_langevin_needs_and_honours_set_step(gm):
+    # the per-bead noise is keyed by the time level (Philox counter word 2): gm_set_step(n) continues the sequence.
+    # Remaining difference: at the restart the drag acts on the full-step v^n instead of the stored half-step
+    # velocity (O(gamma dt^2 a) = 4e-4 in v once), as it does in the oracle when it is restarted the same way.
+    w = make_config("C2", scale=0.4)
+    rms, _ = _restart(gm, w, 10)
+    assert rms <= 1e-4
+    rms_wrong, _ = _restart(gm, w, 10, with_set_step=False)       # noise of steps 0..n replayed: a different trajectory
+    assert rms_wrong >= 50 * rms
