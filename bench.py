@@ -182,6 +182,9 @@ def main():
     ap.add_argument("--skin", type=float, default=None,
                     help="override the config's neighbor skin (a tuning knob that never changes results; "
                          "BASELINE.json gives none for C4)")
+    ap.add_argument("--tune", action="append", default=[], metavar="FIELD=INT",
+                    help="gm_config tuning override (x_cell_div, nl_scan_trip, step_shape, win_capacity); never changes results")
+    ap.add_argument("--no-windows", action="store_true", help="GM_FLAG_NO_WINDOWS: 32-bit neighbor rows and L1/L2 gathers")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     args = ap.parse_args()
@@ -225,7 +228,10 @@ def main():
         import copy
         w_run = copy.copy(w)
         w_run.integrator = "langevin"
-    s = gm.System(w_run, device=local, flags=gm.GM_FLAG_NO_COND_NODES if args.no_cond_nodes else 0)
+    flags = (gm.GM_FLAG_NO_COND_NODES if args.no_cond_nodes else 0) | (gm.GM_FLAG_NO_WINDOWS if args.no_windows else 0)
+    tune = {k: int(v) for k, v in (kv.split("=") for kv in args.tune)}
+    flags |= tune.pop("flags", 0)
+    s = gm.System(w_run, device=local, flags=flags, tune=tune)
     if w.equil_steps:
         s.step(w.equil_steps)                   # C3: 1,000 Langevin steps (kT=1, gamma=1), then NVE
         s.set_integrator(w.integrator, w.kT, 0.0)
@@ -345,7 +351,7 @@ def main():
             "pairs_in_rc": pairs_in_rc, "mean_nn": nbar_l, "max_nn": st2["max_nn"],
             "rebuilds": rebuilds, "rebuild_interval": m_interval, "reorders": reorders,
             "rebuild_ms_per_timestep_direct": tk["rebuild_ms"] / max(1, tk["force_launches"]),
-            "energy_per_bead": en["etot"] / w.n, "temperature": en["T"],
+            "energy_per_bead": en["etot"] / w.n, "temperature": en["T"], "tuning": s.tuning(),
             "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
         }
         print(json.dumps(line))

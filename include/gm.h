@@ -71,7 +71,7 @@ typedef struct {
     uint32_t struct_size;
     int32_t device;                  /* CUDA device ordinal                                        */
     void *stream;                    /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy default */
-    int64_t n_particles;             /* N >= 1, < 2^28 (bond rows pack the partner index in 28 bits) */
+    int64_t n_particles;             /* N >= 1, < 2^27 (bond rows pack the partner index in 27 bits) */
     int32_t n_types;                 /* 1..GM_MAX_TYPES                                            */
     int32_t max_bonds_per_particle;  /* rows of the BL table (Fig. 2); 0 = no bonds  */
     float box[3];                    /* cuboid edge lengths                                        */
@@ -91,12 +91,15 @@ typedef struct {
     int32_t x_cell_div;              /* 1..8: cells are (r_cut_max + r_skin) / x_cell_div wide in x (DESIGN.md c-12)  */
     int32_t nl_scan_trip;            /* 4 or 8: candidates the neighbor search loads together                         */
     int32_t step_shape;              /* 1: one-warp CTAs (short lists), 2: CTAs of 128 (long lists)                    */
-    int32_t reserved;                /* must be 0                                                                      */
+    int32_t win_capacity;            /* positions a tile window holds (shared memory per CTA = 16 B x this), <= 8000    */
 } gm_config;
 
 enum {
     GM_FLAG_NO_GRAPH = 1,            /* launch every kernel directly (debugging)                   */
     GM_FLAG_NO_COND_NODES = 2,       /* gate the rebuild with early-exit kernels instead of a CUDA conditional graph node */
+    GM_FLAG_NO_WINDOWS = 8,          /* no tile windows: 32-bit neighbor rows and gathers from L1/L2 everywhere (the round-1
+                                        data path; same results up to fp32 summation order -- there is none: the row order
+                                        is the same, so results are bit-identical) */
     GM_FLAG_STEP_SUBWARP = 4         /* step kernel variant for long neighbor lists: 8 lanes share a bead, partial
                                         forces summed by warp shuffles (same results up to fp32 summation order;
                                         measured slower than one thread per bead on B200 -- kept for comparison) */
@@ -188,6 +191,12 @@ gm_status gm_get_neighbors(gm_system *s, int32_t *nn, int32_t *nl_tags, int64_t 
  * sum of nn of the current list, latched device error word (0 = none), nl_row_capacity,
  * number of cells.  Synchronises; returns the latched device error as status if one is set. */
 gm_status gm_get_stats(gm_system *s, int64_t out[8]);
+
+/* out (HOST, 8 int64): what gm_create chose and what the last neighbor build did -- x_cell_div, nl_scan_trip,
+ * step_shape (1 narrow, 2 wide), tile windows in use (0/1), window capacity in positions, tiles (128 beads each),
+ * tiles of the current list that are NOT window-staged, dynamic shared memory of the neighbor-build kernel in bytes.
+ * Synchronises.  Diagnostics only: none of these changes results. */
+gm_status gm_get_tuning(gm_system *s, int64_t out[8]);
 
 /* Host-only utility (a2): the space-filling-curve rank of every cell of an nc[0] x nc[1] x nc[2] grid
  * (linear cell id = (z * nc[1] + y) * nc[0] + x), i.e. the key every neighbor rebuild sorts the beads by:

@@ -47,7 +47,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
 {
     memset(P, 0, sizeof(*P));
     if (!c || c->struct_size != sizeof(gm_config)) return GM_ERR_INVALID_ARG;
-    if (c->n_particles < 1 || c->n_particles >= (1ll << GM_BOND_SHIFT)) return GM_ERR_INVALID_ARG;
+    if (c->n_particles < 1 || c->n_particles >= (1ll << 27)) return GM_ERR_INVALID_ARG;
     if (c->n_types < 1 || c->n_types > GM_MAX_TYPES) return GM_ERR_INVALID_ARG;
     if (c->max_bonds_per_particle < 0 || c->max_bonds_per_particle > 16) return GM_ERR_INVALID_ARG;
     if (c->pair_style < GM_PAIR_NONE || c->pair_style > GM_PAIR_DPD) return GM_ERR_INVALID_ARG;
@@ -56,7 +56,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
-        c->step_shape < 0 || c->step_shape > 2 || c->reserved != 0)
+        c->step_shape < 0 || c->step_shape > 2 || c->win_capacity < 0 || c->win_capacity > 8000)
         return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
     P->ns = (P->n + 8 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+7 (at least): far-away pad beads
@@ -130,9 +130,30 @@ static gm_status derive(const gm_config *c, GmParams *P)
     P->step_subw = (c->flags & GM_FLAG_STEP_SUBWARP) ? 8 : 1;
     P->capq = cap / 4;
     P->minq = std::min(4, P->capq);
+    // tile windows (gm_nlist.cu): LJ-family pair styles, one thread per bead.  A window holds the hulls of the x runs
+    // of a tile's 128 beads in 9 (y, z) rows: 9 (128 + (2 sx + 1) beads-per-x-cell) positions for a tile inside one row;
+    // tiles at a row end hold two partial hulls plus the wrapped pieces -- 1.25 x + 64 covers nearly all of them, the
+    // rest keep the gather path.
+    {
+        const double per_xcell = (double)P->n / ((double)P->nc[0] * P->nc[1] * P->nc[2]);
+        const double est = 9.0 * ((double)GM_TILE + (2.0 * P->sx + 1.0) * per_xcell);
+        int wc = (int)(1.25 * est) + 64;
+        wc = (wc + 7) / 8 * 8;
+        if (c->win_capacity > 0) wc = (c->win_capacity + 7) / 8 * 8;
+        P->use_win = (c->pair_style == GM_PAIR_LJ && P->step_subw == 1 && !(c->flags & GM_FLAG_NO_WINDOWS) &&
+                      wc <= 8000 && P->n < (1 << 27)) ? 1 : 0;
+        if (P->n <= 4096 && P->use_win) wc = std::max(wc, (P->n + 7) / 8 * 8);
+        P->win_cap = P->use_win ? wc : 0;
+    }
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
     for (int t = 0; t < GM_MAX_TYPES * GM_MAX_TYPES; ++t) { P->pair[t].c0 = 0.f; P->pair[t].c1 = 0.f; P->pair[t].c2 = 0.f; P->pair[t].c3 = 0.f; }
     return GM_OK;
+}
+
+static size_t scan_state_bytes(const GmParams &P)
+{
+    const size_t per = (size_t)GM_SCAN_BLOCK * GM_SCAN_ITEMS;
+    return (((size_t)P.n_cells + 1 + per - 1) / per + 1) * 8;
 }
 
 // ---- workspace layout: one pass with base == nullptr sizes it, a second pass assigns pointers ------
@@ -163,11 +184,13 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
         const size_t bb = n * 4 * (size_t)P.max_bonds;
         d.bl = (int *)take(bb); d.blt[0] = (int *)take(bb); d.blt[1] = (int *)take(bb); d.bl_tag = (int *)take(bb);
     }
+    if (P.use_win) d.wdesc = (int4 *)take((n / GM_TILE + 1) * (size_t)GM_WD_STRIDE * sizeof(int4));
     d.key = (int *)take(n * 4); d.rank = (int *)take(n * 4); d.sorted = (int *)take(n * 4);
     d.cstart = (int *)take(((size_t)P.n_cells + 1 + 4) * 4);
     d.ccount = (int *)take(((size_t)P.n_cells + 1 + 4) * 4);
     size_t per = (size_t)GM_SCAN_BLOCK * GM_SCAN_ITEMS;
-    d.scan_sums = (int *)take((((size_t)P.n_cells + 1 + per - 1) / per + 1) * 4);
+    d.scan_state = (unsigned long long *)take(scan_state_bytes(P));
+    d.scan_ticket = (int *)take(4);
     d.row_rank = (uint32_t *)take((size_t)P.nc[1] * P.nc[2] * 4);
     d.stage = (float *)take(n * 4 * 11);
     d.esum = (double *)take(((size_t)GM_ESUM_BLOCKS + 1) * 8 * sizeof(double));
@@ -273,6 +296,7 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     cudaError_t e = cudaSetDevice(cfg->device);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st2, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = gm_nl_prepare(P);
     if (e == cudaSuccess) {
         std::vector<uint32_t> rr;
         sfc_row_order(P.nc[1], P.nc[2], rr);
@@ -280,6 +304,7 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
         if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
     }
     if (e == cudaSuccess) e = cudaMemsetAsync(s->D.ccount, 0, ((size_t)P.n_cells + 1 + 4) * 4, s->st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(s->D.scan_state, 0, scan_state_bytes(P), s->st);
     if (e == cudaSuccess && P.max_bonds > 0) {
         const size_t bb = (size_t)P.ns * 4 * (size_t)P.max_bonds;       // -1 everywhere: no bonds
         e = cudaMemsetAsync(s->D.bl, 0xFF, bb, s->st);
@@ -385,6 +410,7 @@ extern "C" gm_status gm_set_particles(gm_system *s, const float *pos3, const flo
     }
     s->cur = 0;
     gm_launch_set_ctl(s->D, 0, 1, 0, s->st);             // clears the latched device errors: before the pack
+    CU(cudaMemsetAsync(s->D.scan_state, 0, scan_state_bytes(s->P), s->st));   // the rebuild counter (scan epoch) restarts
     gm_launch_pack(s->P, s->D, 0, dp, dv, dt, dm, s->st);
     CU(cudaGetLastError());
     s->step = 0;
@@ -679,6 +705,7 @@ extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, f
 static gm_status dev_error(gm_system *s, const GmCtl &c)
 {
     if (c.err & GM_DEV_ERR_BAD_INPUT) return fail(s, GM_ERR_INVALID_ARG, "gm_set_particles: a type outside [0, n_types) or a mass <= 0%s");
+    if (c.err & GM_DEV_ERR_WINDOW) return fail(s, GM_ERR_CUDA, "a tile window copy did not complete (internal error)%s");
     if (c.err & GM_DEV_ERR_NONFINITE) return fail(s, GM_ERR_NONFINITE, "a coordinate became non-finite%s");
     if (c.err & GM_DEV_ERR_OVERSTRETCH) return fail(s, GM_ERR_BOND_OVERSTRETCH, "a FENE bond reached r >= R0%s");
     if (c.err & GM_DEV_ERR_OVERFLOW) return fail(s, GM_ERR_NEIGHBOR_OVERFLOW, "a neighbor row exceeded nl_row_capacity%s");
@@ -773,6 +800,21 @@ extern "C" gm_status gm_get_neighbors(gm_system *s, int32_t *nn, int32_t *nl_tag
         CU(cudaMemcpyAsync(nl_tags + t0 * row_stride, st + m, m * 4 * (size_t)row_stride, cudaMemcpyDeviceToHost, s->st));
         CU(cudaStreamSynchronize(s->st));
     }
+    return GM_OK;
+}
+
+extern "C" gm_status gm_get_tuning(gm_system *s, int64_t out[8])
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!out) return fail(s, GM_ERR_INVALID_ARG, "gm_get_tuning: NULL out%s");
+    CU(cudaSetDevice(s->cfg.device));
+    GmCtl c;
+    gm_status r = sync_and_check(s, &c);
+    if (r == GM_ERR_CUDA) return r;
+    out[0] = s->P.sx; out[1] = s->P.nl_trip; out[2] = s->P.step_wide ? 2 : 1; out[3] = s->P.use_win;
+    out[4] = s->P.win_cap; out[5] = (s->P.n + GM_TILE - 1) / GM_TILE;
+    out[6] = s->P.use_win ? c.n_glob_tiles : out[5];
+    out[7] = gm_nl_smem_bytes(s->P);
     return GM_OK;
 }
 

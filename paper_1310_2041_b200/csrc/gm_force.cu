@@ -23,7 +23,7 @@
 // of this batch are in flight before the first force term is evaluated.
 #include "gm_internal.cuh"
 
-#define FORCE_BLOCK 128
+#define FORCE_BLOCK 128          // = GM_TILE: a CTA of k_force / k_energy owns one tile
 #ifndef STEP_BLOCK
 #define STEP_BLOCK 32            // beads per CTA of the short-list step kernel: one warp
 #endif
@@ -37,6 +37,10 @@
 #ifndef WIDE_NQ
 #define WIDE_NQ 2                //   gather batches of two quads
 #endif
+#ifndef WINS_MINB
+#define WINS_MINB 8              // short lists on window-staged systems: CTAs of GM_TILE beads, 8 resident per SM
+#endif
+static_assert(WIDE_BLOCK == GM_TILE && FORCE_BLOCK == GM_TILE, "a CTA of the window-staged force kernels owns one tile");
 #ifndef SUB_BLOCK
 #define SUB_BLOCK 128            // threads per CTA of the sub-warp step kernel
 #endif
@@ -123,14 +127,25 @@ __device__ __forceinline__ const int4 *nl_row(const GmParams &P, const GmDev &D,
     return D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31);
 }
 
-// The first quads of row i, issued together with the other streaming loads of the bead (always written
-// by the build, padded with the far-away bead, so they do not depend on NN).
+// The head of row i, issued together with the other streaming loads of the bead (always written by the build and
+// padded, so it does not depend on NN).  The first two int4 are needed whatever the tile's format is (quads 0-1 of
+// a 32-bit row, octs 0-1 of a 16-bit row); quads 2-3 of a 32-bit row follow once the format is known (at once on
+// systems without tile windows).
 __device__ __forceinline__ void nl_preload(const GmParams &P, const int4 *__restrict__ t, uint64_t pol,
                                            int4 (&pre)[GM_PRE])
 {
     const int4 pad = make_int4(P.n, P.n, P.n, P.n);
 #pragma unroll
-    for (int u = 0; u < GM_PRE; ++u) pre[u] = (u < P.minq) ? gm_ld_stream(t + u * 32, pol) : pad;
+    for (int u = 0; u < GM_PRE; ++u)
+        pre[u] = (u < P.minq && (u < 2 || !P.use_win)) ? gm_ld_stream(t + u * 32, pol) : pad;
+}
+
+__device__ __forceinline__ void nl_preload_rest(const GmParams &P, const int4 *__restrict__ t, uint64_t pol,
+                                                int4 (&pre)[GM_PRE])
+{
+#pragma unroll
+    for (int u = 2; u < GM_PRE; ++u)
+        if (u < P.minq) pre[u] = gm_ld_stream(t + u * 32, pol);
 }
 
 // Gather loop over row i of NL (Alg. 2), NQ quads (4 NQ list entries) per batch:
@@ -179,6 +194,114 @@ __device__ __forceinline__ void pair_loop(const GmParams &P, const Src &S, const
         for (int u = 0; u < 4 * NQ; ++u)
             pair_term<PAIR, NT1, ENERGY, MI>(P, me, pj[u], PAIR == GM_PAIR_DPD ? vj[u] : zero4, p0,
                                              (uint32_t)step, fx, fy, fz, pe, cnt);
+    }
+    o.fx += fx; o.fy += fy; o.fz += fz;
+    o.pe_pair = 0.5f * pe;
+    o.cnt = cnt;
+}
+
+// ---- window-staged tiles (gm_nlist.cu "tile windows") -------------------------------------------------------------
+// The positions a tile's NL rows refer to are a few contiguous ranges of the position array (the same ranges at every
+// step until the next rebuild, because storage order is fixed in between).  The warp copies them into shared memory
+// with cp.async.bulk (TMA engine: no LSU wavefronts, no registers, completion on an mbarrier) while its lanes request
+// their own streams; the NL rows hold 16-bit window offsets, and every neighbor "gather" is an LDS.128.
+// shared memory of one CTA (= one tile of GM_TILE beads) of a force kernel: the window (pad bead + win_cap positions)
+// and its mbarrier
+__host__ __device__ __forceinline__ int gm_win_bytes(const GmParams &P) { return P.use_win ? (P.win_cap + 2) * 16 : 0; }
+
+struct Tile {
+    uint32_t win;            // shared-memory byte address of window position 0 (the far-away pad bead)
+    uint32_t mbar;
+    int staged;              // 1: window-staged tile (16-bit rows), copies in flight; 0: 32-bit rows, gathers
+    uint32_t parity;         // mbarrier phase to wait for
+};
+
+#define GM_WD_FIRST 12       // descriptor entries fetched before the range count is known (a tile inside one row has 9-10)
+
+// Step 1, with the bead's other streaming loads: the header word of the tile's window descriptor (every thread; one
+// broadcast load) and, in warp 0, this lane's range.
+__device__ __forceinline__ int4 tile_desc(const GmParams &P, const GmDev &D, int tile)
+{
+    int4 d = make_int4(0, 0, 0, 0);
+    if (!P.use_win) return d;
+    const int4 *__restrict__ wd = D.wdesc + (size_t)tile * GM_WD_STRIDE;
+    if (threadIdx.x < GM_WD_FIRST) d = __ldg(wd + threadIdx.x);
+    d.w = __ldg(&wd[0].w);                   // entries past the tile's range count are stale: the header is entry 0's
+    return d;
+}
+
+// Step 2 (all threads of the CTA that owns `tile`; one block-level barrier inside): thread 0 arms the mbarrier, the
+// lanes of warp 0 issue one bulk copy per range.  smem: the CTA's window area (pad bead + win_cap positions) + mbarrier.
+__device__ __forceinline__ Tile tile_stage(const GmParams &P, const GmDev &D, const Src &S, int tile, int4 d, char *smem,
+                                           uint32_t parity, bool first)
+{
+    Tile T;
+    T.win = (uint32_t)__cvta_generic_to_shared(smem);
+    T.mbar = T.win + (uint32_t)(P.win_cap + 1) * 16u;
+    T.staged = 0;
+    T.parity = parity;
+    if (!P.use_win) return T;
+    const int hdr = d.w;                     // the same word in every entry of the descriptor
+    if (first) {
+        if (threadIdx.x == 0) {
+            gm_mbar_init(T.mbar, 1);
+            *reinterpret_cast<float4 *>(smem) = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+        }
+        __syncthreads();
+    }
+    if (!(hdr & 0x100)) return T;
+    T.staged = 1;
+    if (threadIdx.x >= 32) return T;
+    const int lane = threadIdx.x;
+    const int nr = hdr & 0xff;
+    if (lane == 0) gm_mbar_expect_tx(T.mbar, (uint32_t)(hdr >> 16) * 16u);
+    __syncwarp();
+    const int4 *__restrict__ wd = D.wdesc + (size_t)tile * GM_WD_STRIDE;
+    if (lane >= GM_WD_FIRST && lane < nr) d = __ldg(wd + lane);
+    if (lane < nr) gm_bulk_g2s(T.win + (uint32_t)d.y * 16u, S.pos + d.x, (uint32_t)d.z * 16u, T.mbar);
+    if (lane + 32 < nr) {
+        const int4 e = __ldg(wd + lane + 32);
+        gm_bulk_g2s(T.win + (uint32_t)e.y * 16u, S.pos + e.x, (uint32_t)e.z * 16u, T.mbar);
+    }
+    return T;
+}
+
+// Gather loop over row i of a window-staged tile: eight 16-bit window offsets per int4 ("oct"), the first GM_PRE_W
+// octs preloaded; unused slots hold offset 0, the pad bead.
+#define GM_PRE_W 2
+template <int PAIR, bool NT1, bool ENERGY, bool MI>
+__device__ __forceinline__ void pair_loop_win(const GmParams &P, const Tile &T, const int4 *__restrict__ t,
+                                              uint64_t pol, const int4 (&pre)[GM_PRE], const int nn, const Own &me,
+                                              BeadForce &o)
+{
+    const int no = (nn + 7) >> 3;
+    float fx = 0.f, fy = 0.f, fz = 0.f, pe = 0.f, cnt = 0.f;
+    const GmPair p0 = P.pair[0];
+    const float4 zero4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    const int4 none = make_int4(0, 0, 0, 0);
+    const uint32_t win = T.win;
+    auto half_oct = [&](const uint32_t a, const uint32_t b) {
+        float4 pj[4];
+        pj[0] = gm_lds128(win + ((a & 0xffffu) << 4));
+        pj[1] = gm_lds128(win + ((a >> 16) << 4));
+        pj[2] = gm_lds128(win + ((b & 0xffffu) << 4));
+        pj[3] = gm_lds128(win + ((b >> 16) << 4));
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+            pair_term<PAIR, NT1, ENERGY, MI>(P, me, pj[u], zero4, p0, 0u, fx, fy, fz, pe, cnt);
+    };
+    int4 en = (GM_PRE_W < no) ? gm_ld_stream(t + GM_PRE_W * 32, pol) : none;
+#pragma unroll
+    for (int b = 0; b < GM_PRE_W; ++b)
+        if (b < no) {
+            half_oct((uint32_t)pre[b].x, (uint32_t)pre[b].y);
+            half_oct((uint32_t)pre[b].z, (uint32_t)pre[b].w);
+        }
+    for (int q = GM_PRE_W; q < no; ++q) {
+        const int4 e = en;
+        en = (q + 1 < no) ? gm_ld_stream(t + (q + 1) * 32, pol) : none;
+        half_oct((uint32_t)e.x, (uint32_t)e.y);
+        half_oct((uint32_t)e.z, (uint32_t)e.w);
     }
     o.fx += fx; o.fy += fy; o.fz += fz;
     o.pe_pair = 0.5f * pe;
@@ -254,9 +377,20 @@ __device__ __forceinline__ void pair_loop_dpd(const GmParams &P, const Src &S, c
 }
 
 // Bond partners of bead i from column i of BL (Fig. 2), two at a time; -1 = no bond.
+template <int BOND>
+__device__ __forceinline__ void bond_head(const GmParams &P, const GmDev &D, int i, int (&be)[2])
+{
+    be[0] = be[1] = -1;
+    if (BOND == GM_BOND_NONE) return;
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
+        if (u < P.max_bonds) be[u] = __ldg(D.bl + i + (size_t)u * P.ns);
+}
+
+// be: rows 0 and 1 of column i (bond_head, requested with the bead's other streams)
 template <int BOND, bool ENERGY>
 __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, const Src &S, int i, const float4 pi,
-                                          BeadForce &o)
+                                          const int (&be)[2], const Tile &T, BeadForce &o)
 {
     if (BOND == GM_BOND_NONE) return;
     float pe = 0.f;
@@ -266,9 +400,14 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
         int e[2];
         float4 pj[2];
 #pragma unroll
-        for (int u = 0; u < 2; ++u) e[u] = (k + u < P.max_bonds) ? __ldg(bl + (size_t)(k + u) * n) : -1;
+        for (int u = 0; u < 2; ++u) e[u] = (k == 0) ? be[u] : ((k + u < P.max_bonds) ? __ldg(bl + (size_t)(k + u) * n) : -1);
 #pragma unroll
-        for (int u = 0; u < 2; ++u) pj[u] = (e[u] >= 0) ? __ldg(S.pos + (e[u] & GM_BOND_MASK)) : pi;
+        for (int u = 0; u < 2; ++u) {
+            // a partner inside the tile's window is a window offset (GM_BOND_LOCAL, set by k_nl_build), else a bead index
+            if (e[u] < 0) pj[u] = pi;
+            else if (e[u] & GM_BOND_LOCAL) pj[u] = gm_lds128(T.win + ((uint32_t)(e[u] & 0xffff) << 4));
+            else pj[u] = __ldg(S.pos + (e[u] & GM_BOND_MASK));
+        }
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             if (e[u] < 0) continue;
@@ -308,11 +447,13 @@ template <int PAIR, bool NT1, int BOND, bool ENERGY, int NQL>
 __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &D, const Src &S, int i,
                                                 const float4 pi, const float4 vti, const int4 *__restrict__ t,
                                                 uint64_t pol, const int4 (&pre)[GM_PRE], const int nn,
-                                                unsigned long long step, int *__restrict__ col)
+                                                unsigned long long step, int *__restrict__ col, const Tile &T,
+                                                const int (&be)[2], const bool valid)
 {
     BeadForce o;
     o.fx = o.fy = o.fz = o.pe_pair = o.pe_bond = o.cnt = 0.f;
-    bond_loop<BOND, ENERGY>(P, D, S, i, pi, o);
+    if (T.staged && !gm_mbar_wait(T.mbar, T.parity)) atomicOr(&D.ctl->err, GM_DEV_ERR_WINDOW);   // the window has landed
+    bond_loop<BOND, ENERGY>(P, D, S, i, pi, be, T, o);
     if (PAIR != GM_PAIR_NONE) {
         Own me;
         me.p = pi; me.vt = vti; me.t = __float_as_int(pi.w);
@@ -322,11 +463,14 @@ __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &
         // boundary (both moved < skin/2 since the build): plain differences, no image test.  Decided per
         // warp so that a warp runs one of the two loops, not both.
         const float m = P.edge_margin;
-        const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
-                              fabsf(pi.z) < P.half[2] - m;
+        const bool interior = !valid || (fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m &&
+                                         fabsf(pi.z) < P.half[2] - m);
         if (PAIR == GM_PAIR_DPD) {
             if (__all_sync(__activemask(), interior)) pair_loop_dpd<NT1, ENERGY, false>(P, S, t, pol, pre, nn, me, step, o, col);
             else pair_loop_dpd<NT1, ENERGY, true>(P, S, t, pol, pre, nn, me, step, o, col);
+        } else if (T.staged) {
+            if (__all_sync(__activemask(), interior)) pair_loop_win<PAIR, NT1, ENERGY, false>(P, T, t, pol, pre, nn, me, o);
+            else pair_loop_win<PAIR, NT1, ENERGY, true>(P, T, t, pol, pre, nn, me, o);
         } else if (__all_sync(__activemask(), interior)) pair_loop<PAIR, NT1, ENERGY, false, NQL>(P, S, t, pol, pre, nn, me, step, o);
         else pair_loop<PAIR, NT1, ENERGY, true, NQL>(P, S, t, pol, pre, nn, me, step, o);
     }
@@ -352,12 +496,16 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, in
 }
 
 // ---- the per-step work of one bead (MODE_STEP) / its materialised force (MODE_FORCES) -----------------
+// Called by all threads of the CTA (window staging is a block-collective step); threads past the last bead
+// (valid = false) work on the pad slots (far away, NN = 0, no bonds) and store nothing.
 template <int PAIR, bool NT1, int BOND, int MODE, int NQL>
-__device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, const Src &S, const int i,
+__device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, const Src &S, const int i, const bool valid,
                                           const unsigned long long step, const int parity, const float kick,
-                                          const float kick_vt, int *__restrict__ col)
+                                          const float kick_vt, int *__restrict__ col, char *wsm)
 {
-    // every stream of this bead is requested before anything is used
+    // every stream of this bead is requested before anything is used; the tile's window descriptor first (the bulk
+    // copies wait for it)
+    const int4 wd = tile_desc(P, D, blockIdx.x);
     const uint64_t pol = gm_policy_evict_first();
     const int4 *__restrict__ t = nl_row(P, D, i);
     int4 pre[GM_PRE];
@@ -369,7 +517,13 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
     if (MODE == GM_MODE_STEP) rf = gm_ld_nol1(D.ref + i);
     float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
     if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES, NQL>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col);
+    int be[2];
+    bond_head<BOND>(P, D, i, be);
+    // the window's ranges are known: the copies go out while the streams above are in flight
+    const Tile T = tile_stage(P, D, S, blockIdx.x, wd, wsm, 0u, true);
+    if (PAIR != GM_PAIR_NONE && P.use_win && !T.staged) nl_preload_rest(P, t, pol, pre);
+    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES, NQL>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col, T, be, valid);
+    if (!valid) return;
     const float3 a = bead_accel(P, S, i, f, u, step);
     if (MODE == GM_MODE_FORCES) {
         D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
@@ -398,8 +552,9 @@ k_force(const __grid_constant__ GmParams P, GmDev D, int parity)
     const unsigned long long step = D.ctl->step[parity];
     const Src S = current_src(D, parity, step);
     GM_CPT_DECL(PAIR, FORCE_BLOCK);
-    if (i >= P.n) return;
-    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES, GM_LJ_NQ>(P, D, S, i, step, parity, 0.f, 0.f, gm_cpt + threadIdx.x);
+    extern __shared__ __align__(16) char gm_win_smem[];
+    bead_step<PAIR, NT1, BOND, GM_MODE_FORCES, GM_LJ_NQ>(P, D, S, i, i < P.n, step, parity, 0.f, 0.f, gm_cpt + threadIdx.x,
+                                                        gm_win_smem);
 }
 
 // The step kernel (a4..a8).  A CTA owns BLOCK consecutive beads: storage order is cell order along the curve,
@@ -424,7 +579,11 @@ k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, floa
     }
     const int i = blockIdx.x * BLOCK + threadIdx.x;
     GM_CPT_DECL(PAIR, BLOCK);
-    if (i < P.n) bead_step<PAIR, NT1, BOND, GM_MODE_STEP, NQL>(P, D, S, i, step, parity, kick, kick_vt, gm_cpt + threadIdx.x);
+    extern __shared__ __align__(16) char gm_win_smem[];
+    // window-staged systems run CTAs of GM_TILE beads (one tile each); every thread takes part in the staging
+    if (P.use_win || i < P.n)
+        bead_step<PAIR, NT1, BOND, GM_MODE_STEP, NQL>(P, D, S, i, i < P.n, step, parity, kick, kick_vt, gm_cpt + threadIdx.x,
+                                                      gm_win_smem);
 }
 
 // The step kernel for LONG neighbor lists (n_l of 80-100: LJ with r_c = 2.5, configs C2/C5): SUBW lanes share
@@ -491,7 +650,11 @@ k_step_sub(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, 
     if (!valid || sub != 0) return;
     BeadForce f;
     f.fx = 0.f; f.fy = 0.f; f.fz = 0.f; f.pe_pair = 0.f; f.pe_bond = 0.f; f.cnt = 0.f;
-    bond_loop<BOND, false>(P, D, S, i, pi, f);
+    Tile T;
+    T.win = 0; T.mbar = 0; T.staged = 0; T.parity = 0;     // GM_FLAG_STEP_SUBWARP systems keep 32-bit rows everywhere
+    int be[2];
+    bond_head<BOND>(P, D, i, be);
+    bond_loop<BOND, false>(P, D, S, i, pi, be, T, f);
     f.fx += fx; f.fy += fy; f.fz += fz;
     const float4 u = gm_ld_nol1(S.vel + i);
     const float4 rf = gm_ld_nol1(D.ref + i);
@@ -515,7 +678,16 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
     const Src S = current_src(D, parity, step);
     GM_CPT_DECL(PAIR, FORCE_BLOCK);
     double acc[7] = { 0, 0, 0, 0, 0, 0, 0 };   // ke, pe_pair, pe_bond, px, py, pz, pairs
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < P.n; i += gridDim.x * blockDim.x) {
+    extern __shared__ __align__(16) char gm_win_smem[];
+    char *wsm = gm_win_smem;
+    uint32_t phase = 0;
+    bool armed = false;                                     // the CTA's mbarrier is initialised
+    // a CTA takes tiles blockIdx, blockIdx + gridDim, ...: the trip count is CTA-uniform (window staging is a
+    // block-collective step)
+    for (int base = blockIdx.x * FORCE_BLOCK; base < P.n; base += gridDim.x * FORCE_BLOCK) {
+        const int i = base + threadIdx.x;
+        __syncthreads();                                    // every thread is done with the previous window
+        const bool valid = i < P.n;
         const uint64_t pol = gm_policy_evict_first();
         const int4 *__restrict__ t = nl_row(P, D, i);
         int4 pre[GM_PRE];
@@ -524,7 +696,14 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
         const int nn = (PAIR != GM_PAIR_NONE) ? D.nn[i] : 0;
         float4 vti = make_float4(0.f, 0.f, 0.f, 0.f);
         if (PAIR == GM_PAIR_DPD) vti = S.vt[i];
-        const BeadForce f = bead_force<PAIR, NT1, BOND, true, GM_LJ_NQ>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x);
+        int be[2];
+        bond_head<BOND>(P, D, i, be);
+        const Tile T = tile_stage(P, D, S, base / GM_TILE, tile_desc(P, D, base / GM_TILE), wsm, phase, !armed);
+        armed = true;
+        if (T.staged) phase ^= 1u;                          // the mbarrier completes one phase per staged tile
+        if (PAIR != GM_PAIR_NONE && P.use_win && !T.staged) nl_preload_rest(P, t, pol, pre);
+        const BeadForce f = bead_force<PAIR, NT1, BOND, true, GM_LJ_NQ>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x, T, be, valid);
+        if (!valid) continue;
         const float4 u = S.vel[i];
         float vx = u.x, vy = u.y, vz = u.z;
         if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m
@@ -566,27 +745,45 @@ __global__ void __launch_bounds__(7 * 32) k_energy_final(GmDev D, int n_blocks)
     if (lane == 0) D.esum[(size_t)GM_ESUM_BLOCKS * 8 + q] = v;
 }
 
+// Kernels that stage tile windows take their shared memory at launch; above 48 KB per CTA that needs an opt-in, set
+// once per instantiation and size.
+template <typename K>
+static void allow_smem(K kernel, int bytes)
+{
+    if (bytes > 48 * 1024) cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
 template <int PAIR, bool NT1, int BOND>
 static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
                            int lagged, cudaStream_t st)
 {
     int nb = (P.n + FORCE_BLOCK - 1) / FORCE_BLOCK;
+    const int wb = gm_win_bytes(P);
     if (mode == GM_MODE_STEP) {
         if (P.step_subw == 8 && PAIR != GM_PAIR_NONE) {
             const long long nt = (long long)P.n * 8;
             k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + SUB_BLOCK - 1) / SUB_BLOCK), SUB_BLOCK, 0, st>>>(
                 P, D, parity, kick, kick_vt);
-        } else if (P.step_wide || PAIR == GM_PAIR_DPD)
-            k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, WIDE_NQ><<<(P.n + WIDE_BLOCK - 1) / WIDE_BLOCK, WIDE_BLOCK, 0, st>>>(
+        } else if (P.step_wide || PAIR == GM_PAIR_DPD) {
+            allow_smem(k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, WIDE_NQ>, wb);
+            k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, WIDE_NQ><<<(P.n + WIDE_BLOCK - 1) / WIDE_BLOCK, WIDE_BLOCK, wb, st>>>(
                 P, D, parity, kick, kick_vt);
-        else if constexpr (PAIR != GM_PAIR_DPD)
-            k_step<PAIR, NT1, BOND, STEP_BLOCK, STEP_MINB, GM_LJ_NQ><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(
-                P, D, parity, kick, kick_vt);
-    } else if (mode == GM_MODE_FORCES)
-        k_force<PAIR, NT1, BOND><<<nb, FORCE_BLOCK, 0, st>>>(P, D, parity);
-    else {
+        } else if constexpr (PAIR != GM_PAIR_DPD) {
+            if (P.use_win) {        // short lists, window-staged: CTAs of one tile, 8 resident per SM (<= 64 registers)
+                allow_smem(k_step<PAIR, NT1, BOND, GM_TILE, WINS_MINB, GM_LJ_NQ>, wb);
+                k_step<PAIR, NT1, BOND, GM_TILE, WINS_MINB, GM_LJ_NQ><<<(P.n + GM_TILE - 1) / GM_TILE, GM_TILE, wb, st>>>(
+                    P, D, parity, kick, kick_vt);
+            } else
+                k_step<PAIR, NT1, BOND, STEP_BLOCK, STEP_MINB, GM_LJ_NQ><<<(P.n + STEP_BLOCK - 1) / STEP_BLOCK, STEP_BLOCK, 0, st>>>(
+                    P, D, parity, kick, kick_vt);
+        }
+    } else if (mode == GM_MODE_FORCES) {
+        allow_smem(k_force<PAIR, NT1, BOND>, wb);
+        k_force<PAIR, NT1, BOND><<<nb, FORCE_BLOCK, wb, st>>>(P, D, parity);
+    } else {
         int g = nb < GM_ESUM_BLOCKS ? nb : GM_ESUM_BLOCKS;
-        k_energy<PAIR, NT1, BOND><<<g, FORCE_BLOCK, 0, st>>>(P, D, parity, lagged);
+        allow_smem(k_energy<PAIR, NT1, BOND>, wb);
+        k_energy<PAIR, NT1, BOND><<<g, FORCE_BLOCK, wb, st>>>(P, D, parity, lagged);
         k_energy_final<<<1, 7 * 32, 0, st>>>(D, g);
     }
 }

@@ -18,6 +18,11 @@
 //   nl      int4[n_tiles * capq * 32]  NL in tiles of 32 beads: entries 4q..4q+3 of bead (tile, lane)
 //                       are the int4 at (tile * capq + q) * 32 + lane; slots past NN hold the index n
 //                       (a far-away pad bead).  PAPER.md:L51, Fig. 1 (table form NL[k*Np+i], re-tiled)
+//                       Window-staged tiles (wdesc header mode 1) hold 16-bit offsets into the tile's position window
+//                       instead, eight per uint4 ("oct"), oct o of bead (tile, lane) at (tile * capq + o) * 32 + lane;
+//                       unused slots hold 0, the window's pad bead.
+//   wdesc   int4[n_tiles * GM_WD_STRIDE]  tile window descriptors: [k] = (first slot, window offset, length,
+//                       n_ranges | mode << 8 | window length << 16) of range k < n_ranges; mode 0: [0] = 0
 //   nn      int[ns]     NN[i];   nnw int[ns/32]: max NN per tile
 //   blt[2]  int[mb*ns]  BL in TAG space, storage order: blt[k*ns + i] = partner tag | btype << 28, -1 = none
 //   bl      int[mb*ns]  BL in index space: bl[k*ns + i] = j | btype << 28, -1 = none   PAPER.md:L97, Fig. 2
@@ -31,11 +36,16 @@
 
 #define GM_PAD 256               // per-bead arrays are allocated (and table rows strided) in multiples of this
 #define GM_BOND_SHIFT 28
-#define GM_BOND_MASK ((1 << GM_BOND_SHIFT) - 1)
+#define GM_BOND_LOCAL (1 << 27)  // BL entry: the partner index is an offset into the tile's position window
+#define GM_BOND_MASK ((1 << 27) - 1)
+#define GM_TILE 128              // beads per tile of the window-staged path: one CTA of k_nl_build and of the force kernels
+#define GM_WD_STRIDE 40          // int4 entries per tile window descriptor, one per range
+#define GM_WD_MAXR 40
+#define GM_WIN_SLOTS 54          // window range slots of a tile: 2 row groups x 9 (y, z) rows x {A, B_lo, B_hi}
 #define GM_NEVER (~0ull)
 
 // latched device error bits (GmCtl::err)
-enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE = 4, GM_DEV_ERR_BAD_INPUT = 8 };
+enum { GM_DEV_ERR_OVERFLOW = 1, GM_DEV_ERR_OVERSTRETCH = 2, GM_DEV_ERR_NONFINITE = 4, GM_DEV_ERR_BAD_INPUT = 8, GM_DEV_ERR_WINDOW = 16 };
 
 // Small device control block (one per system).
 struct GmCtl {
@@ -47,7 +57,7 @@ struct GmCtl {
     int max_nn;
     int err;
     int go;                        // decision of the last k_gate: the rebuild chain runs iff != 0
-    int pad;
+    int n_glob_tiles;              // tiles of the current list that are NOT window-staged (32-bit rows, gathers from HBM/L2)
 };
 
 // Per-type-pair coefficients.  LJ: c0 = r_c^2, c1 = 48 eps sigma^12, c2 = 24 eps sigma^6, c3 = U_shift.
@@ -66,6 +76,8 @@ struct GmParams {
     int step_wide;                 // step kernel shape: 0 = one-warp CTAs (short lists), 1 = CTAs of 128 (long lists)
     int step_subw;                 // lanes per bead of the step kernel: 1 (short lists), 4 or 8 (long lists)
     int sfc_period;                // a rebuild (= SFC sort) is forced after this many steps without one; <= 0: never
+    int use_win;                   // 1: tiles are window-staged where they can be (16-bit window-local NL rows)
+    int win_cap;                   // positions a tile window holds at most (the shared-memory budget per warp)
     float box[3], half[3], inv_w[3];
     float r_list2, half_skin2;
     float edge_margin;             // r_list + r_skin: beads further than this from every face need no image test
@@ -92,9 +104,11 @@ struct GmDev {
     int *bl;                 // index space
     int *blt[2];             // tag space, storage order
     int *bl_tag;             // tag space master copy in TAG order (bl_tag[k*ns + tag]), from gm_set_bonds
+    int4 *wdesc;             // [n_tiles * GM_WD_STRIDE] tile window descriptors (see gm_nlist.cu)
     int *key, *rank, *sorted;
     int *cstart, *ccount;
-    int *scan_sums;          // per scan block
+    unsigned long long *scan_state;   // per scan tile: value | (epoch << 2 | status) << 32 (k_scan)
+    int *scan_ticket;
     uint32_t *row_rank;      // SFC rank of each (y, z) row of cells
     float *stage;            // 11 ns floats: I/O staging (pos3, vel3, force3, type, mass)
     double *esum;            // [GM_ESUM_BLOCKS * 8] partials, then [8] totals at the end
@@ -114,6 +128,8 @@ void gm_launch_gate(const GmDev &D, int gate, int parity, unsigned long long con
 void gm_launch_sort(const GmParams &P, const GmDev &D, int parity, cudaStream_t st);    // a1 + a2 (if ctl->go)
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st);            // a3      (if ctl->go)
 int gm_nl_capacity_ok(const GmParams &P);
+int gm_nl_smem_bytes(const GmParams &P);
+cudaError_t gm_nl_prepare(const GmParams &P);      // opt-in shared-memory sizes of the kernels that stage windows
 void gm_launch_bonds_from_master(const GmParams &P, const GmDev &D, cudaStream_t st);
 void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
                      int lagged, cudaStream_t st);
@@ -200,6 +216,46 @@ __device__ __forceinline__ float4 gm_ld_nol1(const float4 *ptr)
     float4 v;
     asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
                  : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(ptr));
+    return v;
+}
+
+// ---- mbarrier + 1-D bulk copy (TMA engine: global -> shared without LSU wavefronts) ----------------------------
+__device__ __forceinline__ void gm_mbar_init(uint32_t mbar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(mbar), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+
+__device__ __forceinline__ void gm_mbar_expect_tx(uint32_t mbar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mbar), "r"(bytes) : "memory");
+}
+
+// bytes > 0, multiple of 16; dst and src 16-byte aligned
+__device__ __forceinline__ void gm_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t mbar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+
+// try_wait with a suspend-time hint: the warp sleeps in hardware until the phase completes (or the hint, 1 ms, runs
+// out) instead of burning issue slots in a polling loop.  Returns false if the phase did not complete within ~4 s
+// (a byte-count mismatch would otherwise hang the GPU); the caller latches GM_DEV_ERR_WINDOW and carries on.
+__device__ __forceinline__ bool gm_mbar_wait(uint32_t mbar, uint32_t parity)
+{
+    uint32_t ok;
+    int polls = 0;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+                     "selp.u32 %0, 1, 0, p;\n\t}" : "=r"(ok) : "r"(mbar), "r"(parity), "r"(1000000u) : "memory");
+    } while (!ok && ++polls < 4096);
+    return ok != 0;
+}
+
+__device__ __forceinline__ float4 gm_lds128(uint32_t addr)
+{
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
     return v;
 }
 

@@ -105,7 +105,7 @@ __global__ void k_set_ctl(GmDev D, unsigned long long step, int reset_all, int p
     c->rebuilt_at = fresh ? step : GM_NEVER;
     c->go = 0;
     if (reset_all) {
-        c->n_rebuilds = 0; c->sum_nn = 0; c->max_nn = 0; c->err = 0; c->pad = 0;
+        c->n_rebuilds = 0; c->sum_nn = 0; c->max_nn = 0; c->err = 0; c->n_glob_tiles = 0;
     }
 }
 

@@ -19,10 +19,32 @@
 // whatever the row capacity, which leaves the rest of the SM's 228 KB to L1 for the candidate loads.
 #include "gm_internal.cuh"
 
-#define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 4)
+#define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 8)
 #ifndef NL_WARPS
 #define NL_WARPS 4
 #endif
+static_assert(NL_WARPS * 32 == GM_TILE, "one CTA of k_nl_build owns one tile");
+
+// ---- tile windows -----------------------------------------------------------------------------------------------
+// A tile = the GM_TILE = 128 consecutive beads of one CTA.  Storage order is cell order, so the candidates of ALL beads of a
+// tile lie in a few contiguous ranges of the position array: for each of the 9 (y, z) rows around the tile's row the
+// hull of the beads' x runs ("A"), plus, for beads within sx cells of an x face, the cells at the other end of the
+// row ("B_lo": beads at the low face see the high end, "B_hi": the reverse); a tile that straddles a row end has two
+// row groups, each with its own 27 range slots.  The concatenation of the non-empty ranges is the tile's WINDOW.
+// k_nl_build writes the window's descriptor (D.wdesc) and the NL row of a bead as 16-bit offsets into the window;
+// the force kernels (gm_force.cu) bulk-copy the window of the CURRENT positions into shared memory each step
+// (cp.async.bulk, TMA engine: no LSU wavefronts; storage order is fixed until the next rebuild) and turn the neighbor
+// gathers into LDS.128.  Window offset 0 is a far-away pad bead.
+// A system of at most win_cap beads takes the whole position array as the window of every tile (one range).
+// Tiles whose window does not fit (more than GM_WD_MAXR ranges, more than GmParams::win_cap positions, more than two
+// rows of cells) keep 32-bit rows and the gather path (mode 0).
+// The build itself keeps reading its candidates through L1 (79 % hits; a shared-memory copy of the window cost more
+// in occupancy than the remaining misses do -- profiles/r02_windows.md).
+struct NlWin {
+    const int4 *rng;         // [GM_WIN_SLOTS] (first slot, window offset, length, row base r0 * ncx) per range slot
+    int group;               // row group of this lane's bead (0 or 1)
+    int whole;               // the window is the whole position array (small systems): offset = bead slot + 1
+};
 
 struct NlRow {
     int *ring;               // this lane's column of the ring: ring[(k & (NL_STAGE-1)) * 32]
@@ -33,21 +55,37 @@ struct NlRow {
     int cap;
 };
 
-// write entries [flushed, flushed + 16) of the row (whole quads) from the ring to the tile
+__device__ __forceinline__ uint32_t nl_pack2(int lo, int hi) { return (uint32_t)lo | ((uint32_t)hi << 16); }
+
+// write entries [flushed, flushed + 16) of the row from the ring to the tile: four quads of 32-bit bead indices, or
+// (W16) two octs of 16-bit window offsets
+template <bool W16>
 __device__ __forceinline__ void nl_flush16(NlRow &r)
 {
     if (r.flushed + 16 <= r.cap) {
+        if (W16) {
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int e = r.flushed + 4 * q;
-            r.tile[(e >> 2) * 32] = make_int4(r.ring[((e + 0) & (NL_STAGE - 1)) * 32], r.ring[((e + 1) & (NL_STAGE - 1)) * 32],
-                                              r.ring[((e + 2) & (NL_STAGE - 1)) * 32], r.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+            for (int o = 0; o < 2; ++o) {
+                const int e = r.flushed + 8 * o;
+                int v[8];
+#pragma unroll
+                for (int u = 0; u < 8; ++u) v[u] = r.ring[((e + u) & (NL_STAGE - 1)) * 32];
+                r.tile[(e >> 3) * 32] = make_int4((int)nl_pack2(v[0], v[1]), (int)nl_pack2(v[2], v[3]),
+                                                  (int)nl_pack2(v[4], v[5]), (int)nl_pack2(v[6], v[7]));
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int e = r.flushed + 4 * q;
+                r.tile[(e >> 2) * 32] = make_int4(r.ring[((e + 0) & (NL_STAGE - 1)) * 32], r.ring[((e + 1) & (NL_STAGE - 1)) * 32],
+                                                  r.ring[((e + 2) & (NL_STAGE - 1)) * 32], r.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+            }
         }
     }
     r.flushed += 16;
 }
 
-// Append candidate slot s to the lane's ring column if it is inside the run (u < left), inside r_list and
+// Append candidate s to the lane's ring column if it is inside the run (u < left), inside r_list and
 // (SELF) not bead i: ring[(k & (NL_STAGE-1)) * 32] = s; k += 1, with k kept as the byte offset kb = 128 k.
 // The address is (kb & mask) | lb, one LOP3 (the warp's ring is 4 KB-aligned, so the two terms share no
 // bits); store and increment are predicated on the hit (written in PTX: the compiler otherwise builds the
@@ -70,17 +108,19 @@ __device__ __forceinline__ void nl_append(uint32_t &kb, uint32_t lb, float r2, f
                        "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
 }
 
-// One run of candidates ref[s0 .. s1) against bead i, four at a time, every one predicated on s < s1 (the
-// runs of C3 hold ~9 candidates: no remainder loop, and the lanes of a warp make ceil(len / 4) trips).
+// One run of candidates ref[s0 .. s1) against bead i, TRIP at a time, every one predicated on s < s1 (the
+// runs of C3 hold ~7 candidates: no remainder loop, and the lanes of a warp make ceil(len / TRIP) trips).
+// The entry appended for candidate s is s + delta: the bead index (delta = 0), or (W16) its offset in the tile's window.
 // SHIFT: the run lies across a periodic face in some dimension; the displacement is then taken relative to
 // the two faces, (a -+ L/2) - (b +- L/2) (see gm_min_image), with the bead side (ax, ay, az) prepared once
 // per run and the candidate side b + (hx, hy, hz) per candidate.  SELF: the run holds bead i itself.
-template <int TRIP, bool SHIFT, bool SELF>
-__device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int i, float ax,
+template <int TRIP, bool SHIFT, bool SELF, bool W16>
+__device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int s0, int s1, int delta, int i, float ax,
                                             float ay, float az, float hx, float hy, float hz, float r_list2,
                                             NlRow &r)
 {
     uint32_t kb = (uint32_t)r.k * 128u;
+    const int ie = i + delta;
     for (int s = s0; s < s1; s += TRIP) {
         // loads past the end of the run stay inside the array (per-bead arrays carry >= 8 pad slots after
         // bead n - 1, GmParams::ns); what they return is masked by the `left` test
@@ -88,17 +128,163 @@ __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int 
 #pragma unroll
         for (int u = 0; u < TRIP; ++u) q[u] = __ldg(ref + s + u);
         const int left = s1 - s;
+        const int se = s + delta;
 #pragma unroll
         for (int u = 0; u < TRIP; ++u) {
             float dx, dy, dz;
             if (SHIFT) { dx = ax - (q[u].x + hx); dy = ay - (q[u].y + hy); dz = az - (q[u].z + hz); }
             else { dx = ax - q[u].x; dy = ay - q[u].y; dz = az - q[u].z; }
             const float r2 = dx * dx + dy * dy + dz * dz;
-            nl_append<SELF>(kb, r.lb, r2, r_list2, left, u, s + u, i);
+            nl_append<SELF>(kb, r.lb, r2, r_list2, left, u, se + u, ie);
         }
         // at most TRIP <= 8 new entries per trip: flush as soon as 16 are staged (ring of 32)
         r.k = (int)(kb >> 7);
-        if (r.k - r.flushed >= 16) nl_flush16(r);
+        if (r.k - r.flushed >= 16) nl_flush16<W16>(r);
+    }
+}
+
+// Window set-up of a tile (all threads of the CTA; block-level barriers inside): range slots -> rng[], descriptor ->
+// D.wdesc.  Returns 1 if the tile is window-staged (16-bit rows), 0 if it keeps 32-bit rows and the gather path.
+// Descriptor: int4 per non-empty range k = 0 .. nr-1: (first slot, window offset, length, nr | mode << 8 | total << 16);
+// a tile in mode 0 has entry 0 = (0, 0, 0, 0).
+// cell: [GM_TILE] scratch, rng: [GM_WIN_SLOTS], sh_mode: one int -- all shared by the CTA.
+__device__ __forceinline__ int nl_window(const GmParams &P, const GmDev &D, int tile, bool valid, int cx, int cy, int cz,
+                                         int4 *rng, int4 *cell, int *sh_mode, int *group_out)
+{
+    const unsigned full = 0xffffffffu;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int ncx = P.nc[0], ncy = P.nc[1], ncz = P.nc[2], sx = P.sx;
+    int4 *__restrict__ wd = D.wdesc + (size_t)tile * GM_WD_STRIDE;
+    *group_out = 0;
+    if (P.n <= P.win_cap) {                  // small system: one range, the whole array
+        if (tid == 0) wd[0] = make_int4(0, 1, P.n, 1 | (1 << 8) | (P.n << 16));
+        if (tid < GM_WIN_SLOTS) rng[tid] = make_int4(0, 1, P.n, 0);
+        __syncthreads();
+        return 1;
+    }
+    const int rowid = valid ? cz * ncy + cy : -1;
+    cell[tid] = make_int4(cx, cy, cz, rowid);
+    const int nv = __syncthreads_count(valid);                         // valid beads are threads 0 .. nv - 1, nv >= 1
+    const int4 ca = cell[0], cb = cell[nv - 1];
+    const int ok = __syncthreads_and(!valid || rowid == ca.w || rowid == cb.w);
+    const int n_a = __syncthreads_count(valid && rowid == ca.w);       // beads of row group 0 (keys ascend: group 0 first)
+    const int ngroups = n_a < nv ? 2 : 1;
+    *group_out = (valid && rowid != ca.w) ? 1 : 0;
+    if (tid < 32) {
+        // hull of each group in x cells: its first and last bead (cx ascends inside a group)
+        const int f0 = ca.x, l0 = cell[n_a - 1].x, f1 = cell[n_a < nv ? n_a : 0].x, l1 = cb.x;
+        const int y0 = ca.y, z0 = ca.z, y1 = cb.y, z1 = cb.z;
+        int st_[2], off_[2], len_[2], k_[2];
+        int total = 0, nr = 0;
+#pragma unroll
+        for (int round = 0; round < 2; ++round) {
+            const int q = round * 32 + lane;
+            int start = 0, len = 0, r0 = 0;
+            const int g = q / 27, rem = q - 27 * g, run = rem / 3, piece = rem - 3 * run;
+            if (q < GM_WIN_SLOTS && g < ngroups) {
+                const int f = g ? f1 : f0, l = g ? l1 : l0;
+                int y = (g ? y1 : y0) + (run - 3 * (run / 3)) - 1, z = (g ? z1 : z0) + run / 3 - 1;
+                y += (y < 0) ? ncy : 0; y -= (y >= ncy) ? ncy : 0;
+                z += (z < 0) ? ncz : 0; z -= (z >= ncz) ? ncz : 0;
+                r0 = (int)__ldg(D.row_rank + z * ncy + y) * ncx;
+                int c0 = 0, c1 = -1;
+                if (piece == 0) { c0 = max(f - sx, 0); c1 = min(l + sx, ncx - 1); }
+                else if (piece == 1) { if (f < sx) { c0 = ncx - (sx - f); c1 = ncx - 1; } }
+                else { if (l + sx > ncx - 1) { c0 = 0; c1 = l + sx - ncx; } }
+                if (c1 >= c0) { start = __ldg(D.cstart + r0 + c0); len = __ldg(D.cstart + r0 + c1 + 1) - start; }
+            }
+            int incl = len;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(full, incl, o);
+                if (lane >= o) incl += t;
+            }
+            const unsigned ne = __ballot_sync(full, len > 0);
+            st_[round] = start; len_[round] = len;
+            off_[round] = 1 + total + incl - len;                         // window offset 0 is the pad bead
+            k_[round] = nr + __popc(ne & ((1u << lane) - 1u));            // rank among the non-empty ranges
+            if (q < GM_WIN_SLOTS) rng[q] = make_int4(start, off_[round], len, r0);
+            total += __shfl_sync(full, incl, 31);
+            nr += __popc(ne);
+        }
+        const int mode = (ok && nr <= GM_WD_MAXR && total <= P.win_cap) ? 1 : 0;
+        if (mode) {
+            const int hdr = nr | (1 << 8) | (total << 16);
+#pragma unroll
+            for (int round = 0; round < 2; ++round)
+                if (len_[round] > 0) wd[k_[round]] = make_int4(st_[round], off_[round], len_[round], hdr);
+        } else if (lane == 0) {
+            wd[0] = make_int4(0, 0, 0, 0);
+            atomicAdd(&D.ctl->n_glob_tiles, 1);
+        }
+        if (lane == 0) *sh_mode = mode;
+    }
+    __syncthreads();
+    return *sh_mode;
+}
+
+// The nine (or, at the x faces, eighteen) runs of bead i.  WIN: the entries written are window offsets.
+template <int TRIP, bool WIN>
+__device__ __forceinline__ void nl_scan_bead(const GmParams &P, const GmDev &D, int i, const float4 pi, int cx, int cy,
+                                             int cz, const NlWin &W, NlRow &row)
+{
+    const float4 *__restrict__ ref = D.ref;
+    const int *__restrict__ cstart = D.cstart;
+    const uint32_t *__restrict__ rr = D.row_rank;
+    const int ncx = P.nc[0], ncy = P.nc[1], ncz = P.nc[2];
+    const float rl2 = P.r_list2;
+    // x pieces of a row: cells [xa0, xa1] are contiguous in ref (cells are r_list / sx wide in x, so the
+    // run reaches sx cells to either side); a bead within sx cells of a face also sees the cells
+    // [xb0, xb1] on the other side of the box
+    const int sx = P.sx;
+    const int xa0 = max(cx - sx, 0), xa1 = min(cx + sx, ncx - 1);
+    const int xb0 = (cx < sx) ? ncx - (sx - cx) : 0;
+    const int xb1 = (cx < sx) ? ncx - 1 : cx + sx - ncx;
+    const bool has_xb = cx < sx || cx + sx > ncx - 1;
+    const float hxb = (cx < sx) ? -P.half[0] : P.half[0];       // candidate side of the wrapped x piece
+    const int pb = (cx < sx) ? 1 : 2;                           // window piece of the wrapped cells: B_lo or B_hi
+    const bool inner = cx >= sx && cx + sx <= ncx - 1 && cy > 0 && cy < ncy - 1 && cz > 0 && cz < ncz - 1;
+    // bounds of the piece [c0, c1] of row r0 (bead slots) and, for WIN, d: window offset = bead slot + d
+    auto bounds = [&](int r0, int c0, int c1, int slot, int &s0, int &s1, int &d) {
+        s0 = __ldg(cstart + r0 + c0); s1 = __ldg(cstart + r0 + c1 + 1); d = 0;
+        if (WIN) {
+            const int4 g = W.rng[slot];
+            d = g.y - g.x;
+        }
+    };
+    if (inner) {
+#pragma unroll 1
+        for (int run = 0; run < 9; ++run) {
+            const int oz = run / 3 - 1, oy = run - 3 * (run / 3) - 1;
+            const int slot = W.group * 27 + run * 3;
+            const int r0 = (WIN && !W.whole) ? W.rng[slot].w : (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
+            int s0, s1, is;
+            bounds(r0, xa0, xa1, slot, s0, s1, is);
+            if (run == 4)
+                nl_scan_run<TRIP, false, true, WIN>(ref, s0, s1, is, i, pi.x, pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
+            else
+                nl_scan_run<TRIP, false, false, WIN>(ref, s0, s1, is, i, pi.x, pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
+        }
+    } else {
+#pragma unroll 1
+        for (int run = 0; run < 9; ++run) {
+            const int oz = run / 3 - 1, oy = run - 3 * (run / 3) - 1;
+            int z = cz + oz, y = cy + oy;
+            float az = pi.z, hz = 0.f, ay = pi.y, hy = 0.f;
+            if (z < 0) { z += ncz; az = pi.z + P.half[2]; hz = -P.half[2]; }
+            else if (z >= ncz) { z -= ncz; az = pi.z - P.half[2]; hz = P.half[2]; }
+            if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
+            else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
+            const int slot = W.group * 27 + run * 3;
+            const int r0 = (WIN && !W.whole) ? W.rng[slot].w : (int)__ldg(rr + z * ncy + y) * ncx;
+            int s0, s1, is;
+            bounds(r0, xa0, xa1, slot, s0, s1, is);
+            nl_scan_run<TRIP, true, true, WIN>(ref, s0, s1, is, i, pi.x, ay, az, 0.f, hy, hz, rl2, row);
+            if (has_xb) {
+                bounds(r0, xb0, xb1, slot + pb, s0, s1, is);
+                nl_scan_run<TRIP, true, true, WIN>(ref, s0, s1, is, i, pi.x - hxb, ay, az, hxb, hy, hz, rl2, row);
+            }
+        }
     }
 }
 
@@ -110,79 +296,64 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     if (!D.ctl->go) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    // [NL_WARPS][NL_STAGE][32] ints, 4 KB per warp, aligned by hand to 4 KB in the shared window (nl_ring_put
-    // ORs the entry offset into the lane's base address); the launch asks for 4 KB of slack
-    extern __shared__ int nl_ring_raw[];
-    const uint32_t raw = (uint32_t)__cvta_generic_to_shared(nl_ring_raw);
-    int *nl_ring = nl_ring_raw + (((raw + 4095u) & ~4095u) - raw) / 4;
+    // shared memory: [NL_WARPS][NL_STAGE][32] ring ints, 4 KB per warp, aligned by hand to 4 KB in the shared window
+    // (nl_append ORs the entry offset into the lane's base address; the launch asks for 4 KB of slack), then the
+    // range slots of the CTA's tile window and the scratch of its set-up
+    extern __shared__ int nl_smem_raw[];
+    const uint32_t raw = (uint32_t)__cvta_generic_to_shared(nl_smem_raw);
+    int *nl_ring = nl_smem_raw + (((raw + 4095u) & ~4095u) - raw) / 4;
+    int4 *rng = reinterpret_cast<int4 *>(nl_ring + NL_WARPS * NL_STAGE * 32);       // [GM_WIN_SLOTS], then cell[GM_TILE], mode
+    int4 *cell = rng + GM_WIN_SLOTS;
+    int *sh_mode = reinterpret_cast<int *>(cell + GM_TILE);
+    NlWin W;
+    W.rng = rng;
+    W.group = 0;
+    W.whole = P.use_win && P.n <= P.win_cap;
     NlRow row;
     row.ring = nl_ring + wid * (NL_STAGE * 32) + lane;
     row.lb = (uint32_t)__cvta_generic_to_shared(row.ring);
     row.tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
     row.k = 0; row.flushed = 0; row.cap = P.nl_cap;
     const int cap = P.nl_cap;
-    if (i < P.n) {
-        const float4 *__restrict__ ref = D.ref;
-        const int *__restrict__ cstart = D.cstart;
-        const uint32_t *__restrict__ rr = D.row_rank;
-        const float4 pi = ref[i];
-        const int cx = gm_cell_coord(pi.x, P.half[0], P.inv_w[0], P.nc[0]);
-        const int cy = gm_cell_coord(pi.y, P.half[1], P.inv_w[1], P.nc[1]);
-        const int cz = gm_cell_coord(pi.z, P.half[2], P.inv_w[2], P.nc[2]);
-        const int ncx = P.nc[0], ncy = P.nc[1], ncz = P.nc[2];
-        const float rl2 = P.r_list2;
-        // x pieces of a row: cells [xa0, xa1] are contiguous in ref (cells are r_list / sx wide in x, so the
-        // run reaches sx cells to either side); a bead within sx cells of a face also sees the cells
-        // [xb0, xb1] on the other side of the box
-        const int sx = P.sx;
-        const int xa0 = max(cx - sx, 0), xa1 = min(cx + sx, ncx - 1);
-        const int xb0 = (cx < sx) ? ncx - (sx - cx) : 0;
-        const int xb1 = (cx < sx) ? ncx - 1 : cx + sx - ncx;
-        const bool has_xb = cx < sx || cx + sx > ncx - 1;
-        const float hxb = (cx < sx) ? -P.half[0] : P.half[0];       // candidate side of the wrapped x piece
-        const bool inner = cx >= sx && cx + sx <= ncx - 1 && cy > 0 && cy < ncy - 1 && cz > 0 && cz < ncz - 1;
-        if (inner) {
-            for (int oz = -1; oz <= 1; ++oz)
-                for (int oy = -1; oy <= 1; ++oy) {
-                    const int r0 = (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
-                    if (oz == 0 && oy == 0)
-                        nl_scan_run<TRIP, false, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
-                                                 pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
-                    else
-                        nl_scan_run<TRIP, false, false>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x,
-                                                  pi.y, pi.z, 0.f, 0.f, 0.f, rl2, row);
-                }
-        } else {
-            for (int oz = -1; oz <= 1; ++oz) {
-                int z = cz + oz;
-                float az = pi.z, hz = 0.f;
-                if (z < 0) { z += ncz; az = pi.z + P.half[2]; hz = -P.half[2]; }
-                else if (z >= ncz) { z -= ncz; az = pi.z - P.half[2]; hz = P.half[2]; }
-                for (int oy = -1; oy <= 1; ++oy) {
-                    int y = cy + oy;
-                    float ay = pi.y, hy = 0.f;
-                    if (y < 0) { y += ncy; ay = pi.y + P.half[1]; hy = -P.half[1]; }
-                    else if (y >= ncy) { y -= ncy; ay = pi.y - P.half[1]; hy = P.half[1]; }
-                    const int r0 = (int)__ldg(rr + z * ncy + y) * ncx;
-                    nl_scan_run<TRIP, true, true>(ref, __ldg(cstart + r0 + xa0), __ldg(cstart + r0 + xa1 + 1), i, pi.x, ay, az,
-                                      0.f, hy, hz, rl2, row);
-                    if (has_xb)
-                        nl_scan_run<TRIP, true, true>(ref, __ldg(cstart + r0 + xb0), __ldg(cstart + r0 + xb1 + 1), i, pi.x - hxb,
-                                          ay, az, hxb, hy, hz, rl2, row);
-                }
-            }
-        }
+    const bool valid = i < P.n;
+    float4 pi = make_float4(0.f, 0.f, 0.f, 0.f);
+    int cx = 0, cy = 0, cz = 0;
+    if (valid) {
+        pi = D.ref[i];
+        cx = gm_cell_coord(pi.x, P.half[0], P.inv_w[0], P.nc[0]);
+        cy = gm_cell_coord(pi.y, P.half[1], P.inv_w[1], P.nc[1]);
+        cz = gm_cell_coord(pi.z, P.half[2], P.inv_w[2], P.nc[2]);
+    }
+    int mode = 0;
+    if (P.use_win && (int)(blockIdx.x * blockDim.x) < P.n)      // CTA-uniform: the tile holds at least one bead
+        mode = nl_window(P, D, blockIdx.x, valid, cx, cy, cz, rng, cell, sh_mode, &W.group);
+    if (valid) {
+        if (mode) nl_scan_bead<TRIP, true>(P, D, i, pi, cx, cy, cz, W, row);
+        else nl_scan_bead<TRIP, false>(P, D, i, pi, cx, cy, cz, W, row);
         if (row.k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
     }
-    // the tail of the row: whole quads, at least minq of them in all (the force kernel loads those before
-    // it knows NN), padded with the far-away bead
+    // the tail of the row: whole quads (octs), at least minq quads in all (the force kernel loads those before
+    // it knows NN), padded with the far-away bead (index n; window offset 0)
     const int kc = min(row.k, cap);
-    const int nq = max((kc + 3) >> 2, P.minq);
-    for (int e = max(kc, row.flushed); e < 4 * nq; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = P.n;
-    for (int q = row.flushed >> 2; q < nq; ++q) {
-        const int e = 4 * q;
-        row.tile[q * 32] = make_int4(row.ring[((e + 0) & (NL_STAGE - 1)) * 32], row.ring[((e + 1) & (NL_STAGE - 1)) * 32],
-                                     row.ring[((e + 2) & (NL_STAGE - 1)) * 32], row.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+    if (mode) {
+        const int no = max((kc + 7) >> 3, P.minq >> 1);
+        for (int e = max(kc, row.flushed); e < 8 * no; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = 0;
+        for (int o = row.flushed >> 3; o < no; ++o) {
+            const int e = 8 * o;
+            int v[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) v[u] = row.ring[((e + u) & (NL_STAGE - 1)) * 32];
+            row.tile[o * 32] = make_int4((int)nl_pack2(v[0], v[1]), (int)nl_pack2(v[2], v[3]),
+                                         (int)nl_pack2(v[4], v[5]), (int)nl_pack2(v[6], v[7]));
+        }
+    } else {
+        const int nq = max((kc + 3) >> 2, P.minq);
+        for (int e = max(kc, row.flushed); e < 4 * nq; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = P.n;
+        for (int q = row.flushed >> 2; q < nq; ++q) {
+            const int e = 4 * q;
+            row.tile[q * 32] = make_int4(row.ring[((e + 0) & (NL_STAGE - 1)) * 32], row.ring[((e + 1) & (NL_STAGE - 1)) * 32],
+                                         row.ring[((e + 2) & (NL_STAGE - 1)) * 32], row.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+        }
     }
     if (i < P.ns) D.nn[i] = kc;
     const int m = __reduce_max_sync(0xffffffffu, kc);
@@ -198,7 +369,9 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
 
 // a7 set-up: BL of every slot in index space from its tag-space row (the sort moved the beads).  A kernel of
 // its own (full occupancy, a dozen registers): at the end of k_nl_build the dependent blt -> rtag -> store chain
-// kept every warp's slot for two more memory latencies.
+// kept every warp's slot for two more memory latencies.  Runs after k_nl_build: a partner that lies inside the
+// window of the bead's tile is stored as a window offset (GM_BOND_LOCAL) and read from shared memory by the force
+// kernels; the others keep their bead index and are gathered.
 __global__ void __launch_bounds__(256)
 k_bl_remap(const __grid_constant__ GmParams P, GmDev D)
 {
@@ -207,21 +380,51 @@ k_bl_remap(const __grid_constant__ GmParams P, GmDev D)
     if (i >= P.n) return;
     const int sel = (int)(D.ctl->n_rebuilds & 1ull);
     const size_t ns = (size_t)P.ns;
+    const int4 *__restrict__ wd = D.wdesc + (size_t)(i / GM_TILE) * GM_WD_STRIDE;
+    const int hdr = P.use_win ? __ldg(&wd[0].w) : 0;
+    const int nr = (hdr & 0x100) ? (hdr & 0xff) : 0;
     for (int b = 0; b < P.max_bonds; ++b) {
         const int e = D.blt[sel][b * ns + i];
-        D.bl[b * ns + i] = e < 0 ? -1 : (D.rtag[e & GM_BOND_MASK] | (e & ~GM_BOND_MASK));
+        int out = -1;
+        if (e >= 0) {
+            const int j = D.rtag[e & GM_BOND_MASK];
+            out = j | (e & ~(GM_BOND_MASK | GM_BOND_LOCAL));
+            for (int r = 0; r < nr; ++r) {
+                const int4 g = __ldg(wd + r);
+                if ((unsigned)(j - g.x) < (unsigned)g.z) {
+                    out = (g.y + j - g.x) | GM_BOND_LOCAL | (e & ~(GM_BOND_MASK | GM_BOND_LOCAL));
+                    break;
+                }
+            }
+        }
+        D.bl[b * ns + i] = out;
     }
 }
 
-int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 4 == 0; }
+int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 8 == 0; }
+
+// dynamic shared memory of k_nl_build: the rings (+ 4 KB of alignment slack), the range slots and the set-up scratch
+int gm_nl_smem_bytes(const GmParams &P)
+{
+    (void)P;
+    return NL_WARPS * NL_STAGE * 32 * 4 + 4096 + (GM_WIN_SLOTS + GM_TILE + 1) * 16;
+}
+
+cudaError_t gm_nl_prepare(const GmParams &P)
+{
+    cudaError_t e = cudaFuncSetAttribute(k_nl_build<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, gm_nl_smem_bytes(P));
+    if (e == cudaSuccess)
+        e = cudaFuncSetAttribute(k_nl_build<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, gm_nl_smem_bytes(P));
+    return e;
+}
 
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     const int threads = NL_WARPS * 32;
-    if (P.max_bonds > 0) k_bl_remap<<<(P.n + 255) / 256, 256, 0, st>>>(P, D);
-    const int smem = NL_WARPS * NL_STAGE * 32 * 4 + 4096;
+    const int smem = gm_nl_smem_bytes(P);
     if (P.nl_trip == 8) k_nl_build<8><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
     else k_nl_build<4><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
+    if (P.max_bonds > 0) k_bl_remap<<<(P.n + 255) / 256, 256, 0, st>>>(P, D);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors), tags [t0, t1): nn_out[tag - t0],
@@ -237,6 +440,20 @@ k_unpack_neighbors(const __grid_constant__ GmParams P, GmDev D, int *__restrict_
     const int nn = D.nn[i];
     nn_out[t - t0] = nn;
     const int *__restrict__ tile = reinterpret_cast<const int *>(D.nl + ((size_t)(i >> 5) * P.capq) * 32 + (i & 31));
+    const int4 *__restrict__ wd = D.wdesc + (size_t)(i / GM_TILE) * GM_WD_STRIDE;
+    const int hdr = P.use_win ? wd[0].w : 0;
+    if (hdr & 0x100) {
+        // window-staged tile: 16-bit window offsets, eight per int4; offset -> range -> bead index
+        const int nr = hdr & 0xff;
+        const unsigned short *__restrict__ t16 = reinterpret_cast<const unsigned short *>(tile);
+        for (int k = 0; k < nn && k < stride; ++k) {
+            const int off = t16[(k >> 3) * 256 + (k & 7)];
+            int r = 0;
+            while (r + 1 < nr && wd[r + 1].y <= off) ++r;
+            nl_out[(long long)(t - t0) * stride + k] = tag[wd[r].x + off - wd[r].y];
+        }
+        return;
+    }
     for (int k = 0; k < nn && k < stride; ++k)
         nl_out[(long long)(t - t0) * stride + k] = tag[tile[(k >> 2) * 128 + (k & 3)]];
 }

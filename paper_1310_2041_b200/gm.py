@@ -22,11 +22,12 @@ GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_
 GM_PAIR = {"none": 0, "lj": 1, "dpd": 2}
 GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
 GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
-GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP = 1, 2, 4
+GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP, GM_FLAG_NO_WINDOWS = 1, 2, 4, 8
 
 SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_bond_params",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
+           "gm_get_tuning",
            "gm_sfc_cell_order", "gm_last_error"]
 
 
@@ -40,7 +41,7 @@ class gm_config(C.Structure):
         ("kT", C.c_float), ("gamma", C.c_float), ("lam", C.c_float),
         ("sfc_period", C.c_int32), ("nl_row_capacity", C.c_int32), ("flags", C.c_int32),
         ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
-        ("reserved", C.c_int32),
+        ("win_capacity", C.c_int32),
     ]
 
 
@@ -79,6 +80,7 @@ def lib():
         L.gm_get_particles.argtypes = [vp, vp, vp, vp, i32]
         L.gm_get_neighbors.argtypes = [vp, vp, vp, i64, i32]
         L.gm_get_stats.argtypes = [vp, vp]
+        L.gm_get_tuning.argtypes = [vp, vp]
         L.gm_sfc_cell_order.argtypes = [vp, vp]
         L.gm_last_error.argtypes = [vp]
         L.gm_last_error.restype = C.c_char_p
@@ -200,6 +202,14 @@ def gm_get_stats(h, check: bool = True) -> dict:
     d = dict(zip(keys, (int(x) for x in out)))
     d["status"] = st
     return d
+
+
+def gm_get_tuning(h) -> dict:
+    out = np.zeros(8, dtype=np.int64)
+    _check(lib().gm_get_tuning(h, out.ctypes.data), h)
+    keys = ["x_cell_div", "nl_scan_trip", "step_shape", "windows", "win_capacity", "tiles", "tiles_not_windowed",
+            "nl_smem_bytes"]
+    return dict(zip(keys, (int(x) for x in out)))
 
 
 def gm_sfc_cell_order(nc) -> np.ndarray:
@@ -328,6 +338,9 @@ class System:
         nl = np.zeros((self.n, stride), np.int32)
         gm_get_neighbors(self.h, nn, nl)
         return nn, nl
+
+    def tuning(self) -> dict:
+        return gm_get_tuning(self.h)
 
     def stats(self, check: bool = True) -> dict:
         return gm_get_stats(self.h, check)
