@@ -167,6 +167,137 @@ def describe(w) -> str:
             f"{w.bond_style} bonds, {w.integrator}, dt={w.dt}, skin={w.r_skin}, sfc_period={w.sfc_period}")
 
 
+def src_sha16() -> str:
+    """Hash of the CUDA sources: the ncu-derived figures under profiles/ carry the hash of the code they were taken
+    on and are only quoted while it still matches (otherwise the field is null)."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_1310_2041_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            with open(os.path.join(d, f), "rb") as fh:
+                h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def profile_row(config: str):
+    """Row of profiles/kernels_r02.csv for this config's step kernel, or None if absent or taken on other code."""
+    path = os.path.join(ROOT, "profiles", "kernels_r02.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    sha = src_sha16()
+    with open(path) as f:
+        for row in csv.DictReader(f):
+            if row["config"] == config and row["src_sha16"] == sha:
+                return row
+    return None
+
+
+def measure(gm, torch, w, local, stream, inner, steps, warmup, flags, tune, barrier, world, dev, clocks=None,
+            pair_samples=5):
+    """Set-up by the config's own protocol (untimed), W warm-up bench steps, exactly K timed ones (CUDA events on the
+    library's stream), then the step kernel alone (gm_step_timed) and the in-cutoff pair count averaged over
+    `pair_samples` states."""
+    import copy
+    w_run = w
+    if w.equil_steps:
+        w_run = copy.copy(w)
+        w_run.integrator = "langevin"
+    s = gm.System(w_run, device=local, flags=flags, tune=tune)
+    if w.equil_steps:
+        s.step(w.equil_steps)                   # C3: 1,000 Langevin steps (kT=1, gamma=1), then NVE
+        s.set_integrator(w.integrator, w.kT, 0.0)
+    for _ in range(warmup):
+        s.step(inner)
+    barrier()
+    st1 = s.stats()
+    if clocks is not None:
+        clocks.start()
+        time.sleep(0.05)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(steps):
+        s.step(inner)
+    e1.record(stream)
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clk = clocks.stop() if clocks is not None else {}
+    st2 = s.stats()
+    ms = max_over_ranks(ms, world, dev)
+    n_ts = steps * inner
+    rebuilds = st2["rebuilds"] - st1["rebuilds"]
+    # the dominant kernel alone: CUDA events around every launch (gm_step_timed)
+    tk = s.step_timed(min(inner, 200))
+    k_ms = tk["force_ms"] / max(1, tk["force_launches"])
+    # unique pairs inside r_cut, averaged over several states (SURVEY.md 8(d): >= 5 samples)
+    pairs, en = [], None
+    for _ in range(pair_samples):
+        s.step(max(1, min(inner, 100) // pair_samples))
+        en = s.energies()
+        pairs.append(en["n_pairs"])
+    st3 = s.stats()
+    nbar_l = st3["sum_nn"] / w.n
+    bbar = 2.0 * len(w.bonds) / w.n
+    dpd = w.pair_style == "dpd"
+    bytes_kernel = w.n * ((48 + 48 if dpd else 32 + 32) + 16 + 4 + 4 * nbar_l + 4 + 4 * bbar)
+    m_interval = n_ts / max(1, rebuilds)
+    bytes_step = bytes_kernel + w.n * (80 + 4 * nbar_l) / m_interval
+    # kernels launched inside the timed region: per timestep the gate + the fused force/integrate kernel; per rebuild
+    # keys, scan, scatter, permute (= SFC sort of all particle arrays), NL build, and with bonds the BL remap
+    launches = n_ts * 2 + rebuilds * (6 if len(w.bonds) else 5)
+    return dict(system=s, ms=ms, n_ts=n_ts, tps=whole_job_value(world, n_ts, ms), ms_ts=ms / n_ts, k_ms=k_ms,
+                rebuilds=rebuilds, reorders=st2["reorders"] - st1["reorders"], m_interval=m_interval, nbar_l=nbar_l,
+                max_nn=st3["max_nn"], sum_nn=st3["sum_nn"], pairs_in_rc=float(np.mean(pairs)), energies=en,
+                bytes_kernel=bytes_kernel, bytes_step=bytes_step, launches=int(launches), clocks=clk,
+                rebuild_ms_direct=tk["rebuild_ms"] / max(1, tk["force_launches"]), tuning=s.tuning())
+
+
+def rooflines(config, w, m, hbm_gbs, peak_src, sm_mhz):
+    """HBM roofline of the step kernel (algorithmic bytes of SURVEY.md 8(d) / CUDA-event time) and of the whole timestep,
+    plus -- from the ncu capture of the same code, profiles/kernels_r02.csv -- measured DRAM traffic, the issue-slot
+    ("alu") roofline and L2 throughput.  DESIGN.md 7 derives the peaks."""
+    k_s, ts_s = m["k_ms"] * 1e-3, m["ms_ts"] * 1e-3
+    achieved = m["bytes_kernel"] / k_s / 1e9
+    whole = m["bytes_step"] / ts_s / 1e9
+    roof = {"bound": "hbm", "kernel": "k_step (fused a4+a5/a6+a7+a8)", "achieved": achieved, "peak": hbm_gbs,
+            "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None, "peak_source": peak_src,
+            "what": "achieved = ALGORITHMIC bytes per launch / CUDA-event time of the kernel (not a DRAM counter)",
+            "kernel_ms": m["k_ms"], "algorithmic_bytes_per_launch": m["bytes_kernel"],
+            "kernel_share_of_step": m["k_ms"] / m["ms_ts"],
+            "whole_step": {"algorithmic_bytes_per_timestep": m["bytes_step"], "achieved": whole,
+                           "frac": whole / hbm_gbs, "frac_of_nominal_8TBs": whole / 8000.0},
+            "target": {"what": "whole timestep >= 0.50 of the HBM roofline (BASELINE.json north_star; C3)",
+                       "value": whole / hbm_gbs, "met": bool(whole / hbm_gbs >= 0.5)} if config == "C3" else None}
+    row = profile_row(config)
+    if row is not None:
+        traffic = float(row["dram_bytes_per_launch"])
+        tinst = float(row["thread_inst_per_launch"])
+        # issue-slot peak: 148 SMs x 4 schedulers x 1 warp instruction per clock x 32 lanes at the SM clock seen under load
+        peak_alu = 148 * 4 * 32 * sm_mhz * 1e6
+        roof["traffic"] = traffic
+        roof["dram_gbs_measured"] = traffic / k_s / 1e9
+        roof["alu"] = {"bound": "alu", "achieved": tinst / k_s / 1e12, "peak": peak_alu / 1e12,
+                       "unit": "T thread-instructions/s", "frac": tinst / k_s / peak_alu,
+                       "thread_inst_per_bead": tinst / w.n, "source": "ncu smsp__thread_inst_executed.sum, same code"}
+        roof["l2"] = {"lts_throughput_pct": float(row["lts_throughput_pct"]), "lts_hit_pct": float(row["lts_hit_pct"]),
+                      "l1_lsu_wavefronts_pct": float(row["l1_lsu_wavefronts_pct"])}
+    return roof
+
+
+def compact(name, w, m, hbm_gbs, peak_src, sm_mhz):
+    r = rooflines(name, w, m, hbm_gbs, peak_src, sm_mhz)
+    out = {"workload": describe(w), "tps": m["tps"], "ms_per_timestep": m["ms_ts"], "mean_nn": m["nbar_l"],
+           "rebuild_interval": m["m_interval"], "k_step_ms": m["k_ms"], "k_step_frac": r["frac"],
+           "whole_step_frac": r["whole_step"]["frac"], "pair_interactions_per_s": m["tps"] * m["pairs_in_rc"],
+           "timesteps": m["n_ts"], "tiles_not_windowed": m["tuning"]["tiles_not_windowed"], "tiles": m["tuning"]["tiles"]}
+    for k in ("traffic", "dram_gbs_measured", "alu", "l2"):
+        if k in r and r[k] is not None:
+            out[k] = r[k]
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -187,6 +318,8 @@ def main():
     ap.add_argument("--no-windows", action="store_true", help="GM_FLAG_NO_WINDOWS: 32-bit neighbor rows and L1/L2 gathers")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="skip the short runs of C1, C2, C4, C5 that the default C3 line carries in `configs`")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
@@ -220,82 +353,19 @@ def main():
 
     inner = args.inner or (w.sfc_period if w.sfc_period > 0 else 500)
     hbm_gbs, peak_src = load_peaks()
-
-    # ---- set-up (untimed): the config's own protocol -----------------------------------------------
-    first = "langevin" if w.equil_steps else w.integrator
-    w_run = w
-    if w.equil_steps:
-        import copy
-        w_run = copy.copy(w)
-        w_run.integrator = "langevin"
     flags = (gm.GM_FLAG_NO_COND_NODES if args.no_cond_nodes else 0) | (gm.GM_FLAG_NO_WINDOWS if args.no_windows else 0)
     tune = {k: int(v) for k, v in (kv.split("=") for kv in args.tune)}
     flags |= tune.pop("flags", 0)
-    s = gm.System(w_run, device=local, flags=flags, tune=tune)
-    if w.equil_steps:
-        s.step(w.equil_steps)                   # C3: 1,000 Langevin steps (kT=1, gamma=1), then NVE
-        s.set_integrator(w.integrator, w.kT, 0.0)
-    st0 = s.stats()
     stream = torch.cuda.current_stream(dev)
 
     # ---- device-resident throughput: W warm-up steps, then exactly K timed steps -------------------
-    for _ in range(args.warmup):
-        s.step(inner)
-    barrier()
-    st1 = s.stats()
     clocks = ClockSampler(dev)
-    clocks.start()
-    time.sleep(0.05)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        s.step(inner)
-    e1.record(stream)
-    barrier()
-    ms = e0.elapsed_time(e1)
-    clk = clocks.stop()
-    st2 = s.stats()
-    ms = max_over_ranks(ms, world, dev)
-    n_ts = args.steps * inner
-    tps = whole_job_value(world, n_ts, ms)
-    rebuilds = st2["rebuilds"] - st1["rebuilds"]
-    reorders = st2["reorders"] - st1["reorders"]
-    nbar_l = st2["sum_nn"] / w.n
-    bbar = 2.0 * len(w.bonds) / w.n
-    en = s.energies()
-    pairs_in_rc = en["n_pairs"]
-
-    # kernels launched inside the timed region: per timestep the gate + the fused force/integrate kernel;
-    # per rebuild 6 (keys, 2 scan, scatter, permute = SFC sort of all particle arrays, NL build), 7 with bonds
-    # (BL remap to the new bead indices)
-
-    launches = n_ts * 2 + rebuilds * (7 if len(w.bonds) else 6)
-
-    # ---- the dominant kernel alone: CUDA events around every launch (gm_step_timed) ----------------
-    n_prof = min(inner, 200)
-    tk = s.step_timed(n_prof)
-    k_ms = tk["force_ms"] / max(1, tk["force_launches"])
-    dpd = w.pair_style == "dpd"
-    bytes_kernel = w.n * ((48 + 48 if dpd else 32 + 32) + 16 + 4 + 4 * nbar_l + 4 + 4 * bbar)
-    m_interval = n_ts / max(1, rebuilds)
-    bytes_step = bytes_kernel + w.n * (80 + 4 * nbar_l) / m_interval
-    achieved = bytes_kernel / (k_ms * 1e-3) / 1e9
-    ms_ts = ms / n_ts
-    roof = {"bound": "hbm", "kernel": "k_step (fused a4+a5+a7+a8)", "achieved": achieved, "peak": hbm_gbs,
-            "unit": "GB/s", "frac": achieved / hbm_gbs, "traffic": None, "peak_source": peak_src,
-            "kernel_ms": k_ms, "algorithmic_bytes_per_launch": bytes_kernel,
-            "kernel_share_of_step": k_ms / ms_ts,
-            "whole_step": {"algorithmic_bytes_per_timestep": bytes_step, "achieved": bytes_step / (ms_ts * 1e-3) / 1e9,
-                           "frac": bytes_step / (ms_ts * 1e-3) / 1e9 / hbm_gbs,
-                           "frac_of_nominal_8TBs": bytes_step / (ms_ts * 1e-3) / 1e9 / 8000.0}}
-    tr = os.path.join(ROOT, "profiles", "traffic_r01.csv")      # dram bytes/launch of k_step from the ncu capture
-    if os.path.exists(tr):
-        import csv
-        with open(tr) as f:
-            for row in csv.DictReader(f):
-                if row["config"] == args.config:
-                    roof["traffic"] = float(row["dram_bytes_per_launch"])
+    m = measure(gm, torch, w, local, stream, inner, args.steps, args.warmup, flags, tune, barrier, world, dev, clocks)
+    s, ms, tps, n_ts, ms_ts, k_ms = m["system"], m["ms"], m["tps"], m["n_ts"], m["ms_ts"], m["k_ms"]
+    clk = m["clocks"]
+    sm_mhz = clk.get("sm_mhz") or clk.get("sm_max_mhz") or 1965.0
+    roof = rooflines(args.config, w, m, hbm_gbs, peak_src, sm_mhz)
+    launches = m["launches"]
 
     # ---- end to end through the C ABI with HOST buffers ---------------------------------------------
     e2e = None
@@ -309,7 +379,7 @@ def main():
         for _ in range(1):
             gm.gm_set_particles(s.h, hp, hv, ht, None); s.step(inner); gm.gm_get_particles(s.h, hp, hv, None)
         barrier()
-        t0 = time.perf_counter()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record(stream)
         for _ in range(k_e2e):
             gm.gm_set_particles(s.h, hp, hv, ht, None)      # H2D: pos, vel, type (pinned host memory)
@@ -333,29 +403,47 @@ def main():
         t1, _ = oracle_timesteps(w, 1, cores)
         k = int(max(2, min(200, 15.0 / max(t1, 1e-3))))       # about 15 s of CPU work
         tt, thr = oracle_timesteps(w, k, cores)
+        k1 = int(max(1, min(50, 5.0 / max(t1 * thr, 1e-3))))   # about 5 s more on ONE thread
+        t1t, _ = oracle_timesteps(w, k1, 1)
         cpu = {"value": k / tt, "unit": "timesteps/s", "cores": thr, "kind": "oracle",
-               "sample": f"{k} MD timesteps of {w.name} (N={w.n}) from the start state, fp64 cell-list oracle, OpenMP over beads"}
+               "sample": f"{k} MD timesteps of {w.name} (N={w.n}) from the start state, fp64 cell-list oracle, OpenMP over beads",
+               "one_thread": {"value": k1 / t1t, "unit": "timesteps/s", "cores": 1, "sample": f"{k1} MD timesteps"}}
+
+    s.close()
+    # ---- the other configs of BASELINE.json, short runs (rank 0, N=1 only): one line carries all five -------------
+    others = None
+    if rank == 0 and world == 1 and args.config == "C3" and not args.no_other_configs and args.scale is None:
+        others = {}
+        for name in ("C1", "C2", "C4", "C5"):
+            wo = make_config(name)
+            io = min(200, wo.sfc_period if wo.sfc_period > 0 else 200)
+            mo = measure(gm, torch, wo, local, stream, io, 3, 3, flags, {}, barrier, 1, dev)
+            mo["system"].close()
+            others[name] = compact(name, wo, mo, hbm_gbs, peak_src, sm_mhz)
+            del mo, wo
+            torch.cuda.empty_cache()
 
     if rank == 0:
+        en = m["energies"]
         line = {
             "metric": METRIC, "value": tps, "unit": "timesteps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": describe(w), "timesteps_per_step": inner, "parallelism": f"replicas x{world}",
                        "l2": f"no flush: successive timesteps are data-dependent; per-timestep working set "
-                             f"{(bytes_kernel + 16 * w.n) / 1e6:.0f} MB vs L2 {L2_BYTES / 1e6:.0f} MB",
+                             f"{(m['bytes_kernel'] + 16 * w.n) / 1e6:.0f} MB vs L2 {L2_BYTES / 1e6:.0f} MB",
                        "equilibration": f"{w.equil_steps} Langevin steps (untimed set-up)" if w.equil_steps else "none"},
             "ms_per_timestep": ms_ts,
-            "pair_interactions_per_s": tps * pairs_in_rc,
-            "list_entries_per_s": tps * st2["sum_nn"],
-            "pairs_in_rc": pairs_in_rc, "mean_nn": nbar_l, "max_nn": st2["max_nn"],
-            "rebuilds": rebuilds, "rebuild_interval": m_interval, "reorders": reorders,
-            "rebuild_ms_per_timestep_direct": tk["rebuild_ms"] / max(1, tk["force_launches"]),
-            "energy_per_bead": en["etot"] / w.n, "temperature": en["T"], "tuning": s.tuning(),
+            "pair_interactions_per_s": tps * m["pairs_in_rc"],
+            "list_entries_per_s": tps * m["sum_nn"],
+            "pairs_in_rc": m["pairs_in_rc"], "pairs_in_rc_samples": 5, "mean_nn": m["nbar_l"], "max_nn": m["max_nn"],
+            "rebuilds": m["rebuilds"], "rebuild_interval": m["m_interval"], "reorders": m["reorders"],
+            "rebuild_ms_per_timestep_direct": m["rebuild_ms_direct"],
+            "energy_per_bead": en["etot"] / w.n, "temperature": en["T"], "tuning": m["tuning"],
             "roofline": roof, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches), "clocks": clk,
+            "configs": others,
         }
         print(json.dumps(line))
-    s.close()
     if world > 1:
         dist.destroy_process_group()
 
