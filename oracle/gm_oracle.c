@@ -20,6 +20,9 @@
  *   - harmonic bond U = k (r - r0)^2, Eq. (7) (no 1/2)
  *   - bonds act from both ends, no exclusions
  *   - velocity-Verlet NVE / "BD" (Langevin) / GW-VV for DPD
+ *   - harmonic repulsion Eq. (2), Gaussian repulsion Eq. (3)
+ *   - tabulated pair potential: cubic spline in z = r^2, Eq. (12); F = -2 r dV/dz, Eq. (11);
+ *     cutoff = "point < Npoint", Alg. 2 lines 8-12
  *   - FENE, WCA, the DPD force law, Philox: not in PAPER.md; readings c-3..c-8:
  *     Kremer-Grest FENE, Groot-Warren DPD with uniform unit-variance noise, Philox4x32-10
  *     (Salmon et al., SC'11) keyed (seed; min tag, max tag, step, stream).
@@ -39,7 +42,7 @@
 #include <omp.h>
 #endif
 
-enum { ORC_PAIR_NONE = 0, ORC_PAIR_LJ = 1, ORC_PAIR_DPD = 2 };
+enum { ORC_PAIR_NONE = 0, ORC_PAIR_LJ = 1, ORC_PAIR_DPD = 2, ORC_PAIR_HARMONIC = 3, ORC_PAIR_GAUSS = 4, ORC_PAIR_TABLE = 5 };
 enum { ORC_BOND_NONE = 0, ORC_BOND_FENE = 1, ORC_BOND_HARMONIC = 2 };
 enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2 };
 enum { ORC_OK = 0, ORC_ERR_BOND_OVERSTRETCH = -7, ORC_ERR_ARG = -1 };
@@ -64,6 +67,11 @@ typedef struct {
     const double *mass;     /* [n] */
     int32_t use_cells;      /* 0: all pairs O(N^2) (the definition); 1: cell-list O(N) */
     int32_t n_threads;      /* OpenMP threads for the per-bead loops; <=0: library default */
+    /* ORC_PAIR_TABLE (Eqs. 11-12, Alg. 2): cubic-spline coefficients on a grid of z = r^2,       */
+    /* table[((ti * n_types + tj) * table_points + point) * 4 + {0,1,2,3}] = c0, c1, c2, c3       */
+    const double *table;
+    int32_t table_points;   /* Npoint: a pair interacts iff int(r^2 / interval) < Npoint */
+    double table_interval;
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -247,8 +255,43 @@ static int pair_term(const orc_params *p, const double *pos, const double *vel, 
     double dz = orc_min_image(pos[3 * i + 2] - pos[3 * j + 2], p->box[2]);
     double r2 = dx * dx + dy * dy + dz * dz;
     int t = p->type[i] * p->n_types + p->type[j];
+    if (p->pair_style == ORC_PAIR_TABLE) {
+        /* Alg. 2 lines 8-12: point = int(dr^2 / interval); if point < Npoint: delta = dr^2 -
+           point * interval; Eq. (12): V = c0 + c1 d + c2 d^2 + c3 d^3; Eq. (11): F = -2 r dV/dz */
+        long point = (long)(r2 / p->table_interval);
+        if (!(point < p->table_points)) return 0;
+        const double *c = p->table + ((size_t)t * p->table_points + point) * 4;
+        double d = r2 - (double)point * p->table_interval;
+        double dvdz = c[1] + 2.0 * c[2] * d + 3.0 * c[3] * d * d;
+        double fs = -2.0 * dvdz;
+        f[0] += fs * dx; f[1] += fs * dy; f[2] += fs * dz;
+        *u += c[0] + c[1] * d + c[2] * d * d + c[3] * d * d * d;
+        return 1;
+    }
     double rc = p->rc[t];
     if (!(r2 < rc * rc)) return 0;
+    if (p->pair_style == ORC_PAIR_HARMONIC) {
+        /* Eq. (2): U = alpha (1 - r/r_cut)^2 (no 1/2);  F_i = -dU/dr e = (2 alpha / r_cut) (1 - r/r_cut) e */
+        double a = p->eps[t];
+        double r = sqrt(r2);
+        double w = 1.0 - r / rc;
+        *u += a * w * w;
+        if (r > 0.0) {
+            double fs = 2.0 * a / rc * w / r;
+            f[0] += fs * dx; f[1] += fs * dy; f[2] += fs * dz;
+        }
+        return 1;
+    }
+    if (p->pair_style == ORC_PAIR_GAUSS) {
+        /* Eq. (3): U = eps exp(-1/2 (r/sigma)^2);  F_i = (eps / sigma^2) exp(-1/2 (r/sigma)^2) r_ij;
+           truncated at r_cut, energy shifted by U(r_cut) when asked (as for LJ, reading c-9) */
+        double e = p->eps[t], sig = p->sigma[t];
+        double g = e * exp(-0.5 * r2 / (sig * sig));
+        double fs = g / (sig * sig);
+        f[0] += fs * dx; f[1] += fs * dy; f[2] += fs * dz;
+        *u += g - p->ushift[t];
+        return 1;
+    }
     if (p->pair_style == ORC_PAIR_LJ) {
         /* Eq. (1): U = 4 eps [(s/r)^12 - (s/r)^6];  F_i = 24 eps / r^2 [2 (s/r)^12 - (s/r)^6] r_ij */
         double eps = p->eps[t], sig = p->sigma[t];

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gm_oracle.c")
 _LIB = os.path.join(_HERE, "libgm_oracle.so")
 
-PAIR = {"none": 0, "lj": 1, "dpd": 2}
+PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 BOND = {"none": 0, "fene": 1, "harmonic": 2}
 INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
 ORC_ERR_BOND_OVERSTRETCH = -7
@@ -44,6 +44,7 @@ class _Params(C.Structure):
         ("bond_k", C.c_void_p), ("bond_r0", C.c_void_p),
         ("type", C.c_void_p), ("mass", C.c_void_p),
         ("use_cells", C.c_int32), ("n_threads", C.c_int32),
+        ("table", C.c_void_p), ("table_points", C.c_int32), ("table_interval", C.c_double),
     ]
 
 
@@ -126,6 +127,39 @@ def neighbor_pairs(pos, box, r_list: float, use_cells: bool = False) -> np.ndarr
     return pairs[order]
 
 
+def spline_table(v, interval: float) -> np.ndarray:
+    """Eq. (12): cubic spline through the potential values v[k] = V(z_k) on the grid z_k = k *
+    interval of z = r^2, k = 0 .. Npoint (Npoint intervals).  Returns c[Npoint, 4] with V(z_k + d) = c0 + c1 d + c2 d^2
+    + c3 d^3: c0 is the value at the grid point, c1..c3 make first and second derivative continuous across the grid
+    points ("continuous up to second order").  The paper does not say how the spline ends: natural ends, V'' = 0 at
+    z_0 and z_Npoint (reading c-24).  Plain tridiagonal solve for the second derivatives M_k (the textbook
+    construction, ref. 41 of the paper), then c1 = (v[k+1] - v[k]) / h - h (2 M_k + M_{k+1}) / 6, c2 = M_k / 2,
+    c3 = (M_{k+1} - M_k) / (6 h)."""
+    v = np.asarray(v, np.float64)
+    n = len(v) - 1
+    h = float(interval)
+    M = np.zeros(n + 1)
+    if n >= 2:
+        # h/6 M_{k-1} + 2h/3 M_k + h/6 M_{k+1} = (v[k+1] - 2 v[k] + v[k-1]) / h,  k = 1 .. n-1;  M_0 = M_n = 0
+        a = np.full(n - 1, h / 6.0); b = np.full(n - 1, 2.0 * h / 3.0); c = np.full(n - 1, h / 6.0)
+        d = (v[2:] - 2.0 * v[1:-1] + v[:-2]) / h
+        for k in range(1, n - 1):               # forward elimination
+            m = a[k] / b[k - 1]
+            b[k] -= m * c[k - 1]
+            d[k] -= m * d[k - 1]
+        x = np.zeros(n - 1)
+        x[-1] = d[-1] / b[-1]
+        for k in range(n - 3, -1, -1):          # back substitution
+            x[k] = (d[k] - c[k] * x[k + 1]) / b[k]
+        M[1:n] = x
+    out = np.zeros((n, 4))
+    out[:, 0] = v[:-1]
+    out[:, 1] = (v[1:] - v[:-1]) / h - h * (2.0 * M[:-1] + M[1:]) / 6.0
+    out[:, 2] = 0.5 * M[:-1]
+    out[:, 3] = (M[1:] - M[:-1]) / (6.0 * h)
+    return out
+
+
 def lj_ushift(eps, sigma, rc):
     """Energy shift of the 'shifted' LJ of the configs: U_shift = 4 eps [(s/rc)^12 - (s/rc)^6]
     (energy only, the force is untouched; reading c-9)."""
@@ -154,11 +188,24 @@ class Oracle:
             self.rc = np.ascontiguousarray(w.pair["rc"], np.float64).reshape(nt, nt)
             self.ushift = (lj_ushift(self.eps, self.sigma, self.rc) if w.pair.get("shift", True)
                            else np.zeros((nt, nt)))
-        elif w.pair_style == "dpd":
+        elif w.pair_style in ("dpd", "harmonic"):
+            # DPD: a;  harmonic repulsion, Eq. (2): alpha
             self.eps = np.ascontiguousarray(w.pair["a"], np.float64).reshape(nt, nt)
             self.sigma = np.ones((nt, nt))
             self.rc = np.ascontiguousarray(w.pair["rc"], np.float64).reshape(nt, nt)
             self.ushift = np.zeros((nt, nt))
+        elif w.pair_style == "gauss":
+            # Eq. (3): eps exp(-r^2 / 2 sigma^2), cut at rc; shifted = minus its value at rc
+            self.eps = np.ascontiguousarray(w.pair["eps"], np.float64).reshape(nt, nt)
+            self.sigma = np.ascontiguousarray(w.pair["sigma"], np.float64).reshape(nt, nt)
+            self.rc = np.ascontiguousarray(w.pair["rc"], np.float64).reshape(nt, nt)
+            self.ushift = (self.eps * np.exp(-0.5 * (self.rc / self.sigma) ** 2) if w.pair.get("shift", True)
+                           else np.zeros((nt, nt)))
+        elif w.pair_style == "table":
+            # the fp32 coefficients the GPU is given, promoted: table[ti, tj, point, 0..3]
+            self.table = np.ascontiguousarray(w.pair["table"], np.float64).reshape(nt, nt, -1, 4)
+            self.eps = np.zeros((nt, nt)); self.sigma = np.ones((nt, nt)); self.ushift = np.zeros((nt, nt))
+            self.rc = np.ascontiguousarray(w.pair["rc"], np.float64).reshape(nt, nt)
         else:
             self.eps = np.zeros((nt, nt)); self.sigma = np.ones((nt, nt))
             self.rc = np.ones((nt, nt)); self.ushift = np.zeros((nt, nt))
@@ -188,6 +235,10 @@ class Oracle:
         P.bond_k = _p(self.bond_k).value; P.bond_r0 = _p(self.bond_r0).value
         P.type = _p(self.type).value; P.mass = _p(self.mass).value
         P.use_cells = int(use_cells); P.n_threads = int(n_threads)
+        if w.pair_style == "table":
+            P.table = _p(self.table).value
+            P.table_points = int(self.table.shape[2])
+            P.table_interval = float(np.float32(w.pair["interval"]))
         self.last = np.zeros(3)     # pe_pair, pe_bond, n_pairs_in_rc of the last force call
 
     # -- forces ---------------------------------------------------------------------------------

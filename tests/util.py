@@ -8,7 +8,7 @@ from workloads import Workload
 
 def custom(pos, box, vel=None, typ=None, bonds=None, pair_style="lj", eps=1.0, sigma=1.0, rc=2.5,
            shift=True, a=25.0, bond_style="none", k=30.0, r0=1.5, integrator="nve", dt=0.005,
-           kT=1.0, gamma=0.0, lam=0.65, r_skin=0.4, seed=7, n_types=1, mass=None) -> Workload:
+           kT=1.0, gamma=0.0, lam=0.65, r_skin=0.4, seed=7, n_types=1, mass=None, table=None, interval=None) -> Workload:
     pos = np.asarray(pos, dtype=np.float32).reshape(-1, 3)
     n = pos.shape[0]
     box = np.asarray(box, dtype=np.float32).reshape(-1)
@@ -23,7 +23,12 @@ def custom(pos, box, vel=None, typ=None, bonds=None, pair_style="lj", eps=1.0, s
         x = np.asarray(x, np.float32)
         return np.broadcast_to(x, (n_types, n_types)).copy() if x.ndim == 0 else x.reshape(n_types, n_types).copy()
 
-    if pair_style == "dpd":
+    if pair_style == "table":
+        # table: (n_types, n_types, Npoint, 4) spline coefficients on a grid of z = r^2; the cutoff is "point < Npoint"
+        tb = np.asarray(table, np.float32).reshape(n_types, n_types, -1, 4)
+        iv = float(np.float32(interval))
+        pair = dict(table=tb, interval=iv, rc=mat(np.sqrt(tb.shape[2] * iv)))
+    elif pair_style in ("dpd", "harmonic"):
         pair = dict(a=mat(a), rc=mat(rc))
     else:
         pair = dict(eps=mat(eps), sigma=mat(sigma), rc=mat(rc), shift=shift)

@@ -26,8 +26,9 @@ class Workload:
     bonds: np.ndarray          # (n_bonds,2) int32 tag pairs
     bond_type: np.ndarray      # (n_bonds,) int32
     n_types: int
-    pair_style: str            # "lj" | "dpd"
-    pair: dict                 # lj: eps,sigma,rc (n_types x n_types float32), shift (bool); dpd: a, rc
+    pair_style: str            # "lj" | "dpd" | "harmonic" | "gauss" | "table" | "none"
+    pair: dict                 # lj / gauss: eps,sigma,rc (n_types x n_types float32), shift (bool); dpd / harmonic: a, rc;
+                               # table: table (n_types, n_types, Npoint, 4) float32, interval, rc = sqrt(Npoint * interval)
     bond_style: str            # "fene" | "harmonic" | "none"
     bond: dict                 # k, r0 (per bond type, float32)   (FENE: r0 means R0)
     integrator: str            # "nve" | "langevin" | "gwvv"
@@ -165,9 +166,62 @@ CONFIGS = {
 }
 
 
-def make_config(name: str, scale: float | None = None) -> Workload:
-    """Build one of C1..C5.  `scale` (tests only) shrinks a config to a geometrically similar
-    smaller melt: KG lattice edge and DPD chain count are scaled, density and all parameters kept."""
+def make_lj_liquid(n_side: int, seed: int = BASE_SEED + 6, kT: float = 1.2) -> Workload:
+    """The paper's own LJ benchmark liquid (Fig. 4): monomers, packing fraction 0.2
+    (rho = 0.2 * 6 / pi = 0.38197 sigma^-3), dt = 0.001, r_cut = 3.0, no bonds.  N = n_side^3 beads on a simple-cubic
+    lattice with +-0.1 a jitter.  The paper gives no temperature, ensemble or buffer: kT = 1.2 (one-phase fluid at this
+    density), NVE, skin 0.4, plain cut with shifted energy (reading c-25)."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    n = n_side ** 3
+    rho = 0.2 * 6.0 / np.pi
+    L = (n / rho) ** (1.0 / 3.0)
+    a = L / n_side
+    g = np.arange(n_side, dtype=np.float64)
+    ix, iy, iz = np.meshgrid(g, g, g, indexing="ij")
+    pos = (np.stack([ix.ravel(), iy.ravel(), iz.ravel()], axis=1) + 0.5) * a - 0.5 * L
+    pos += rng.uniform(-0.1, 0.1, size=(n, 3)) * a
+    pos = pos.astype(np.float32)
+    mass = np.ones(n, dtype=np.float32)
+    vel = maxwell_velocities(rng, n, kT, mass)
+    one = np.ones((1, 1), dtype=np.float32)
+    return Workload(
+        name=f"F4LJ{n_side}", box=np.array([L, L, L], dtype=np.float32), pos=pos, vel=vel,
+        type=np.zeros(n, np.int32), mass=mass, bonds=np.zeros((0, 2), np.int32), bond_type=np.zeros(0, np.int32),
+        n_types=1, pair_style="lj", pair=dict(eps=one.copy(), sigma=one.copy(), rc=one * np.float32(3.0), shift=True),
+        bond_style="none", bond=dict(k=np.zeros(1, np.float32), r0=np.zeros(1, np.float32)),
+        integrator="nve", dt=0.001, kT=kT, gamma=0.0, r_skin=0.4, seed=seed, n_steps=10_000, sfc_period=500,
+    )
+
+
+def make_dpd_liquid(n: int, seed: int = BASE_SEED + 7) -> Workload:
+    """The paper's own DPD benchmark liquid (Fig. 4): monomers at number density 3.0, dt = 0.04,
+    r_cut = 1.0, no bonds, uniform random start.  a = 25, gamma = 4.5, kT = 1, GW-VV lambda = 0.65 as in config C4
+    (the paper names none of them; reading c-25), skin 0.6."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    L = (n / 3.0) ** (1.0 / 3.0)
+    pos = (rng.uniform(-0.5, 0.5, size=(n, 3)) * L).astype(np.float32)
+    half = np.float32(0.5 * L)
+    pos = np.where(pos >= half, pos - np.float32(L), pos).astype(np.float32)
+    mass = np.ones(n, dtype=np.float32)
+    vel = maxwell_velocities(rng, n, 1.0, mass)
+    one = np.ones((1, 1), dtype=np.float32)
+    return Workload(
+        name=f"F4DPD{n}", box=np.array([L, L, L], dtype=np.float32), pos=pos, vel=vel,
+        type=np.zeros(n, np.int32), mass=mass, bonds=np.zeros((0, 2), np.int32), bond_type=np.zeros(0, np.int32),
+        n_types=1, pair_style="dpd", pair=dict(a=one * np.float32(25.0), rc=one.copy()),
+        bond_style="none", bond=dict(k=np.zeros(1, np.float32), r0=np.zeros(1, np.float32)),
+        integrator="gwvv", dt=0.04, kT=1.0, gamma=4.5, lam=0.65, r_skin=0.6, seed=seed, n_steps=5_000, sfc_period=500,
+    )
+
+
+def make_config(name: str, scale: float | None = None, n: int | None = None) -> Workload:
+    """Build one of C1..C5, or the paper's Fig. 4 liquids "F4LJ" / "F4DPD" with about `n` beads (default 1,000,000).
+    `scale` (tests only) shrinks a config to a geometrically similar smaller melt: KG lattice edge and DPD chain
+    count are scaled, density and all parameters kept."""
+    if name == "F4LJ":
+        return make_lj_liquid(int(round((n or 1_000_000) ** (1.0 / 3.0))))
+    if name == "F4DPD":
+        return make_dpd_liquid(int(n or 1_000_000))
     c = dict(CONFIGS[name])
     seed = BASE_SEED + int(name[1])
     if c["kind"] == "kg":
