@@ -306,6 +306,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="C3")
     ap.add_argument("--scale", type=float, default=None, help="shrink the config (debugging only)")
+    ap.add_argument("--beads", type=int, default=None,
+                    help="bead count of the paper's Fig. 4 liquids (--config F4LJ | F4DPD; default 1,000,000)")
     ap.add_argument("--inner", type=int, default=0, help="MD timesteps per bench step (0: one SFC period)")
     ap.add_argument("--no-cond-nodes", action="store_true",
                     help="gate the rebuild with early-exit kernels instead of a conditional graph node "
@@ -325,7 +327,7 @@ def main():
         args.warmup = 3
 
     from workloads import make_config
-    w = make_config(args.config, scale=args.scale)
+    w = make_config(args.config, scale=args.scale, n=args.beads)
     if args.skin is not None:
         w.r_skin = float(args.skin)
     if args.impl == "reference":

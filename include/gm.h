@@ -10,6 +10,8 @@
  *                                            r_cut + r_buffer)
  *   a4 rebuild when a bead moved > skin/2
  *   a5 Lennard-Jones / WCA pair force        PAPER.md:L59-61 Eq. (1); loop shape Alg. 2
+ *      harmonic / Gaussian repulsion         PAPER.md:L63-72 Eqs. (2), (3)
+ *      tabulated pair potential              PAPER.md:L118-129 Eqs. (11)-(12), Alg. 2 L458 (cubic spline in z = r^2)
  *   a6 DPD pair force (Groot-Warren)         PAPER.md:L43, L135, L197 (law itself: ref. 24; DESIGN.md c-3)
  *   a7 bond force from the BL/BN table       PAPER.md:L97, Eq. (7) L99-101 (harmonic); FENE: DESIGN.md c-8
  *   a8 velocity-Verlet NVE / Langevin "BD" / GW-VV
@@ -59,7 +61,7 @@ enum {
     GM_ERR_NONFINITE = -8            /* a coordinate became NaN/Inf                               */
 };
 
-enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2 };
+enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2, GM_PAIR_HARMONIC = 3, GM_PAIR_GAUSS = 4, GM_PAIR_TABLE = 5 };
 enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2 };
 enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2 };
 
@@ -91,6 +93,7 @@ typedef struct {
     int32_t x_cell_div;              /* 1..8: cells are (r_cut_max + r_skin) / x_cell_div wide in x (DESIGN.md c-12)  */
     int32_t nl_scan_trip;            /* 4 or 8: candidates the neighbor search loads together                         */
     int32_t step_shape;              /* 1: one-warp CTAs (short lists), 2: CTAs of 128 (long lists)                    */
+    int32_t table_points;            /* GM_PAIR_TABLE: grid points (Npoint of Alg. 2) of every pair table; else 0       */
     int32_t win_capacity;            /* positions a tile window holds (shared memory per CTA = 16 B x this), <= 8000    */
 } gm_config;
 
@@ -122,8 +125,24 @@ gm_status gm_destroy(gm_system *s);
  *               (shift_flag != 0: the energy is shifted by U(r_cut) so that it vanishes at the
  *               cutoff; the force is never altered -- DESIGN.md c-9)
  *   GM_PAIR_DPD (DESIGN.md c-3):         n = 2: a, r_cut   (gamma and kT are global, gm_config)
+ *   GM_PAIR_HARMONIC (Eq. (2): U = alpha (1 - r/r_cut)^2):       n = 2: alpha, r_cut
+ *   GM_PAIR_GAUSS (Eq. (3): U = eps exp(-(r/sigma)^2 / 2)):      n = 4: eps, sigma, r_cut, shift_flag
  * r_cut must be <= cfg.r_cut_max.  Errors: INVALID_ARG. */
 gm_status gm_set_pair_params(gm_system *s, int ti, int tj, const float *p, int n);
+
+/* GM_PAIR_TABLE (Eqs. (11)-(12), Algorithm 2): the potential of the type pair (ti, tj) and
+ * (tj, ti) as cubic-spline coefficients on a grid of z = r^2.  c4 is a HOST array of 4 * cfg.table_points floats,
+ * c4[4 * point + {0,1,2,3}] = c0..c3 of V(z) = c0 + c1 d + c2 d^2 + c3 d^3, d = z - point * interval.  A pair
+ * interacts iff point = int(r^2 / interval) < table_points ("the judgement for ... the cutoff is done ... by checking
+ * if the index of grid point exceeds the maximum value"), so r_cut = sqrt(table_points * interval) <= cfg.r_cut_max;
+ * the force is F_i = -2 r_ij dV/dz.  Errors: INVALID_ARG, STATE (pair_style is not GM_PAIR_TABLE). */
+gm_status gm_set_pair_table(gm_system *s, int ti, int tj, float interval, const float *c4);
+
+/* Host-only utility: the spline of Eq. (12) through n_point + 1 potential values v[k] = V(k * interval) (HOST,
+ * doubles) -- c0 the value at the grid point, c1..c3 such that first and second derivative are continuous across the
+ * grid points, natural ends (V'' = 0; reading c-24).  c4_out: HOST array of 4 * n_point floats in the layout
+ * gm_set_pair_table takes.  Errors: INVALID_ARG. */
+gm_status gm_fit_pair_table(int n_point, double interval, const double *v, float *c4_out);
 
 /* Bond parameters of bond type `btype`: FENE (k, R0): U = -1/2 k R0^2 ln(1 - r^2/R0^2);
  * harmonic (k, r0): U = k (r - r0)^2 -- Eq. (7), no factor 1/2. */

@@ -50,7 +50,9 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (c->n_particles < 1 || c->n_particles >= (1ll << 27)) return GM_ERR_INVALID_ARG;
     if (c->n_types < 1 || c->n_types > GM_MAX_TYPES) return GM_ERR_INVALID_ARG;
     if (c->max_bonds_per_particle < 0 || c->max_bonds_per_particle > 16) return GM_ERR_INVALID_ARG;
-    if (c->pair_style < GM_PAIR_NONE || c->pair_style > GM_PAIR_DPD) return GM_ERR_INVALID_ARG;
+    if (c->pair_style < GM_PAIR_NONE || c->pair_style > GM_PAIR_TABLE) return GM_ERR_INVALID_ARG;
+    if (c->table_points < 0 || c->table_points > (1 << 20) || ((c->pair_style == GM_PAIR_TABLE) != (c->table_points > 0)))
+        return GM_ERR_INVALID_ARG;
     if (c->bond_style < GM_BOND_NONE || c->bond_style > GM_BOND_HARMONIC) return GM_ERR_INVALID_ARG;
     if (c->integrator < GM_NVE || c->integrator > GM_DPD_GWVV) return GM_ERR_INVALID_ARG;
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
@@ -130,7 +132,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     P->step_subw = (c->flags & GM_FLAG_STEP_SUBWARP) ? 8 : 1;
     P->capq = cap / 4;
     P->minq = std::min(4, P->capq);
-    // tile windows (gm_nlist.cu): LJ-family pair styles, one thread per bead.  A window holds the hulls of the x runs
+    // tile windows (gm_nlist.cu): every pair style but DPD (which also gathers velocities), one thread per bead.  A window holds the hulls of the x runs
     // of a tile's 128 beads in 9 (y, z) rows: 9 (128 + (2 sx + 1) beads-per-x-cell) positions for a tile inside one row;
     // tiles at a row end hold two partial hulls plus the wrapped pieces -- 1.25 x + 64 covers nearly all of them, the
     // rest keep the gather path.
@@ -140,13 +142,13 @@ static gm_status derive(const gm_config *c, GmParams *P)
         int wc = (int)(1.25 * est) + 64;
         wc = (wc + 7) / 8 * 8;
         if (c->win_capacity > 0) wc = (c->win_capacity + 7) / 8 * 8;
-        P->use_win = (c->pair_style == GM_PAIR_LJ && P->step_subw == 1 && !(c->flags & GM_FLAG_NO_WINDOWS) &&
+        P->use_win = (c->pair_style != GM_PAIR_NONE && c->pair_style != GM_PAIR_DPD && P->step_subw == 1 && !(c->flags & GM_FLAG_NO_WINDOWS) &&
                       wc <= 8000 && P->n < (1 << 27)) ? 1 : 0;
         if (P->n <= 4096 && P->use_win) wc = std::max(wc, (P->n + 7) / 8 * 8);
         P->win_cap = P->use_win ? wc : 0;
     }
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
-    for (int t = 0; t < GM_MAX_TYPES * GM_MAX_TYPES; ++t) { P->pair[t].c0 = 0.f; P->pair[t].c1 = 0.f; P->pair[t].c2 = 0.f; P->pair[t].c3 = 0.f; }
+    P->table_points = c->table_points;      // (memset above: every pair coefficient starts at 0 = no interaction)
     return GM_OK;
 }
 
@@ -176,6 +178,7 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
         d.vt[0] = (float4 *)take(n * 16); d.vt[1] = (float4 *)take(n * 16); d.svt = (float4 *)take(n * 16);
     }
     d.frc = (float4 *)take(n * 16);
+    if (P.table_points > 0) d.table = (float4 *)take((size_t)P.n_types * P.n_types * P.table_points * 16);
     d.tag[0] = (int *)take(n * 4); d.tag[1] = (int *)take(n * 4); d.rtag = (int *)take(n * 4);
     d.nn = (int *)take(n * 4);
     d.nnw = (int *)take(n / 32 * 4);
@@ -289,6 +292,7 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     s->cfg = *cfg;
     s->P = P;
     carve(P, *cfg, (char *)dev_workspace, &s->D);
+    s->P.table = s->D.table;
     s->st = (cudaStream_t)cfg->stream;
     s->use_graph = !(cfg->flags & GM_FLAG_NO_GRAPH);
     s->use_cond = !(cfg->flags & GM_FLAG_NO_COND_NODES);
@@ -349,6 +353,7 @@ extern "C" gm_status gm_set_pair_params(gm_system *s, int ti, int tj, const floa
     if (!p || ti < 0 || tj < 0 || ti >= s->P.n_types || tj >= s->P.n_types)
         return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: bad type index or NULL%s");
     GmPair c;
+    memset(&c, 0, sizeof(c));
     if (s->P.pair_style == GM_PAIR_LJ) {
         if (n != 4) return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: LJ takes eps, sigma, r_cut, shift%s");
         double eps = p[0], sig = p[1], rc = p[2];
@@ -366,6 +371,22 @@ extern "C" gm_status gm_set_pair_params(gm_system *s, int ti, int tj, const floa
         if (!(rc > 0.0) || rc > (double)s->cfg.r_cut_max * (1.0 + 1e-6))
             return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: r_cut outside (0, r_cut_max]%s");
         c.c0 = (float)(rc * rc); c.c1 = p[0]; c.c2 = (float)(1.0 / rc); c.c3 = p[1];
+    } else if (s->P.pair_style == GM_PAIR_HARMONIC) {
+        if (n != 2) return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: harmonic repulsion takes alpha, r_cut%s");
+        double rc = p[1];
+        if (!(rc > 0.0) || rc > (double)s->cfg.r_cut_max * (1.0 + 1e-6))
+            return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: r_cut outside (0, r_cut_max]%s");
+        c.c0 = (float)(rc * rc); c.c1 = (float)(2.0 * (double)p[0] / rc); c.c2 = (float)(1.0 / rc); c.c3 = p[0];
+    } else if (s->P.pair_style == GM_PAIR_GAUSS) {
+        if (n != 4) return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: Gaussian repulsion takes eps, sigma, r_cut, shift%s");
+        double eps = p[0], sig = p[1], rc = p[2];
+        if (!(rc > 0.0) || rc > (double)s->cfg.r_cut_max * (1.0 + 1e-6) || !(sig > 0.0))
+            return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_params: r_cut outside (0, r_cut_max] or sigma <= 0%s");
+        c.c0 = (float)(rc * rc); c.c1 = (float)(eps / (sig * sig)); c.c2 = (float)(-0.5 / (sig * sig));
+        c.c3 = (p[3] != 0.f) ? (float)(eps * std::exp(-0.5 * rc * rc / (sig * sig))) : 0.f;
+        c.c4 = p[0];
+    } else if (s->P.pair_style == GM_PAIR_TABLE) {
+        return fail(s, GM_ERR_STATE, "gm_set_pair_params: tables are set with gm_set_pair_table%s");
     } else {
         return fail(s, GM_ERR_STATE, "gm_set_pair_params: pair_style is GM_PAIR_NONE%s");
     }
@@ -373,6 +394,61 @@ extern "C" gm_status gm_set_pair_params(gm_system *s, int ti, int tj, const floa
     s->P.pair[tj * s->P.n_types + ti] = c;
     s->force_current = false;
     drop_graphs(s);     // kernel parameters are baked into the graphs
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_pair_table(gm_system *s, int ti, int tj, float interval, const float *c4)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (s->P.pair_style != GM_PAIR_TABLE) return fail(s, GM_ERR_STATE, "gm_set_pair_table: pair_style is not GM_PAIR_TABLE%s");
+    if (!c4 || ti < 0 || tj < 0 || ti >= s->P.n_types || tj >= s->P.n_types || !(interval > 0.f))
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_table: bad type index, interval or NULL%s");
+    const int np = s->P.table_points;
+    const double zc = (double)np * (double)interval;
+    if (std::sqrt(zc) > (double)s->cfg.r_cut_max * (1.0 + 1e-6))
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_pair_table: sqrt(table_points * interval) exceeds r_cut_max%s");
+    CU(cudaSetDevice(s->cfg.device));
+    const int pairs[2] = { ti * s->P.n_types + tj, tj * s->P.n_types + ti };
+    for (int q = 0; q < (ti == tj ? 1 : 2); ++q) {
+        CU(cudaMemcpyAsync(s->D.table + (size_t)pairs[q] * np, c4, (size_t)np * 16, cudaMemcpyHostToDevice, s->st));
+        GmPair c;
+        memset(&c, 0, sizeof(c));
+        c.c0 = (float)zc; c.c1 = (float)(1.0 / (double)interval); c.c2 = interval;
+        const int off = pairs[q] * np;
+        memcpy(&c.c4, &off, sizeof(int));
+        s->P.pair[pairs[q]] = c;
+    }
+    CU(cudaStreamSynchronize(s->st));              // the caller may reuse c4 at once
+    s->force_current = false;
+    drop_graphs(s);
+    return GM_OK;
+}
+
+// Eq. (12): natural cubic spline through v[k] = V(k * interval), k = 0 .. n_point (Thomas algorithm for the second
+// derivatives m_k; m_0 = m_n = 0), as coefficients of powers of d = z - z_k.
+extern "C" gm_status gm_fit_pair_table(int n_point, double interval, const double *v, float *c4_out)
+{
+    if (n_point < 1 || !(interval > 0.0) || !v || !c4_out) return GM_ERR_INVALID_ARG;
+    const int n = n_point;
+    const double h = interval;
+    std::vector<double> m((size_t)n + 1, 0.0);
+    if (n >= 2) {
+        // m_{k-1} + 4 m_k + m_{k+1} = 6 (v_{k+1} - 2 v_k + v_{k-1}) / h^2, k = 1 .. n-1
+        std::vector<double> cp((size_t)n, 0.0), dp((size_t)n, 0.0);
+        for (int k = 1; k < n; ++k) {
+            const double rhs = 6.0 * (v[k + 1] - 2.0 * v[k] + v[k - 1]) / (h * h);
+            const double den = 4.0 - cp[k - 1];
+            cp[k] = 1.0 / den;
+            dp[k] = (rhs - dp[k - 1]) / den;
+        }
+        for (int k = n - 1; k >= 1; --k) m[k] = dp[k] - cp[k] * m[k + 1];
+    }
+    for (int k = 0; k < n; ++k) {
+        c4_out[4 * k + 0] = (float)v[k];
+        c4_out[4 * k + 1] = (float)((v[k + 1] - v[k]) / h - h * (2.0 * m[k] + m[k + 1]) / 6.0);
+        c4_out[4 * k + 2] = (float)(0.5 * m[k]);
+        c4_out[4 * k + 3] = (float)((m[k + 1] - m[k]) / (6.0 * h));
+    }
     return GM_OK;
 }
 

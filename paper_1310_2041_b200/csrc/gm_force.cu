@@ -94,6 +94,42 @@ __device__ __forceinline__ void pair_term(const GmParams &P, const Own &me, cons
             pe += in ? r6i * (c.c1 * (1.0f / 12.0f) * r6i - c.c2 * (1.0f / 6.0f)) - c.c3 : 0.0f;
             cnt += in ? 1.0f : 0.0f;
         }
+    } else if (PAIR == GM_PAIR_HARMONIC) {
+        // Eq. (2): U = alpha (1 - r/r_c)^2;  F_i = (2 alpha / r_c) (1 - r/r_c) r_ij / r
+        const bool in = r2 < c.c0;
+        const float ri = rsqrtf(fmaxf(r2, 1e-30f));          // coincident beads: r_ij = 0, no force (as the oracle)
+        const float w = 1.0f - r2 * ri * c.c2;
+        const float fs = in ? c.c1 * w * ri : 0.0f;
+        fx += fs * dx; fy += fs * dy; fz += fs * dz;
+        if (ENERGY) {
+            pe += in ? c.c3 * w * w : 0.0f;
+            cnt += in ? 1.0f : 0.0f;
+        }
+    } else if (PAIR == GM_PAIR_GAUSS) {
+        // Eq. (3): U = eps exp(-r^2 / 2 sigma^2);  F_i = (eps / sigma^2) exp(-r^2 / 2 sigma^2) r_ij
+        const bool in = r2 < c.c0;
+        const float g = __expf(c.c2 * fminf(r2, c.c0));
+        const float fs = in ? c.c1 * g : 0.0f;
+        fx += fs * dx; fy += fs * dy; fz += fs * dz;
+        if (ENERGY) {
+            pe += in ? c.c4 * g - c.c3 : 0.0f;
+            cnt += in ? 1.0f : 0.0f;
+        }
+    } else if (PAIR == GM_PAIR_TABLE) {
+        // Algorithm 2 lines 8-12: point = int(dr^2 / interval); if point < Npoint: delta = dr^2 - point *
+        // interval; Eq. (12) V = c0 + c1 d + c2 d^2 + c3 d^3; Eq. (11) F_i = -2 r_ij dV/dz.  The coefficients come
+        // through the read-only path (L1/L2-resident: the paper's texture fetch of line 10).
+        if (r2 < c.c0) {
+            const int point = min((int)(r2 * c.c1), P.table_points - 1);
+            const float4 k = __ldg(P.table + __float_as_int(c.c4) + point);
+            const float d = r2 - (float)point * c.c2;
+            const float fs = -2.0f * (k.y + d * (2.0f * k.z + 3.0f * k.w * d));
+            fx += fs * dx; fy += fs * dy; fz += fs * dz;
+            if (ENERGY) {
+                pe += k.x + d * (k.y + d * (k.z + d * k.w));
+                cnt += 1.0f;
+            }
+        }
     } else if (PAIR == GM_PAIR_DPD) {
         if (r2 < c.c0) {
             if (ENERGY) cnt += 1.0f;
@@ -760,10 +796,12 @@ static void launch_force_t(const GmParams &P, const GmDev &D, int mode, int pari
     int nb = (P.n + FORCE_BLOCK - 1) / FORCE_BLOCK;
     const int wb = gm_win_bytes(P);
     if (mode == GM_MODE_STEP) {
-        if (P.step_subw == 8 && PAIR != GM_PAIR_NONE) {
-            const long long nt = (long long)P.n * 8;
-            k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + SUB_BLOCK - 1) / SUB_BLOCK), SUB_BLOCK, 0, st>>>(
-                P, D, parity, kick, kick_vt);
+        if (P.step_subw == 8 && (PAIR == GM_PAIR_LJ || PAIR == GM_PAIR_DPD)) {
+            if constexpr (PAIR == GM_PAIR_LJ || PAIR == GM_PAIR_DPD) {
+                const long long nt = (long long)P.n * 8;
+                k_step_sub<PAIR, NT1, BOND, 8><<<(unsigned)((nt + SUB_BLOCK - 1) / SUB_BLOCK), SUB_BLOCK, 0, st>>>(
+                    P, D, parity, kick, kick_vt);
+            }
         } else if (P.step_wide || PAIR == GM_PAIR_DPD) {
             allow_smem(k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, WIDE_NQ>, wb);
             k_step<PAIR, NT1, BOND, WIDE_BLOCK, WIDE_MINB, WIDE_NQ><<<(P.n + WIDE_BLOCK - 1) / WIDE_BLOCK, WIDE_BLOCK, wb, st>>>(
@@ -811,6 +849,18 @@ void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, fl
     case GM_PAIR_DPD:
         if (nt1) launch_force_b<GM_PAIR_DPD, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
         else launch_force_b<GM_PAIR_DPD, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        break;
+    case GM_PAIR_HARMONIC:
+        if (nt1) launch_force_b<GM_PAIR_HARMONIC, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_b<GM_PAIR_HARMONIC, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        break;
+    case GM_PAIR_GAUSS:
+        if (nt1) launch_force_b<GM_PAIR_GAUSS, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_b<GM_PAIR_GAUSS, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        break;
+    case GM_PAIR_TABLE:
+        if (nt1) launch_force_b<GM_PAIR_TABLE, true>(P, D, mode, parity, kick, kick_vt, lagged, st);
+        else launch_force_b<GM_PAIR_TABLE, false>(P, D, mode, parity, kick, kick_vt, lagged, st);
         break;
     default:
         launch_force_b<GM_PAIR_NONE, true>(P, D, mode, parity, kick, kick_vt, lagged, st);

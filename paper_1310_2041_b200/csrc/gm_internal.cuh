@@ -60,9 +60,13 @@ struct GmCtl {
     int n_glob_tiles;              // tiles of the current list that are NOT window-staged (32-bit rows, gathers from HBM/L2)
 };
 
-// Per-type-pair coefficients.  LJ: c0 = r_c^2, c1 = 48 eps sigma^12, c2 = 24 eps sigma^6, c3 = U_shift.
-//                              DPD: c0 = r_c^2, c1 = a, c2 = 1/r_c, c3 = r_c.
-struct GmPair { float c0, c1, c2, c3; };
+// Per-type-pair coefficients.  LJ:       c0 = r_c^2, c1 = 48 eps sigma^12, c2 = 24 eps sigma^6, c3 = U_shift.
+//                              DPD:      c0 = r_c^2, c1 = a, c2 = 1/r_c, c3 = r_c.
+//                              harmonic: c0 = r_c^2, c1 = 2 alpha / r_c, c2 = 1/r_c, c3 = alpha           (Eq. 2)
+//                              Gauss:    c0 = r_c^2, c1 = eps / sigma^2, c2 = -1/(2 sigma^2), c3 = U_shift, c4 = eps   (Eq. 3)
+//                              table:    c0 = Npoint * interval (z at the cutoff), c1 = 1 / interval, c2 = interval,
+//                                        c4 = index of the pair's first grid point in GmParams::table (int bits)   (Eqs. 11-12)
+struct GmPair { float c0, c1, c2, c3, c4, c5, c6, c7; };
 
 // Constants of one system, passed to kernels by value (constant bank).
 struct GmParams {
@@ -89,6 +93,8 @@ struct GmParams {
     GmPair pair[GM_MAX_TYPES * GM_MAX_TYPES];
     float bond_k[GM_MAX_BOND_TYPES], bond_r0[GM_MAX_BOND_TYPES];
     float bond_c[GM_MAX_BOND_TYPES];   // FENE: 1 / R0^2
+    const float4 *table;               // GM_PAIR_TABLE: (c0, c1, c2, c3) per grid point, n_types^2 tables of table_points
+    int table_points;
 };
 
 // Device pointers.
@@ -98,6 +104,7 @@ struct GmDev {
     float4 *vel, *svel;
     float4 *vt[2], *svt;
     float4 *frc;
+    float4 *table;           // GM_PAIR_TABLE: spline coefficients, [n_types^2][table_points]
     int *tag[2], *rtag;
     int *nn, *nnw;
     int4 *nl;

@@ -19,12 +19,13 @@ LIB_PATH = os.path.join(_HERE, "libgm.so")
 GM_OK = 0
 GM_ERR_INVALID_ARG, GM_ERR_STATE, GM_ERR_CUDA, GM_ERR_WORKSPACE_TOO_SMALL = -1, -2, -3, -4
 GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_NONFINITE = -5, -6, -7, -8
-GM_PAIR = {"none": 0, "lj": 1, "dpd": 2}
+GM_PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
 GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
 GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP, GM_FLAG_NO_WINDOWS = 1, 2, 4, 8
 
-SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_bond_params",
+SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_pair_table", "gm_fit_pair_table",
+           "gm_set_bond_params",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
            "gm_get_tuning",
@@ -41,7 +42,7 @@ class gm_config(C.Structure):
         ("kT", C.c_float), ("gamma", C.c_float), ("lam", C.c_float),
         ("sfc_period", C.c_int32), ("nl_row_capacity", C.c_int32), ("flags", C.c_int32),
         ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
-        ("win_capacity", C.c_int32),
+        ("table_points", C.c_int32), ("win_capacity", C.c_int32),
     ]
 
 
@@ -67,6 +68,8 @@ def lib():
         L.gm_create.argtypes = [C.POINTER(gm_config), vp, C.c_size_t, C.POINTER(vp)]
         L.gm_destroy.argtypes = [vp]
         L.gm_set_pair_params.argtypes = [vp, i32, i32, vp, i32]
+        L.gm_set_pair_table.argtypes = [vp, i32, i32, C.c_float, vp]
+        L.gm_fit_pair_table.argtypes = [i32, C.c_double, vp, vp]
         L.gm_set_bond_params.argtypes = [vp, i32, C.c_float, C.c_float]
         L.gm_set_particles.argtypes = [vp, vp, vp, vp, vp, i32]
         L.gm_set_bonds.argtypes = [vp, i64, vp, vp, i32]
@@ -134,6 +137,19 @@ def gm_destroy(h):
 def gm_set_pair_params(h, ti: int, tj: int, p):
     p = np.ascontiguousarray(p, dtype=np.float32)
     _check(lib().gm_set_pair_params(h, ti, tj, p.ctypes.data, p.size), h)
+
+
+def gm_set_pair_table(h, ti: int, tj: int, interval: float, c4):
+    c4 = np.ascontiguousarray(c4, dtype=np.float32)
+    _check(lib().gm_set_pair_table(h, ti, tj, interval, c4.ctypes.data), h)
+
+
+def gm_fit_pair_table(v, interval: float) -> np.ndarray:
+    """Spline coefficients (Npoint, 4) float32 through the Npoint + 1 potential values v on the grid z = k * interval."""
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    out = np.zeros((len(v) - 1, 4), dtype=np.float32)
+    _check(lib().gm_fit_pair_table(len(v) - 1, float(interval), v.ctypes.data, out.ctypes.data))
+    return out
 
 
 def gm_set_bond_params(h, btype: int, k: float, r0: float):
@@ -252,6 +268,7 @@ class System:
             cfg.box[d] = float(w.box[d])
         pair = w.pair
         cfg.r_cut_max = float(np.max(pair["rc"])) if w.pair_style != "none" else 1.0
+        cfg.table_points = int(pair["table"].shape[2]) if w.pair_style == "table" else 0
         cfg.r_skin = float(w.r_skin)
         cfg.dt = float(w.dt)
         cfg.seed = int(w.seed)
@@ -277,8 +294,13 @@ class System:
                 if w.pair_style == "lj":
                     gm_set_pair_params(self.h, ti, tj, [pair["eps"][ti][tj], pair["sigma"][ti][tj],
                                                         pair["rc"][ti][tj], 1.0 if pair.get("shift", True) else 0.0])
-                elif w.pair_style == "dpd":
+                elif w.pair_style in ("dpd", "harmonic"):
                     gm_set_pair_params(self.h, ti, tj, [pair["a"][ti][tj], pair["rc"][ti][tj]])
+                elif w.pair_style == "gauss":
+                    gm_set_pair_params(self.h, ti, tj, [pair["eps"][ti][tj], pair["sigma"][ti][tj],
+                                                        pair["rc"][ti][tj], 1.0 if pair.get("shift", True) else 0.0])
+                elif w.pair_style == "table":
+                    gm_set_pair_table(self.h, ti, tj, float(pair["interval"]), pair["table"][ti][tj])
         if cfg.bond_style:
             for bt in range(len(w.bond["k"])):
                 gm_set_bond_params(self.h, bt, float(w.bond["k"][bt]), float(w.bond["r0"][bt]))
