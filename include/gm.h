@@ -95,6 +95,8 @@ typedef struct {
     int32_t step_shape;              /* 1: one-warp CTAs (short lists), 2: CTAs of 128 (long lists)                    */
     int32_t table_points;            /* GM_PAIR_TABLE: grid points (Npoint of Alg. 2) of every pair table; else 0       */
     int32_t win_capacity;            /* positions a tile window holds (shared memory per CTA = 16 B x this), <= 8000    */
+    int32_t tile_windows;            /* 1: stage tile windows whatever the list length, 2: never (0: lists of >= 40)     */
+    int32_t reserved;                /* must be 0                                                                      */
 } gm_config;
 
 enum {

@@ -58,7 +58,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
-        c->step_shape < 0 || c->step_shape > 2 || c->win_capacity < 0 || c->win_capacity > 8000)
+        c->step_shape < 0 || c->step_shape > 2 || c->win_capacity < 0 || c->win_capacity > 8000 || c->tile_windows < 0 || c->tile_windows > 2 || c->reserved != 0)
         return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
     P->ns = (P->n + 8 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+7 (at least): far-away pad beads
@@ -142,20 +142,19 @@ static gm_status derive(const gm_config *c, GmParams *P)
         int wc = (int)(1.25 * est) + 64;
         wc = (wc + 7) / 8 * 8;
         if (c->win_capacity > 0) wc = (c->win_capacity + 7) / 8 * 8;
-        P->use_win = (c->pair_style != GM_PAIR_NONE && c->pair_style != GM_PAIR_DPD && P->step_subw == 1 && !(c->flags & GM_FLAG_NO_WINDOWS) &&
-                      wc <= 8000 && P->n < (1 << 27)) ? 1 : 0;
+        // Measured (same-box A/B against the gather path): windows pay for long lists -- C5 (n_l 92) 2148 ->
+        // 1970 us per timestep, C2 (88) 37.2 -> 34.5 -- and cost a little for short ones (C3, n_l 13.5: the step kernel
+        // gains 0.3 us, the rebuild loses 3), so they are chosen by the estimated list length; tile_windows overrides.
+        const double nbar_w = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
+        const bool can = c->pair_style != GM_PAIR_NONE && c->pair_style != GM_PAIR_DPD && P->step_subw == 1 &&
+                         !(c->flags & GM_FLAG_NO_WINDOWS) && wc <= 8000;
+        P->use_win = (can && c->tile_windows != 2 && (c->tile_windows == 1 || nbar_w >= 40.0)) ? 1 : 0;
         if (P->n <= 4096 && P->use_win) wc = std::max(wc, (P->n + 7) / 8 * 8);
         P->win_cap = P->use_win ? wc : 0;
     }
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
     P->table_points = c->table_points;      // (memset above: every pair coefficient starts at 0 = no interaction)
     return GM_OK;
-}
-
-static size_t scan_state_bytes(const GmParams &P)
-{
-    const size_t per = (size_t)GM_SCAN_BLOCK * GM_SCAN_ITEMS;
-    return (((size_t)P.n_cells + 1 + per - 1) / per + 1) * 8;
 }
 
 // ---- workspace layout: one pass with base == nullptr sizes it, a second pass assigns pointers ------
@@ -192,8 +191,7 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     d.cstart = (int *)take(((size_t)P.n_cells + 1 + 4) * 4);
     d.ccount = (int *)take(((size_t)P.n_cells + 1 + 4) * 4);
     size_t per = (size_t)GM_SCAN_BLOCK * GM_SCAN_ITEMS;
-    d.scan_state = (unsigned long long *)take(scan_state_bytes(P));
-    d.scan_ticket = (int *)take(4);
+    d.scan_sums = (int *)take((((size_t)P.n_cells + 1 + per - 1) / per + 1) * 4);
     d.row_rank = (uint32_t *)take((size_t)P.nc[1] * P.nc[2] * 4);
     d.stage = (float *)take(n * 4 * 11);
     d.esum = (double *)take(((size_t)GM_ESUM_BLOCKS + 1) * 8 * sizeof(double));
@@ -308,7 +306,6 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
         if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
     }
     if (e == cudaSuccess) e = cudaMemsetAsync(s->D.ccount, 0, ((size_t)P.n_cells + 1 + 4) * 4, s->st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(s->D.scan_state, 0, scan_state_bytes(P), s->st);
     if (e == cudaSuccess && P.max_bonds > 0) {
         const size_t bb = (size_t)P.ns * 4 * (size_t)P.max_bonds;       // -1 everywhere: no bonds
         e = cudaMemsetAsync(s->D.bl, 0xFF, bb, s->st);
@@ -486,7 +483,6 @@ extern "C" gm_status gm_set_particles(gm_system *s, const float *pos3, const flo
     }
     s->cur = 0;
     gm_launch_set_ctl(s->D, 0, 1, 0, s->st);             // clears the latched device errors: before the pack
-    CU(cudaMemsetAsync(s->D.scan_state, 0, scan_state_bytes(s->P), s->st));   // the rebuild counter (scan epoch) restarts
     gm_launch_pack(s->P, s->D, 0, dp, dv, dt, dm, s->st);
     CU(cudaGetLastError());
     s->step = 0;

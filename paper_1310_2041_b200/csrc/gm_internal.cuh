@@ -114,8 +114,7 @@ struct GmDev {
     int4 *wdesc;             // [n_tiles * GM_WD_STRIDE] tile window descriptors (see gm_nlist.cu)
     int *key, *rank, *sorted;
     int *cstart, *ccount;
-    unsigned long long *scan_state;   // per scan tile: value | (epoch << 2 | status) << 32 (k_scan)
-    int *scan_ticket;
+    int *scan_sums;          // per scan block
     uint32_t *row_rank;      // SFC rank of each (y, z) row of cells
     float *stage;            // 11 ns floats: I/O staging (pos3, vel3, force3, type, mass)
     double *esum;            // [GM_ESUM_BLOCKS * 8] partials, then [8] totals at the end

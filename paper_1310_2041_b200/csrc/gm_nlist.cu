@@ -289,8 +289,10 @@ __device__ __forceinline__ void nl_scan_bead(const GmParams &P, const GmDev &D, 
 }
 
 // TRIP: candidates loaded together (4: runs of ~10 candidates, C1/C3; 8: runs of 20 and more, C2/C4/C5)
-template <int TRIP>
-__global__ void __launch_bounds__(NL_WARPS * 32)
+// WINS: the system uses tile windows (GmParams::use_win) -- compiled apart so that systems without them (DPD) run the
+// plain kernel (56 registers, 9 CTAs per SM)
+template <int TRIP, bool WINS>
+__global__ void __launch_bounds__(NL_WARPS * 32, WINS ? 8 : 9)
 k_nl_build(const __grid_constant__ GmParams P, GmDev D)
 {
     if (!D.ctl->go) return;
@@ -308,7 +310,7 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     NlWin W;
     W.rng = rng;
     W.group = 0;
-    W.whole = P.use_win && P.n <= P.win_cap;
+    W.whole = WINS && P.n <= P.win_cap;
     NlRow row;
     row.ring = nl_ring + wid * (NL_STAGE * 32) + lane;
     row.lb = (uint32_t)__cvta_generic_to_shared(row.ring);
@@ -325,17 +327,17 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
         cz = gm_cell_coord(pi.z, P.half[2], P.inv_w[2], P.nc[2]);
     }
     int mode = 0;
-    if (P.use_win && (int)(blockIdx.x * blockDim.x) < P.n)      // CTA-uniform: the tile holds at least one bead
+    if (WINS && (int)(blockIdx.x * blockDim.x) < P.n)           // CTA-uniform: the tile holds at least one bead
         mode = nl_window(P, D, blockIdx.x, valid, cx, cy, cz, rng, cell, sh_mode, &W.group);
     if (valid) {
-        if (mode) nl_scan_bead<TRIP, true>(P, D, i, pi, cx, cy, cz, W, row);
+        if (WINS && mode) nl_scan_bead<TRIP, true>(P, D, i, pi, cx, cy, cz, W, row);
         else nl_scan_bead<TRIP, false>(P, D, i, pi, cx, cy, cz, W, row);
         if (row.k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
     }
     // the tail of the row: whole quads (octs), at least minq quads in all (the force kernel loads those before
     // it knows NN), padded with the far-away bead (index n; window offset 0)
     const int kc = min(row.k, cap);
-    if (mode) {
+    if (WINS && mode) {
         const int no = max((kc + 7) >> 3, P.minq >> 1);
         for (int e = max(kc, row.flushed); e < 8 * no; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = 0;
         for (int o = row.flushed >> 3; o < no; ++o) {
@@ -389,10 +391,18 @@ k_bl_remap(const __grid_constant__ GmParams P, GmDev D)
         if (e >= 0) {
             const int j = D.rtag[e & GM_BOND_MASK];
             out = j | (e & ~(GM_BOND_MASK | GM_BOND_LOCAL));
-            for (int r = 0; r < nr; ++r) {
-                const int4 g = __ldg(wd + r);
-                if ((unsigned)(j - g.x) < (unsigned)g.z) {
-                    out = (g.y + j - g.x) | GM_BOND_LOCAL | (e & ~(GM_BOND_MASK | GM_BOND_LOCAL));
+            // the tile's ranges four at a time (independent loads; entries past nr are stale but inside the
+            // descriptor's GM_WD_STRIDE slots and masked)
+            for (int r = 0; r < nr; r += 4) {
+                int4 g[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) g[u] = __ldg(wd + r + u);
+                int off = -1;
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+                    if (r + u < nr && (unsigned)(j - g[u].x) < (unsigned)g[u].z) off = g[u].y + j - g[u].x;
+                if (off >= 0) {
+                    out = off | GM_BOND_LOCAL | (e & ~(GM_BOND_MASK | GM_BOND_LOCAL));
                     break;
                 }
             }
@@ -412,19 +422,26 @@ int gm_nl_smem_bytes(const GmParams &P)
 
 cudaError_t gm_nl_prepare(const GmParams &P)
 {
-    cudaError_t e = cudaFuncSetAttribute(k_nl_build<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, gm_nl_smem_bytes(P));
-    if (e == cudaSuccess)
-        e = cudaFuncSetAttribute(k_nl_build<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, gm_nl_smem_bytes(P));
-    return e;
+    (void)P;            // 23 KB of dynamic shared memory: below the 48 KB that need an opt-in
+    return cudaSuccess;
 }
 
 void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st)
 {
     const int threads = NL_WARPS * 32;
     const int smem = gm_nl_smem_bytes(P);
-    if (P.nl_trip == 8) k_nl_build<8><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
-    else k_nl_build<4><<<(P.ns + threads - 1) / threads, threads, smem, st>>>(P, D);
-    if (P.max_bonds > 0) k_bl_remap<<<(P.n + 255) / 256, 256, 0, st>>>(P, D);
+    const int nb = (P.ns + threads - 1) / threads;
+    // BL remap: needs the window descriptors of this build on window-staged systems, so it follows the build there;
+    // otherwise it goes first (the order measured best in round 1)
+    if (P.max_bonds > 0 && !P.use_win) k_bl_remap<<<(P.n + 255) / 256, 256, 0, st>>>(P, D);
+    if (P.use_win) {
+        if (P.nl_trip == 8) k_nl_build<8, true><<<nb, threads, smem, st>>>(P, D);
+        else k_nl_build<4, true><<<nb, threads, smem, st>>>(P, D);
+    } else {
+        if (P.nl_trip == 8) k_nl_build<8, false><<<nb, threads, smem, st>>>(P, D);
+        else k_nl_build<4, false><<<nb, threads, smem, st>>>(P, D);
+    }
+    if (P.max_bonds > 0 && P.use_win) k_bl_remap<<<(P.n + 255) / 256, 256, 0, st>>>(P, D);
 }
 
 // Neighbor list in tag space for the boundary (gm_get_neighbors), tags [t0, t1): nn_out[tag - t0],

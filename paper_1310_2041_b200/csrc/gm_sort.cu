@@ -14,8 +14,8 @@
 // Within a cell, beads are ordered by their previous slot, so the result (and with it every fp32 sum
 // downstream) is the same on every run whatever order the histogram atomics were served in.
 //
-// Chain: k_gate (decide, publish ctl->go) -> k_keys (key + histogram) -> k_scan
-// (single-pass exclusive scan -> cstart) -> k_scatter (slot lists per cell) -> k_permute (canonical slot, move state)
+// Chain: k_gate (decide, publish ctl->go) -> k_keys (key + histogram) -> k_scan_local / k_scan_add
+// (exclusive scan -> cstart) -> k_scatter (slot lists per cell) -> k_permute (canonical slot, move state)
 // -> k_bl_remap, k_nl_build (gm_nlist.cu).
 #include "gm_internal.cuh"
 
@@ -57,7 +57,6 @@ k_keys(const __grid_constant__ GmParams P, GmDev D, int parity)
 {
     if (!D.ctl->go) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i == 0) *D.scan_ticket = 0;                // tile tickets of the scan that follows
     if (i >= P.n) return;
     float4 p = D.pos[parity][i];
     int key = 0;
@@ -107,22 +106,16 @@ __device__ __forceinline__ int block_exclusive_scan(int v, int *total)
     return r;
 }
 
-// Exclusive scan of ccount[0 .. n_cells] into cstart in ONE pass: a block scans its 4,096 counts, publishes its total,
-// adds up the totals of ALL blocks before it (a few hundred: one round of loads, eight per lane of warp 0, each polled
-// until this rebuild's value is there) and leaves ccount zeroed for the next rebuild.  Blocks take their tile from a
-// ticket counter, so a block only ever waits for tiles that are already running.  scan_state[t] = total | epoch << 32;
-// the epoch is the rebuild number, so the array is never reset between rebuilds.
+// A single-pass scan (tickets + look-back over the tile totals) measured SLOWER inside the step graphs than these
+// two launches (C3: 72.1 vs 71.5 us per timestep, same box): kept as two kernels.
+// Block-local exclusive scan; leaves ccount zeroed for the next rebuild.
 __global__ void __launch_bounds__(GM_SCAN_BLOCK)
-k_scan(const __grid_constant__ GmParams P, GmDev D)
+k_scan_local(const __grid_constant__ GmParams P, GmDev D)
 {
     if (!D.ctl->go) return;
-    __shared__ int total, tile_sh, prefix_sh;
-    if (threadIdx.x == 0) tile_sh = atomicAdd(D.scan_ticket, 1);
-    __syncthreads();
-    const int tile = tile_sh;
-    const unsigned int epoch = (unsigned int)D.ctl->n_rebuilds;      // >= 1 inside a rebuild; the array starts zeroed
+    __shared__ int total;
     const int n = P.n_cells + 1;
-    const int base = (tile * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
+    const int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
     int v[GM_SCAN_ITEMS], s = 0;
     if (base + GM_SCAN_ITEMS <= n) {
         const int4 q = *reinterpret_cast<const int4 *>(D.ccount + base);
@@ -138,26 +131,6 @@ k_scan(const __grid_constant__ GmParams P, GmDev D)
 #pragma unroll
     for (int q = 0; q < GM_SCAN_ITEMS; ++q) s += v[q];
     int off = block_exclusive_scan(s, &total);
-    volatile unsigned long long *state = D.scan_state;
-    if (threadIdx.x == 0) state[tile] = (unsigned long long)(unsigned int)total | ((unsigned long long)epoch << 32);
-    if (threadIdx.x < 32) {
-        int prefix = 0;
-        for (int p0 = (int)threadIdx.x; p0 < tile; p0 += 256) {
-            unsigned long long w[8];                       // eight loads in flight per lane, then the stragglers are polled
-#pragma unroll
-            for (int u = 0; u < 8; ++u) w[u] = (p0 + 32 * u < tile) ? state[p0 + 32 * u] : ((unsigned long long)epoch << 32);
-#pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                while ((unsigned int)(w[u] >> 32) != epoch) w[u] = state[p0 + 32 * u];
-                prefix += (int)(unsigned int)w[u];
-            }
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) prefix += __shfl_xor_sync(0xffffffffu, prefix, o);
-        if (threadIdx.x == 0) prefix_sh = prefix;
-    }
-    __syncthreads();
-    off += prefix_sh;
     if (base + GM_SCAN_ITEMS <= n) {          // one 16-byte store per thread (cstart is 256-byte aligned)
         *reinterpret_cast<int4 *>(D.cstart + base) = make_int4(off, off + v[0], off + v[0] + v[1], off + v[0] + v[1] + v[2]);
     } else {
@@ -166,6 +139,41 @@ k_scan(const __grid_constant__ GmParams P, GmDev D)
             if (base + q < n) D.cstart[base + q] = off;
             off += v[q];
         }
+    }
+    if (threadIdx.x == 0) D.scan_sums[blockIdx.x] = total;
+}
+
+// Each block adds the sum of the totals of the blocks before it (a few hundred at most).
+__global__ void __launch_bounds__(GM_SCAN_BLOCK)
+k_scan_add(const __grid_constant__ GmParams P, GmDev D)
+{
+    if (!D.ctl->go) return;
+    __shared__ int warp_part[32];
+    __shared__ int add_sh;
+    int part = 0;
+    for (int b = threadIdx.x; b < (int)blockIdx.x; b += GM_SCAN_BLOCK) part += D.scan_sums[b];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) part += __shfl_down_sync(0xffffffffu, part, o);
+    if ((threadIdx.x & 31) == 0) warp_part[threadIdx.x >> 5] = part;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+        int v = warp_part[threadIdx.x];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if (threadIdx.x == 0) add_sh = v;
+    }
+    __syncthreads();
+    const int add = add_sh;
+    const int n = P.n_cells + 1;
+    const int base = (blockIdx.x * GM_SCAN_BLOCK + threadIdx.x) * GM_SCAN_ITEMS;
+    if (base + GM_SCAN_ITEMS <= n) {
+        int4 c = *reinterpret_cast<const int4 *>(D.cstart + base);
+        c.x += add; c.y += add; c.z += add; c.w += add;
+        *reinterpret_cast<int4 *>(D.cstart + base) = c;
+    } else {
+#pragma unroll
+        for (int q = 0; q < GM_SCAN_ITEMS; ++q)
+            if (base + q < n) D.cstart[base + q] += add;
     }
 }
 
@@ -212,7 +220,8 @@ void gm_launch_sort(const GmParams &P, const GmDev &D, int parity, cudaStream_t 
     const int per = GM_SCAN_BLOCK * GM_SCAN_ITEMS;
     const int nsb = (P.n_cells + 1 + per - 1) / per;
     k_keys<<<nb, SORT_BLOCK, 0, st>>>(P, D, parity);
-    k_scan<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D);
+    k_scan_local<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D);
+    k_scan_add<<<nsb, GM_SCAN_BLOCK, 0, st>>>(P, D);
     k_scatter<<<nb, SORT_BLOCK, 0, st>>>(P, D);
     k_permute<<<nb, SORT_BLOCK, 0, st>>>(P, D, parity);
 }

@@ -42,7 +42,7 @@ class gm_config(C.Structure):
         ("kT", C.c_float), ("gamma", C.c_float), ("lam", C.c_float),
         ("sfc_period", C.c_int32), ("nl_row_capacity", C.c_int32), ("flags", C.c_int32),
         ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
-        ("table_points", C.c_int32), ("win_capacity", C.c_int32),
+        ("table_points", C.c_int32), ("win_capacity", C.c_int32), ("tile_windows", C.c_int32), ("reserved", C.c_int32),
     ]
 
 
