@@ -23,6 +23,10 @@
  *   - harmonic repulsion Eq. (2), Gaussian repulsion Eq. (3)
  *   - tabulated pair potential: cubic spline in z = r^2, Eq. (12); F = -2 r dV/dz, Eq. (11);
  *     cutoff = "point < Npoint", Alg. 2 lines 8-12
+ *   - angle potentials Eqs. (8), (9) and the periodic dihedral Eq. (10), each interaction
+ *     stored under every member with its position
+ *     (theta = angle at the middle bead between the two bonds, pi for a straight chain; phi = 0
+ *     for cis, pi for trans: DESIGN.md readings c-26, c-27)
  *   - FENE, WCA, the DPD force law, Philox: not in PAPER.md; readings c-3..c-8:
  *     Kremer-Grest FENE, Groot-Warren DPD with uniform unit-variance noise, Philox4x32-10
  *     (Salmon et al., SC'11) keyed (seed; min tag, max tag, step, stream).
@@ -72,6 +76,15 @@ typedef struct {
     const double *table;
     int32_t table_points;   /* Npoint: a pair interacts iff int(r^2 / interval) < Npoint */
     double table_interval;
+    /* Angles (i, j, k), j the middle bead, and dihedrals (i, j, k, l)      PAPER.md:L97, Eqs. (8)-(10) L103-114 */
+    int32_t angle_style;    /* 0 none, 1 Eq. (8) k (theta - theta0)^2, 2 Eq. (9) k (cos theta - cos theta0)^2 */
+    int64_t n_angles;
+    const int32_t *angle_i, *angle_j, *angle_k, *angle_type;
+    const double *angle_kk, *angle_t0;      /* per angle type */
+    int64_t n_dihedrals;    /* Eq. (10): k [1 + cos(n phi - delta)] */
+    const int32_t *dih_i, *dih_j, *dih_k, *dih_l, *dih_type;
+    const double *dih_kk, *dih_delta;       /* per dihedral type */
+    const int32_t *dih_n;
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -409,6 +422,75 @@ int orc_pair_bond_forces(const orc_params *p, const double *pos, const double *v
             }
             frc[3 * i] += fs * dx; frc[3 * i + 1] += fs * dy; frc[3 * i + 2] += fs * dz;
             frc[3 * j] -= fs * dx; frc[3 * j + 1] -= fs * dy; frc[3 * j + 2] -= fs * dz;
+        }
+    }
+    /* Angles, Eqs. (8)-(9): a = r_i - r_j, b = r_k - r_j (minimum image), cos(theta) = a.b / |a||b|.
+       d cos(theta) / d r_i = (b^ - cos(theta) a^) / |a|, d/d r_k = (a^ - cos(theta) b^) / |b|, and the middle bead takes
+       minus their sum.  Each angle once, acting on its three beads (the GPU evaluates it three times, L97).      */
+    if (p->angle_style != 0) {
+        for (int64_t q = 0; q < p->n_angles; ++q) {
+            int64_t i = p->angle_i[q], j = p->angle_j[q], k = p->angle_k[q];
+            double kk = p->angle_kk[p->angle_type[q]], t0 = p->angle_t0[p->angle_type[q]];
+            double a[3], b[3];
+            for (int d = 0; d < 3; ++d) {
+                a[d] = orc_min_image(pos[3 * i + d] - pos[3 * j + d], p->box[d]);
+                b[d] = orc_min_image(pos[3 * k + d] - pos[3 * j + d], p->box[d]);
+            }
+            double la = sqrt(a[0] * a[0] + a[1] * a[1] + a[2] * a[2]);
+            double lb = sqrt(b[0] * b[0] + b[1] * b[1] + b[2] * b[2]);
+            double c = (a[0] * b[0] + a[1] * b[1] + a[2] * b[2]) / (la * lb);
+            if (c > 1.0) c = 1.0;
+            if (c < -1.0) c = -1.0;
+            double dudc;                                  /* dU / d cos(theta) */
+            if (p->angle_style == 1) {
+                /* Eq. (8): U = k (theta - theta0)^2;  dU/dcos = dU/dtheta * (-1 / sin(theta)) */
+                double th = acos(c), sn = sqrt(1.0 - c * c);
+                if (sn < 1e-12) sn = 1e-12;
+                pe_bond += kk * (th - t0) * (th - t0);
+                dudc = -2.0 * kk * (th - t0) / sn;
+            } else {
+                /* Eq. (9): U = k (cos(theta) - cos(theta0))^2 */
+                double dc = c - cos(t0);
+                pe_bond += kk * dc * dc;
+                dudc = 2.0 * kk * dc;
+            }
+            for (int d = 0; d < 3; ++d) {
+                double fi = -dudc * (b[d] / lb - c * a[d] / la) / la;
+                double fk = -dudc * (a[d] / la - c * b[d] / lb) / lb;
+                frc[3 * i + d] += fi; frc[3 * k + d] += fk; frc[3 * j + d] -= fi + fk;
+            }
+        }
+    }
+    /* Dihedrals, Eq. (10): b1 = r_j - r_i, b2 = r_k - r_j, b3 = r_l - r_k, n1 = b1 x b2, n2 = b2 x b3,
+       phi = atan2(|b2| b1.n2, n1.n2) (0 = cis, pi = trans).  d phi / d r_i = -|b2| n1 / |n1|^2, d phi / d r_l = |b2| n2 / |n2|^2,
+       d phi / d r_j = -(1 + b1.b2 / |b2|^2) dphi/dr_i + (b3.b2 / |b2|^2) dphi/dr_l, d phi / d r_k = -(1 + b3.b2 / |b2|^2) dphi/dr_l
+       + (b1.b2 / |b2|^2) dphi/dr_i  (the textbook form, e.g. Blondel and Karplus 1996; pinned by central differences).  */
+    for (int64_t q = 0; q < p->n_dihedrals; ++q) {
+        int64_t m[4] = { p->dih_i[q], p->dih_j[q], p->dih_k[q], p->dih_l[q] };
+        double kk = p->dih_kk[p->dih_type[q]], dl = p->dih_delta[p->dih_type[q]];
+        int nn = p->dih_n[p->dih_type[q]];
+        double b1[3], b2[3], b3[3], n1[3], n2[3];
+        for (int d = 0; d < 3; ++d) {
+            b1[d] = orc_min_image(pos[3 * m[1] + d] - pos[3 * m[0] + d], p->box[d]);
+            b2[d] = orc_min_image(pos[3 * m[2] + d] - pos[3 * m[1] + d], p->box[d]);
+            b3[d] = orc_min_image(pos[3 * m[3] + d] - pos[3 * m[2] + d], p->box[d]);
+        }
+        n1[0] = b1[1] * b2[2] - b1[2] * b2[1]; n1[1] = b1[2] * b2[0] - b1[0] * b2[2]; n1[2] = b1[0] * b2[1] - b1[1] * b2[0];
+        n2[0] = b2[1] * b3[2] - b2[2] * b3[1]; n2[1] = b2[2] * b3[0] - b2[0] * b3[2]; n2[2] = b2[0] * b3[1] - b2[1] * b3[0];
+        double l2 = sqrt(b2[0] * b2[0] + b2[1] * b2[1] + b2[2] * b2[2]);
+        double n1s = n1[0] * n1[0] + n1[1] * n1[1] + n1[2] * n1[2];
+        double n2s = n2[0] * n2[0] + n2[1] * n2[1] + n2[2] * n2[2];
+        if (n1s < 1e-24 || n2s < 1e-24) continue;     /* three beads in line: phi undefined, no force */
+        double phi = atan2(l2 * (b1[0] * n2[0] + b1[1] * n2[1] + b1[2] * n2[2]), n1[0] * n2[0] + n1[1] * n2[1] + n1[2] * n2[2]);
+        pe_bond += kk * (1.0 + cos(nn * phi - dl));
+        double dudphi = -kk * nn * sin(nn * phi - dl);
+        double s12 = (b1[0] * b2[0] + b1[1] * b2[1] + b1[2] * b2[2]) / (l2 * l2);
+        double s32 = (b3[0] * b2[0] + b3[1] * b2[1] + b3[2] * b2[2]) / (l2 * l2);
+        for (int d = 0; d < 3; ++d) {
+            double gi = -l2 * n1[d] / n1s, gl = l2 * n2[d] / n2s;
+            double gj = -(1.0 + s12) * gi + s32 * gl, gk = -(1.0 + s32) * gl + s12 * gi;
+            frc[3 * m[0] + d] -= dudphi * gi; frc[3 * m[1] + d] -= dudphi * gj;
+            frc[3 * m[2] + d] -= dudphi * gk; frc[3 * m[3] + d] -= dudphi * gl;
         }
     }
     if (out) { out[0] = pe_pair; out[1] = pe_bond; out[2] = 0.5 * n_in; }

@@ -45,6 +45,12 @@ class _Params(C.Structure):
         ("type", C.c_void_p), ("mass", C.c_void_p),
         ("use_cells", C.c_int32), ("n_threads", C.c_int32),
         ("table", C.c_void_p), ("table_points", C.c_int32), ("table_interval", C.c_double),
+        ("angle_style", C.c_int32), ("n_angles", C.c_int64),
+        ("angle_i", C.c_void_p), ("angle_j", C.c_void_p), ("angle_k", C.c_void_p), ("angle_type", C.c_void_p),
+        ("angle_kk", C.c_void_p), ("angle_t0", C.c_void_p),
+        ("n_dihedrals", C.c_int64),
+        ("dih_i", C.c_void_p), ("dih_j", C.c_void_p), ("dih_k", C.c_void_p), ("dih_l", C.c_void_p), ("dih_type", C.c_void_p),
+        ("dih_kk", C.c_void_p), ("dih_delta", C.c_void_p), ("dih_n", C.c_void_p),
     ]
 
 
@@ -235,6 +241,30 @@ class Oracle:
         P.bond_k = _p(self.bond_k).value; P.bond_r0 = _p(self.bond_r0).value
         P.type = _p(self.type).value; P.mass = _p(self.mass).value
         P.use_cells = int(use_cells); P.n_threads = int(n_threads)
+        # angles / dihedrals (optional attributes of the workload: w.topo = dict(angle_style, angles (n,3), angle_type,
+        # angle_k, angle_t0, dihedrals (n,4), dihedral_type, dihedral_k, dihedral_n, dihedral_delta))
+        topo = getattr(w, "topo", None) or {}
+        ANG = {"none": 0, "harmonic": 1, "cosine": 2}
+        self._ang = np.ascontiguousarray(topo.get("angles", np.zeros((0, 3))), np.int32).reshape(-1, 3)
+        self._ang_cols = [np.ascontiguousarray(self._ang[:, c]) for c in range(3)]
+        self._ang_type = np.ascontiguousarray(topo.get("angle_type", np.zeros(len(self._ang))), np.int32)
+        self._ang_k = np.ascontiguousarray(topo.get("angle_k", [0.0]), np.float32).astype(np.float64)
+        self._ang_t0 = np.ascontiguousarray(topo.get("angle_t0", [0.0]), np.float32).astype(np.float64)
+        P.angle_style = ANG[topo.get("angle_style", "none")] if len(self._ang) else 0
+        P.n_angles = len(self._ang)
+        P.angle_i, P.angle_j, P.angle_k = (_p(c).value for c in self._ang_cols)
+        P.angle_type = _p(self._ang_type).value
+        P.angle_kk = _p(self._ang_k).value; P.angle_t0 = _p(self._ang_t0).value
+        self._dih = np.ascontiguousarray(topo.get("dihedrals", np.zeros((0, 4))), np.int32).reshape(-1, 4)
+        self._dih_cols = [np.ascontiguousarray(self._dih[:, c]) for c in range(4)]
+        self._dih_type = np.ascontiguousarray(topo.get("dihedral_type", np.zeros(len(self._dih))), np.int32)
+        self._dih_k = np.ascontiguousarray(topo.get("dihedral_k", [0.0]), np.float32).astype(np.float64)
+        self._dih_delta = np.ascontiguousarray(topo.get("dihedral_delta", [0.0]), np.float32).astype(np.float64)
+        self._dih_n = np.ascontiguousarray(topo.get("dihedral_n", [1]), np.int32)
+        P.n_dihedrals = len(self._dih)
+        P.dih_i, P.dih_j, P.dih_k, P.dih_l = (_p(c).value for c in self._dih_cols)
+        P.dih_type = _p(self._dih_type).value
+        P.dih_kk = _p(self._dih_k).value; P.dih_delta = _p(self._dih_delta).value; P.dih_n = _p(self._dih_n).value
         if w.pair_style == "table":
             P.table = _p(self.table).value
             P.table_points = int(self.table.shape[2])

@@ -43,6 +43,7 @@ class Workload:
     chain_len: int = 1
     equil_steps: int = 0       # Langevin equilibration the config names (C3)
     notes: dict = field(default_factory=dict)
+    topo: dict = field(default_factory=dict)   # angles / dihedrals: see oracle.Oracle and gm.System (empty: none)
 
     @property
     def n(self) -> int:
