@@ -14,6 +14,8 @@
  *      tabulated pair potential              PAPER.md:L118-129 Eqs. (11)-(12), Alg. 2 L458 (cubic spline in z = r^2)
  *   a6 DPD pair force (Groot-Warren)         PAPER.md:L43, L135, L197 (law itself: ref. 24; DESIGN.md c-3)
  *   a7 bond force from the BL/BN table       PAPER.md:L97, Eq. (7) L99-101 (harmonic); FENE: DESIGN.md c-8
+ *      angle and dihedral forces from        PAPER.md:L97 (per-particle tables with the member's position), Eqs. (8)-(10)
+ *      per-particle tables                   L103-114
  *   a8 velocity-Verlet NVE / Langevin "BD" / GW-VV
  *   a9 energies (validation quantities)
  *
@@ -64,6 +66,7 @@ enum {
 enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2, GM_PAIR_HARMONIC = 3, GM_PAIR_GAUSS = 4, GM_PAIR_TABLE = 5 };
 enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2 };
 enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2 };
+enum { GM_ANGLE_NONE = 0, GM_ANGLE_HARMONIC = 1 /* Eq. (8): k (theta - theta0)^2 */, GM_ANGLE_COSINE = 2 /* Eq. (9): k (cos theta - cos theta0)^2 */ };
 
 #define GM_MAX_TYPES 8       /* particle types; pair tables are n_types x n_types */
 #define GM_MAX_BOND_TYPES 8
@@ -96,7 +99,9 @@ typedef struct {
     int32_t table_points;            /* GM_PAIR_TABLE: grid points (Npoint of Alg. 2) of every pair table; else 0       */
     int32_t win_capacity;            /* positions a tile window holds (shared memory per CTA = 16 B x this), <= 8000    */
     int32_t tile_windows;            /* 1: stage tile windows whatever the list length, 2: never (0: lists of >= 40)     */
-    int32_t reserved;                /* must be 0                                                                      */
+    int32_t angle_style;             /* GM_ANGLE_*                                                                     */
+    int32_t max_angles_per_particle; /* rows of the per-particle angle table; 0 = no angles              */
+    int32_t max_dihedrals_per_particle; /* rows of the per-particle dihedral table; 0 = no dihedrals (Eq. (10))         */
 } gm_config;
 
 enum {
@@ -164,6 +169,23 @@ gm_status gm_set_particles(gm_system *s, const float *pos3, const float *vel3, c
 gm_status gm_set_bonds(gm_system *s, int64_t n_bonds, const int32_t *tag_pairs2, const int32_t *btype,
                        int on_device);
 
+/* Angle parameters of angle type `atype` (< GM_MAX_BOND_TYPES): Eq. (8) U = k (theta - theta0)^2 or Eq. (9)
+ * U = k (cos theta - cos theta0)^2 by cfg.angle_style; theta0 in radians; theta is the angle at the
+ * middle bead between its two bonds (pi for a straight chain; DESIGN.md c-26). */
+gm_status gm_set_angle_params(gm_system *s, int atype, float k, float theta0);
+
+/* Dihedral parameters of dihedral type `dtype`: Eq. (10) U = k [1 + cos(n phi - delta)]; phi = 0 for
+ * cis, pi for trans (DESIGN.md c-27). */
+gm_status gm_set_dihedral_params(gm_system *s, int dtype, float k, int n, float delta);
+
+/* Angles as n_angles tag triples (i, j, k), j the middle bead, + a type each (NULL = all 0); dihedrals as tag
+ * quadruples (i, j, k, l).  Each is entered in the per-particle table of EVERY member together with the member's
+ * position, so that one thread sums all angle and dihedral forces of its bead without atomics -- an angle is evaluated
+ * three times, a dihedral four times.  HOST arrays (set-up path).  Their energy is reported with the bond
+ * energy (gm_energies out[2]).  Errors: INVALID_ARG (a bead exceeds max_*_per_particle, tag out of range). */
+gm_status gm_set_angles(gm_system *s, int64_t n_angles, const int32_t *tags3, const int32_t *atype);
+gm_status gm_set_dihedrals(gm_system *s, int64_t n_dihedrals, const int32_t *tags4, const int32_t *dtype);
+
 /* Set the time-level counter (the `step` word of the Philox counter).  For restarts. */
 gm_status gm_set_step(gm_system *s, uint64_t step);
 
@@ -194,7 +216,7 @@ gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma)
  * Synchronises.  Same results, bit for bit, as gm_step. */
 gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4]);
 
-/* out (HOST, 8 doubles): kinetic energy, pair PE, bond PE, temperature (3N-3 dof), px, py, pz,
+/* out (HOST, 8 doubles): kinetic energy, pair PE, bonded PE (bonds + angles + dihedrals), temperature (3N-3 dof), px, py, pz,
  * number of unique pairs inside r_cut.  fp32 terms, fp64 sums.  Synchronises. */
 gm_status gm_energies(gm_system *s, double out[8]);
 

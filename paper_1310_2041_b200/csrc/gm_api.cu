@@ -58,7 +58,10 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
-        c->step_shape < 0 || c->step_shape > 2 || c->win_capacity < 0 || c->win_capacity > 8000 || c->tile_windows < 0 || c->tile_windows > 2 || c->reserved != 0)
+        c->step_shape < 0 || c->step_shape > 2 || c->win_capacity < 0 || c->win_capacity > 8000 || c->tile_windows < 0 || c->tile_windows > 2 ||
+        c->angle_style < GM_ANGLE_NONE || c->angle_style > GM_ANGLE_COSINE || c->max_angles_per_particle < 0 ||
+        c->max_angles_per_particle > 64 || c->max_dihedrals_per_particle < 0 || c->max_dihedrals_per_particle > 64 ||
+        (c->max_angles_per_particle > 0 && c->angle_style == GM_ANGLE_NONE))
         return GM_ERR_INVALID_ARG;
     P->n = (int)c->n_particles;
     P->ns = (P->n + 8 + GM_PAD - 1) / GM_PAD * GM_PAD;     // slots n .. n+7 (at least): far-away pad beads
@@ -129,7 +132,8 @@ static gm_status derive(const gm_config *c, GmParams *P)
     P->nl_cap = cap;
     // lanes per bead of the step kernel: 8 lanes sharing a bead (shuffle reduction) measured SLOWER than one
     // thread per bead on every config, so it is opt-in
-    P->step_subw = (c->flags & GM_FLAG_STEP_SUBWARP) ? 8 : 1;
+    P->angle_style = c->angle_style; P->max_angles = c->max_angles_per_particle; P->max_dihedrals = c->max_dihedrals_per_particle;
+    P->step_subw = ((c->flags & GM_FLAG_STEP_SUBWARP) && P->max_angles + P->max_dihedrals == 0) ? 8 : 1;
     P->capq = cap / 4;
     P->minq = std::min(4, P->capq);
     // tile windows (gm_nlist.cu): every pair style but DPD (which also gathers velocities), one thread per bead.  A window holds the hulls of the x runs
@@ -178,6 +182,9 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     }
     d.frc = (float4 *)take(n * 16);
     if (P.table_points > 0) d.table = (float4 *)take((size_t)P.n_types * P.n_types * P.table_points * 16);
+    if (P.max_angles + P.max_dihedrals > 0) d.ftopo = (float4 *)take(n * 16);
+    if (P.max_angles > 0) d.at = (int4 *)take(n * 16 * (size_t)P.max_angles);
+    if (P.max_dihedrals > 0) d.dt = (int4 *)take(n * 16 * (size_t)P.max_dihedrals);
     d.tag[0] = (int *)take(n * 4); d.tag[1] = (int *)take(n * 4); d.rtag = (int *)take(n * 4);
     d.nn = (int *)take(n * 4);
     d.nnw = (int *)take(n / 32 * 4);
@@ -313,6 +320,9 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
         if (e == cudaSuccess) e = cudaMemsetAsync(s->D.blt[1], 0xFF, bb, s->st);
         if (e == cudaSuccess) e = cudaMemsetAsync(s->D.bl_tag, 0xFF, bb, s->st);
     }
+    if (e == cudaSuccess && P.max_angles + P.max_dihedrals > 0) e = cudaMemsetAsync(s->D.ftopo, 0, (size_t)P.ns * 16, s->st);
+    if (e == cudaSuccess && P.max_angles > 0) e = cudaMemsetAsync(s->D.at, 0xFF, (size_t)P.ns * 16 * P.max_angles, s->st);
+    if (e == cudaSuccess && P.max_dihedrals > 0) e = cudaMemsetAsync(s->D.dt, 0xFF, (size_t)P.ns * 16 * P.max_dihedrals, s->st);
     if (e == cudaSuccess) {
         gm_launch_init_pad(P, s->D, s->st);
         gm_launch_set_ctl(s->D, 0, 1, 0, s->st);
@@ -460,6 +470,80 @@ extern "C" gm_status gm_set_bond_params(gm_system *s, int btype, float k, float 
     s->force_current = false;
     drop_graphs(s);
     return GM_OK;
+}
+
+extern "C" gm_status gm_set_angle_params(gm_system *s, int atype, float k, float theta0)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (atype < 0 || atype >= GM_MAX_BOND_TYPES) return fail(s, GM_ERR_INVALID_ARG, "gm_set_angle_params: bad angle type%s");
+    s->P.angle_k[atype] = k; s->P.angle_t0[atype] = theta0; s->P.angle_c0[atype] = (float)std::cos((double)theta0);
+    s->force_current = false;
+    drop_graphs(s);
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_dihedral_params(gm_system *s, int dtype, float k, int n, float delta)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (dtype < 0 || dtype >= GM_MAX_BOND_TYPES) return fail(s, GM_ERR_INVALID_ARG, "gm_set_dihedral_params: bad dihedral type%s");
+    s->P.dih_k[dtype] = k; s->P.dih_n[dtype] = n; s->P.dih_delta[dtype] = delta;
+    s->force_current = false;
+    drop_graphs(s);
+    return GM_OK;
+}
+
+// Per-particle angle / dihedral tables: every interaction under every member, with the member's
+// position.  NM = members per interaction (3 or 4); entry of the member at position p: the other members in order,
+// then (angles) p and the type, (dihedrals) p | type << 2.
+template <int NM>
+static gm_status set_topology(gm_system *s, int64_t count, const int32_t *tags, const int32_t *type, int max_rows, int4 *table,
+                              const char *who)
+{
+    if (count < 0 || (count > 0 && !tags)) return fail(s, GM_ERR_INVALID_ARG, "%s: bad arguments", who);
+    if (max_rows <= 0) {
+        if (count == 0) return GM_OK;
+        return fail(s, GM_ERR_INVALID_ARG, "%s: the per-particle table has no rows (max_*_per_particle is 0)", who);
+    }
+    CU(cudaSetDevice(s->cfg.device));
+    const size_t n = (size_t)s->P.n, ns = (size_t)s->P.ns;
+    std::vector<int32_t> rows(n, 0);
+    std::vector<int4> tb(ns * (size_t)max_rows, make_int4(-1, -1, -1, -1));
+    for (int64_t q = 0; q < count; ++q) {
+        const int32_t *m = tags + NM * q;
+        const int32_t ty = type ? type[q] : 0;
+        if (ty < 0 || ty >= GM_MAX_BOND_TYPES) return fail(s, GM_ERR_INVALID_ARG, "%s: type out of range", who);
+        for (int a = 0; a < NM; ++a) {
+            if (m[a] < 0 || (size_t)m[a] >= n) return fail(s, GM_ERR_INVALID_ARG, "%s: tag out of range", who);
+            for (int b = 0; b < a; ++b) if (m[a] == m[b]) return fail(s, GM_ERR_INVALID_ARG, "%s: a bead appears twice", who);
+        }
+        for (int p = 0; p < NM; ++p) {
+            const int32_t own = m[p];
+            if (rows[own] >= max_rows) return fail(s, GM_ERR_INVALID_ARG, "%s: a bead exceeds max_*_per_particle", who);
+            int32_t o[3] = { -1, -1, -1 };
+            for (int a = 0, c = 0; a < NM; ++a) if (a != p) o[c++] = m[a];
+            int4 e;
+            if (NM == 3) e = make_int4(o[0], o[1], p, ty);
+            else e = make_int4(o[0], o[1], o[2], p | (ty << 2));
+            tb[(size_t)rows[own] * ns + own] = e;
+            rows[own] += 1;
+        }
+    }
+    CU(cudaMemcpyAsync(table, tb.data(), tb.size() * sizeof(int4), cudaMemcpyHostToDevice, s->st));
+    CU(cudaStreamSynchronize(s->st));
+    s->force_current = false;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_angles(gm_system *s, int64_t n_angles, const int32_t *tags3, const int32_t *atype)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    return set_topology<3>(s, n_angles, tags3, atype, s->P.max_angles, s->D.at, "gm_set_angles");
+}
+
+extern "C" gm_status gm_set_dihedrals(gm_system *s, int64_t n_dihedrals, const int32_t *tags4, const int32_t *dtype)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    return set_topology<4>(s, n_dihedrals, tags4, dtype, s->P.max_dihedrals, s->D.dt, "gm_set_dihedrals");
 }
 
 // ---- particles and bonds ----------------------------------------------------------------------------

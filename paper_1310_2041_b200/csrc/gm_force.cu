@@ -12,6 +12,7 @@ void gm_launch_force_table(const GmParams &, const GmDev &, int, int, float, flo
 void gm_launch_force(const GmParams &P, const GmDev &D, int mode, int parity, float kick, float kick_vt,
                      int lagged, cudaStream_t st)
 {
+    gm_launch_topo(P, D, parity, st);        // a7: angle + dihedral forces of this time level -> D.ftopo (no-op without them)
     switch (P.pair_style) {
     case GM_PAIR_LJ: gm_launch_force_lj(P, D, mode, parity, kick, kick_vt, lagged, st); break;
     case GM_PAIR_DPD: gm_launch_force_dpd(P, D, mode, parity, kick, kick_vt, lagged, st); break;

@@ -515,6 +515,16 @@ __device__ __forceinline__ BeadForce bead_force(const GmParams &P, const GmDev &
     return o;
 }
 
+// a7: the angle + dihedral force of bead i (gm_topo.cu ran just before) and its share of their energy
+__device__ __forceinline__ void topo_add(const GmParams &P, const GmDev &D, int i, BeadForce &f)
+{
+    if (P.max_angles + P.max_dihedrals > 0) {
+        const float4 ft = D.ftopo[i];
+        f.fx += ft.x; f.fy += ft.y; f.fz += ft.z;
+        f.pe_bond += ft.w;
+    }
+}
+
 // Acceleration the integrator uses: F/m, plus Langevin drag on the stored velocity and the per-bead
 // noise of this time level (reading c-7): a = F/m - gamma u + sqrt(6 gamma kT / (dt m)) xi.
 __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, int i, const BeadForce &f,
@@ -563,8 +573,9 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
     T.win = 0; T.mbar = 0; T.staged = 0; T.parity = 0;
     if (WINS) T = tile_stage(P, D, S, blockIdx.x, wd, wsm, 0u, true);
     if (WINS && PAIR != GM_PAIR_NONE && P.use_win && !T.staged) nl_preload_rest(P, t, pol, pre);
-    const BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES, NQL, WINS>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col, T, be, valid);
+    BeadForce f = bead_force<PAIR, NT1, BOND, MODE == GM_MODE_FORCES, NQL, WINS>(P, D, S, i, pi, vti, t, pol, pre, nn, step, col, T, be, valid);
     if (!valid) return;
+    topo_add(P, D, i, f);
     const float3 a = bead_accel(P, S, i, f, u, step);
     if (MODE == GM_MODE_FORCES) {
         D.frc[i] = make_float4(a.x * u.w, a.y * u.w, a.z * u.w, f.pe_pair + f.pe_bond);
@@ -743,8 +754,9 @@ k_energy(const __grid_constant__ GmParams P, GmDev D, int parity, int lagged)
         armed = true;
         if (T.staged) phase ^= 1u;                          // the mbarrier completes one phase per staged tile
         if (PAIR != GM_PAIR_NONE && P.use_win && !T.staged) nl_preload_rest(P, t, pol, pre);
-        const BeadForce f = bead_force<PAIR, NT1, BOND, true, GM_LJ_NQ, PAIR != GM_PAIR_DPD && PAIR != GM_PAIR_NONE>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x, T, be, valid);
+        BeadForce f = bead_force<PAIR, NT1, BOND, true, GM_LJ_NQ, PAIR != GM_PAIR_DPD && PAIR != GM_PAIR_NONE>(P, D, S, i, pi, vti, t, pol, pre, nn, step, gm_cpt + threadIdx.x, T, be, valid);
         if (!valid) continue;
+        topo_add(P, D, i, f);
         const float4 u = S.vel[i];
         float vx = u.x, vy = u.y, vz = u.z;
         if (lagged) {   // complete the half-step velocity: v^m = u^{m-1} + dt/2 a^m

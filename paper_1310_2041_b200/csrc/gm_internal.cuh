@@ -93,6 +93,10 @@ struct GmParams {
     GmPair pair[GM_MAX_TYPES * GM_MAX_TYPES];
     float bond_k[GM_MAX_BOND_TYPES], bond_r0[GM_MAX_BOND_TYPES];
     float bond_c[GM_MAX_BOND_TYPES];   // FENE: 1 / R0^2
+    int angle_style, max_angles, max_dihedrals;   // per-particle angle / dihedral tables (gm_topo.cu); has_topo = either > 0
+    float angle_k[GM_MAX_BOND_TYPES], angle_t0[GM_MAX_BOND_TYPES], angle_c0[GM_MAX_BOND_TYPES];   // c0 = cos(theta0)
+    float dih_k[GM_MAX_BOND_TYPES], dih_delta[GM_MAX_BOND_TYPES];
+    int dih_n[GM_MAX_BOND_TYPES];
     const float4 *table;               // GM_PAIR_TABLE: (c0, c1, c2, c3) per grid point, n_types^2 tables of table_points
     int table_points;
 };
@@ -105,6 +109,9 @@ struct GmDev {
     float4 *vt[2], *svt;
     float4 *frc;
     float4 *table;           // GM_PAIR_TABLE: spline coefficients, [n_types^2][table_points]
+    float4 *ftopo;           // angle + dihedral force (x, y, z) and energy share (w) of every bead, storage order
+    int4 *at;                // angle table in TAG order: at[k * ns + tag] = (tag a, tag b, own position 0/1/2, type); x < 0: none
+    int4 *dt;                // dihedral table in TAG order: dt[k * ns + tag] = (tag a, tag b, tag c, own position | type << 2)
     int *tag[2], *rtag;
     int *nn, *nnw;
     int4 *nl;
@@ -145,6 +152,7 @@ void gm_launch_unpack(const GmParams &P, const GmDev &D, int cur, float *pos3, f
                       int lagged, cudaStream_t st);
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,
                                 int t0, int t1, cudaStream_t st);
+void gm_launch_topo(const GmParams &P, const GmDev &D, int parity, cudaStream_t st);     // angle + dihedral forces -> D.ftopo
 void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, int parity, cudaStream_t st);
 void gm_launch_init_pad(const GmParams &P, const GmDev &D, cudaStream_t st);
 

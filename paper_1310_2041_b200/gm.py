@@ -22,10 +22,11 @@ GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_
 GM_PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
 GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
+GM_ANGLE = {"none": 0, "harmonic": 1, "cosine": 2}
 GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP, GM_FLAG_NO_WINDOWS = 1, 2, 4, 8
 
 SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_pair_table", "gm_fit_pair_table",
-           "gm_set_bond_params",
+           "gm_set_bond_params", "gm_set_angle_params", "gm_set_dihedral_params", "gm_set_angles", "gm_set_dihedrals",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
            "gm_get_tuning",
@@ -42,7 +43,8 @@ class gm_config(C.Structure):
         ("kT", C.c_float), ("gamma", C.c_float), ("lam", C.c_float),
         ("sfc_period", C.c_int32), ("nl_row_capacity", C.c_int32), ("flags", C.c_int32),
         ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
-        ("table_points", C.c_int32), ("win_capacity", C.c_int32), ("tile_windows", C.c_int32), ("reserved", C.c_int32),
+        ("table_points", C.c_int32), ("win_capacity", C.c_int32), ("tile_windows", C.c_int32),
+        ("angle_style", C.c_int32), ("max_angles_per_particle", C.c_int32), ("max_dihedrals_per_particle", C.c_int32),
     ]
 
 
@@ -71,6 +73,10 @@ def lib():
         L.gm_set_pair_table.argtypes = [vp, i32, i32, C.c_float, vp]
         L.gm_fit_pair_table.argtypes = [i32, C.c_double, vp, vp]
         L.gm_set_bond_params.argtypes = [vp, i32, C.c_float, C.c_float]
+        L.gm_set_angle_params.argtypes = [vp, i32, C.c_float, C.c_float]
+        L.gm_set_dihedral_params.argtypes = [vp, i32, C.c_float, i32, C.c_float]
+        L.gm_set_angles.argtypes = [vp, i64, vp, vp]
+        L.gm_set_dihedrals.argtypes = [vp, i64, vp, vp]
         L.gm_set_particles.argtypes = [vp, vp, vp, vp, vp, i32]
         L.gm_set_bonds.argtypes = [vp, i64, vp, vp, i32]
         L.gm_set_step.argtypes = [vp, C.c_uint64]
@@ -154,6 +160,26 @@ def gm_fit_pair_table(v, interval: float) -> np.ndarray:
 
 def gm_set_bond_params(h, btype: int, k: float, r0: float):
     _check(lib().gm_set_bond_params(h, btype, k, r0), h)
+
+
+def gm_set_angle_params(h, atype: int, k: float, theta0: float):
+    _check(lib().gm_set_angle_params(h, atype, k, theta0), h)
+
+
+def gm_set_dihedral_params(h, dtype: int, k: float, n: int, delta: float):
+    _check(lib().gm_set_dihedral_params(h, dtype, k, n, delta), h)
+
+
+def gm_set_angles(h, tags3, atype=None):
+    tags3 = np.ascontiguousarray(tags3, dtype=np.int32).reshape(-1, 3)
+    atype = None if atype is None else np.ascontiguousarray(atype, dtype=np.int32)
+    _check(lib().gm_set_angles(h, len(tags3), tags3.ctypes.data, None if atype is None else atype.ctypes.data), h)
+
+
+def gm_set_dihedrals(h, tags4, dtype=None):
+    tags4 = np.ascontiguousarray(tags4, dtype=np.int32).reshape(-1, 4)
+    dtype = None if dtype is None else np.ascontiguousarray(dtype, dtype=np.int32)
+    _check(lib().gm_set_dihedrals(h, len(tags4), tags4.ctypes.data, None if dtype is None else dtype.ctypes.data), h)
 
 
 def gm_set_particles(h, pos3, vel3, type_, mass=None):
@@ -279,6 +305,14 @@ class System:
         cfg.sfc_period = int(w.sfc_period if sfc_period is None else sfc_period)
         cfg.nl_row_capacity = int(nl_row_capacity)
         cfg.flags = int(flags)
+        topo = getattr(w, "topo", None) or {}
+        ang = np.ascontiguousarray(topo.get("angles", np.zeros((0, 3))), np.int32).reshape(-1, 3)
+        dih = np.ascontiguousarray(topo.get("dihedrals", np.zeros((0, 4))), np.int32).reshape(-1, 4)
+        if len(ang):
+            cfg.angle_style = GM_ANGLE[topo.get("angle_style", "harmonic")]
+            cfg.max_angles_per_particle = int(np.bincount(ang.ravel(), minlength=self.n).max())
+        if len(dih):
+            cfg.max_dihedrals_per_particle = int(np.bincount(dih.ravel(), minlength=self.n).max())
         for k, v in (tune or {}).items():       # gm_config tuning overrides: x_cell_div, nl_scan_trip, step_shape
             setattr(cfg, k, int(v))
         self.cfg = cfg
@@ -304,6 +338,14 @@ class System:
         if cfg.bond_style:
             for bt in range(len(w.bond["k"])):
                 gm_set_bond_params(self.h, bt, float(w.bond["k"][bt]), float(w.bond["r0"][bt]))
+        if len(ang):
+            for at, (k, t0) in enumerate(zip(topo["angle_k"], topo["angle_t0"])):
+                gm_set_angle_params(self.h, at, float(np.float32(k)), float(np.float32(t0)))
+            gm_set_angles(self.h, ang, topo.get("angle_type"))
+        if len(dih):
+            for dt_, (k, nn, dl) in enumerate(zip(topo["dihedral_k"], topo["dihedral_n"], topo["dihedral_delta"])):
+                gm_set_dihedral_params(self.h, dt_, float(np.float32(k)), int(nn), float(np.float32(dl)))
+            gm_set_dihedrals(self.h, dih, topo.get("dihedral_type"))
         if load:
             self.set_particles(w.pos, w.vel, w.type, w.mass)
             if cfg.max_bonds_per_particle:
