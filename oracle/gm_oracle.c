@@ -27,6 +27,8 @@
  *     stored under every member with its position
  *     (theta = angle at the middle bead between the two bonds, pi for a straight chain; phi = 0
  *     for cis, pi for trans: DESIGN.md readings c-26, c-27)
+ *   - NVT by Nose-Hoover, Andersen or Berendsen thermostat: named only
+ *     (leapfrog forms with the temperature of the half-step velocities; readings c-28..c-30)
  *   - FENE, WCA, the DPD force law, Philox: not in PAPER.md; readings c-3..c-8:
  *     Kremer-Grest FENE, Groot-Warren DPD with uniform unit-variance noise, Philox4x32-10
  *     (Salmon et al., SC'11) keyed (seed; min tag, max tag, step, stream).
@@ -48,7 +50,7 @@
 
 enum { ORC_PAIR_NONE = 0, ORC_PAIR_LJ = 1, ORC_PAIR_DPD = 2, ORC_PAIR_HARMONIC = 3, ORC_PAIR_GAUSS = 4, ORC_PAIR_TABLE = 5 };
 enum { ORC_BOND_NONE = 0, ORC_BOND_FENE = 1, ORC_BOND_HARMONIC = 2 };
-enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2 };
+enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2, ORC_NOSE_HOOVER = 3, ORC_ANDERSEN = 4, ORC_BERENDSEN = 5 };
 enum { ORC_OK = 0, ORC_ERR_BOND_OVERSTRETCH = -7, ORC_ERR_ARG = -1 };
 
 typedef struct {
@@ -85,6 +87,10 @@ typedef struct {
     const int32_t *dih_i, *dih_j, *dih_k, *dih_l, *dih_type;
     const double *dih_kk, *dih_delta;       /* per dihedral type */
     const int32_t *dih_n;
+    /* NVT thermostats (equations: DESIGN.md readings c-28..c-30), leapfrog form.  `gamma` is the
+       coupling rate: Nose-Hoover 1/tau, Berendsen 1/tau_T, Andersen collision frequency nu.  thermo[0] = 1 once a
+       half-step velocity exists, thermo[1] = its kinetic energy sum 1/2 m u^2, thermo[2] = Nose-Hoover xi.           */
+    double *thermo;
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -253,6 +259,29 @@ int64_t orc_neighbor_pairs(int64_t n, const double *pos, const double box[3], do
     }
     cells_free(&cl);
     return cnt;
+}
+
+/* Andersen thermostat (reading c-29): bead `tag` collides with the heat bath in the kick of time level `step` iff
+   the top 24 bits of Philox(tag, 0, step, stream 3) word 0 are < floor(nu dt 2^24); its new velocity components are
+   sqrt(kT/m) times three standard normals by Box-Muller from the four words of stream 2:
+   g0 = sqrt(-2 ln u0) cos(2 pi u1), g1 = sqrt(-2 ln u0) sin(2 pi u1), g2 = sqrt(-2 ln u2) cos(2 pi u3). */
+int orc_andersen_hit(uint64_t seed, uint64_t step, int64_t tag, double nu_dt)
+{
+    uint32_t w[4];
+    noise_words(seed, (uint32_t)tag, 0u, step, 3u, w);
+    double thr = floor(nu_dt * 16777216.0);
+    return (double)(w[0] >> 8) < thr;
+}
+
+void orc_andersen_normals(uint64_t seed, uint64_t step, int64_t tag, double g[3])
+{
+    uint32_t w[4];
+    noise_words(seed, (uint32_t)tag, 0u, step, 2u, w);
+    const double two_pi = 6.283185307179586476925286766559;
+    double r0 = sqrt(-2.0 * log(orc_u24(w[0]))), r2 = sqrt(-2.0 * log(orc_u24(w[2])));
+    g[0] = r0 * cos(two_pi * orc_u24(w[1]));
+    g[1] = r0 * sin(two_pi * orc_u24(w[1]));
+    g[2] = r2 * cos(two_pi * orc_u24(w[3]));
 }
 
 /* ------------------------------------------------------------------------------------------ */
@@ -527,7 +556,53 @@ int orc_run(const orc_params *p, double *pos, double *vel, double *frc, uint64_t
     int status = ORC_OK;
     for (int64_t s = 0; s < n_steps; ++s) {
         uint64_t step = step0 + (uint64_t)s + 1;    /* time level of the new force */
-        if (p->integrator == ORC_NVE || p->integrator == ORC_LANGEVIN) {
+        if (p->integrator >= ORC_NOSE_HOOVER) {
+            /* Leapfrog with a thermostat on the half-step velocity u (vel holds the full-step v^m = u^{m-1/2} + dt/2 a^m
+               between steps; a = frc / m is a^m).  First step after a (re)start: u^{1/2} = v^0 + dt/2 a^0, thermostat off.
+                 Berendsen (c-30):   lambda = sqrt(1 + dt gamma (kT / T_half - 1));  u' = lambda (u + dt a)
+                 Nose-Hoover (c-28): xi += dt gamma^2 (T_half / kT - 1);  u' = [u (1 - dt xi / 2) + dt a] / (1 + dt xi / 2)
+                 Andersen (c-29):    u' = u + kick a, then beads hit by the bath draw u' = sqrt(kT/m) g
+               with T_half = 2 K_half / (3N - 3) the temperature of the previous half-step velocities; then
+               r += dt u';  a = F(r) / m;  v = u' + dt/2 a.                                                           */
+            const double dof = n > 1 ? 3.0 * n - 3.0 : 3.0;
+            const int have = p->thermo[0] != 0.0;
+            double sa = 1.0, sb = 1.0;              /* u' = sa u + sb kick a */
+            if (have && p->integrator == ORC_BERENDSEN) {
+                double t_half = 2.0 * p->thermo[1] / dof;
+                sa = sb = sqrt(1.0 + dt * p->gamma * (p->kT / t_half - 1.0));
+            } else if (have && p->integrator == ORC_NOSE_HOOVER) {
+                double t_half = 2.0 * p->thermo[1] / dof;
+                p->thermo[2] += dt * p->gamma * p->gamma * (t_half / p->kT - 1.0);
+                double h = 0.5 * dt * p->thermo[2];
+                sa = (1.0 - h) / (1.0 + h); sb = 1.0 / (1.0 + h);
+            }
+            const double kick = have ? dt : 0.5 * dt;
+            double k_half = 0.0;
+            for (int64_t i = 0; i < n; ++i) {
+                double a[3], u[3], m = p->mass[i];
+                for (int d = 0; d < 3; ++d) {
+                    a[d] = frc[3 * i + d] / m;
+                    double u_old = have ? vel[3 * i + d] - 0.5 * dt * a[d] : vel[3 * i + d];
+                    u[d] = sa * u_old + sb * kick * a[d];
+                }
+                if (p->integrator == ORC_ANDERSEN && orc_andersen_hit(p->seed, step - 1, i, p->gamma * dt)) {
+                    double g[3];
+                    orc_andersen_normals(p->seed, step - 1, i, g);
+                    for (int d = 0; d < 3; ++d) u[d] = sqrt(p->kT / m) * g[d];
+                }
+                for (int d = 0; d < 3; ++d) {
+                    vel[3 * i + d] = u[d];
+                    pos[3 * i + d] = wrap1(pos[3 * i + d] + dt * u[d], p->box[d]);
+                    k_half += 0.5 * m * u[d] * u[d];
+                }
+            }
+            p->thermo[0] = 1.0; p->thermo[1] = k_half;
+            int st = orc_compute_forces(p, pos, vel, step, frc, NULL);
+            if (st != ORC_OK) status = st;
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d)
+                    vel[3 * i + d] += 0.5 * dt * frc[3 * i + d] / p->mass[i];
+        } else if (p->integrator == ORC_NVE || p->integrator == ORC_LANGEVIN) {
             /* v' = v + dt/2 a;  r = r + dt v';  wrap;  a = F(r)/m;  v = v' + dt/2 a */
             for (int64_t i = 0; i < n; ++i)
                 for (int d = 0; d < 3; ++d) {

@@ -19,7 +19,7 @@ _LIB = os.path.join(_HERE, "libgm_oracle.so")
 
 PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 BOND = {"none": 0, "fene": 1, "harmonic": 2}
-INTEG = {"nve": 0, "langevin": 1, "gwvv": 2}
+INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5}
 ORC_ERR_BOND_OVERSTRETCH = -7
 
 
@@ -51,6 +51,7 @@ class _Params(C.Structure):
         ("n_dihedrals", C.c_int64),
         ("dih_i", C.c_void_p), ("dih_j", C.c_void_p), ("dih_k", C.c_void_p), ("dih_l", C.c_void_p), ("dih_type", C.c_void_p),
         ("dih_kk", C.c_void_p), ("dih_delta", C.c_void_p), ("dih_n", C.c_void_p),
+        ("thermo", C.c_void_p),
     ]
 
 
@@ -69,6 +70,10 @@ def lib():
         L.orc_pair_theta.restype = C.c_double
         L.orc_bead_xi.argtypes = [C.c_uint64, C.c_uint64, C.c_int64, C.c_void_p]
         L.orc_bead_xi.restype = None
+        L.orc_andersen_hit.argtypes = [C.c_uint64, C.c_uint64, C.c_int64, C.c_double]
+        L.orc_andersen_hit.restype = C.c_int
+        L.orc_andersen_normals.argtypes = [C.c_uint64, C.c_uint64, C.c_int64, C.c_void_p]
+        L.orc_andersen_normals.restype = None
         L.orc_min_image.argtypes = [C.c_double, C.c_double]
         L.orc_min_image.restype = C.c_double
         L.orc_neighbor_pairs.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_double, C.c_int32,
@@ -265,6 +270,8 @@ class Oracle:
         P.dih_i, P.dih_j, P.dih_k, P.dih_l = (_p(c).value for c in self._dih_cols)
         P.dih_type = _p(self._dih_type).value
         P.dih_kk = _p(self._dih_k).value; P.dih_delta = _p(self._dih_delta).value; P.dih_n = _p(self._dih_n).value
+        self.thermo = np.zeros(4)       # [have half-step velocity, its kinetic energy, Nose-Hoover xi, -]
+        P.thermo = _p(self.thermo).value
         if w.pair_style == "table":
             P.table = _p(self.table).value
             P.table_points = int(self.table.shape[2])
