@@ -65,7 +65,8 @@ enum {
 
 enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2, GM_PAIR_HARMONIC = 3, GM_PAIR_GAUSS = 4, GM_PAIR_TABLE = 5 };
 enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2 };
-enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2 };
+enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2,
+       GM_NVT_NOSE_HOOVER = 3, GM_NVT_ANDERSEN = 4, GM_NVT_BERENDSEN = 5 };   /* PAPER.md:L133, L137; DESIGN.md c-28..c-30 */
 enum { GM_ANGLE_NONE = 0, GM_ANGLE_HARMONIC = 1 /* Eq. (8): k (theta - theta0)^2 */, GM_ANGLE_COSINE = 2 /* Eq. (9): k (cos theta - cos theta0)^2 */ };
 
 #define GM_MAX_TYPES 8       /* particle types; pair tables are n_types x n_types */
@@ -86,8 +87,10 @@ typedef struct {
     uint64_t seed;                   /* key of the counter-based Philox4x32-10 noise               */
     int32_t pair_style;              /* GM_PAIR_*                                                  */
     int32_t bond_style;              /* GM_BOND_*                                                  */
-    int32_t integrator;              /* GM_NVE | GM_LANGEVIN | GM_DPD_GWVV                         */
-    float kT, gamma, lambda;         /* thermostat temperature, friction, GW-VV lambda             */
+    int32_t integrator;              /* GM_NVE | GM_LANGEVIN | GM_DPD_GWVV | GM_NVT_*              */
+    float kT, gamma, lambda;         /* thermostat temperature; friction (Langevin, DPD) or coupling rate of the NVT
+                                        thermostats (Nose-Hoover 1/tau, Berendsen 1/tau_T, Andersen collision frequency);
+                                        GW-VV lambda */
     int32_t sfc_period;              /* largest number of steps between two SFC sorts of the particle arrays (every
                                         neighbor rebuild sorts; > 0 forces a rebuild after this many steps) */
     int32_t nl_row_capacity;         /* rows of the NL table; 0 = choose from density              */
@@ -203,8 +206,9 @@ gm_status gm_compute_forces(gm_system *s);
 gm_status gm_step(gm_system *s, int64_t n_steps);
 
 /* Switch the integrator of an existing system (e.g. Langevin equilibration, then NVE: BASELINE.json
- * config 3).  integrator: GM_NVE | GM_LANGEVIN (GM_DPD_GWVV only on a GM_PAIR_DPD system and vice
- * versa); kT, gamma as in gm_config.  The state (positions, half-step velocities, step counter,
+ * config 3).  integrator: GM_NVE | GM_LANGEVIN | GM_NVT_* (GM_DPD_GWVV only on a GM_PAIR_DPD system and vice
+ * versa); kT, gamma as in gm_config.  The first step after a switch to an NVT thermostat runs without it (the
+ * temperature of the half-step velocities it acts on is measured in that step).  The state (positions, half-step velocities, step counter,
  * neighbor list) is kept.  Errors: INVALID_ARG. */
 gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma);
 

@@ -54,7 +54,8 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (c->table_points < 0 || c->table_points > (1 << 20) || ((c->pair_style == GM_PAIR_TABLE) != (c->table_points > 0)))
         return GM_ERR_INVALID_ARG;
     if (c->bond_style < GM_BOND_NONE || c->bond_style > GM_BOND_HARMONIC) return GM_ERR_INVALID_ARG;
-    if (c->integrator < GM_NVE || c->integrator > GM_DPD_GWVV) return GM_ERR_INVALID_ARG;
+    if (c->integrator < GM_NVE || c->integrator > GM_NVT_BERENDSEN) return GM_ERR_INVALID_ARG;
+    if ((c->integrator == GM_DPD_GWVV) != (c->pair_style == GM_PAIR_DPD)) return GM_ERR_INVALID_ARG;
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
@@ -133,7 +134,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     // lanes per bead of the step kernel: 8 lanes sharing a bead (shuffle reduction) measured SLOWER than one
     // thread per bead on every config, so it is opt-in
     P->angle_style = c->angle_style; P->max_angles = c->max_angles_per_particle; P->max_dihedrals = c->max_dihedrals_per_particle;
-    P->step_subw = ((c->flags & GM_FLAG_STEP_SUBWARP) && P->max_angles + P->max_dihedrals == 0) ? 8 : 1;
+    P->step_subw = ((c->flags & GM_FLAG_STEP_SUBWARP) && P->max_angles + P->max_dihedrals == 0 && c->integrator <= GM_DPD_GWVV) ? 8 : 1;
     P->capq = cap / 4;
     P->minq = std::min(4, P->capq);
     // tile windows (gm_nlist.cu): every pair style but DPD (which also gathers velocities), one thread per bead.  A window holds the hulls of the x runs
@@ -843,8 +844,10 @@ extern "C" gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4])
 extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma)
 {
     if (!s) return GM_ERR_INVALID_ARG;
-    if (integrator < GM_NVE || integrator > GM_DPD_GWVV)
+    if (integrator < GM_NVE || integrator > GM_NVT_BERENDSEN)
         return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: unknown integrator%s");
+    if (integrator >= GM_NVT_NOSE_HOOVER && s->P.step_subw != 1)
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: the NVT thermostats do not run on the sub-warp step kernel%s");
     if ((integrator == GM_DPD_GWVV) != (s->P.pair_style == GM_PAIR_DPD))
         return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: GM_DPD_GWVV goes with GM_PAIR_DPD only%s");
     if (!(kT >= 0.f) || !(gamma >= 0.f)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: kT, gamma must be >= 0%s");
@@ -854,6 +857,9 @@ extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, f
     s->P.lang_amp2 = (float)(6.0 * (double)gamma * (double)kT / (double)s->P.dt);
     s->force_current = false;
     drop_graphs(s);
+    CU(cudaSetDevice(s->cfg.device));
+    gm_launch_thermo_reset(s->D, s->cur, s->st);
+    CU(cudaGetLastError());
     return GM_OK;
 }
 

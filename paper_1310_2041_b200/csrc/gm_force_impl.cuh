@@ -22,6 +22,9 @@
 // The gather loop is software-pipelined: the index quads of the next batch and all position gathers
 // of this batch are in flight before the first force term is evaluated.
 #pragma once
+#include <cooperative_groups.h>
+#include <cooperative_groups/reduce.h>
+
 #include "gm_internal.cuh"
 
 #define FORCE_BLOCK 128          // = GM_TILE: a CTA of k_force / k_energy owns one tile
@@ -543,6 +546,74 @@ __device__ __forceinline__ float3 bead_accel(const GmParams &P, const Src &S, in
     return a;
 }
 
+// ---- NVT thermostats in leapfrog form (readings c-28..c-30) ----------------------------
+// u' = sa u + sb kick a with (sa, sb) from the temperature T_half of the half-step velocities the previous step wrote:
+//   Berendsen:   lambda = sqrt(1 + dt gamma (kT / T_half - 1)), sa = sb = lambda
+//   Nose-Hoover: xi += dt gamma^2 (T_half / kT - 1), h = dt xi / 2, sa = (1 - h) / (1 + h), sb = 1 / (1 + h)
+// Every thread derives the same pair from the control block (a few flops on uniform values); thread 0 of block 0 stores
+// the new xi and clears the accumulator of the step after next (three-slot rotation: no slot is read and written in one
+// launch).  The first kick after a (re)start runs without the thermostat.
+struct Thermo { float sa, sb; bool on; };
+
+__device__ __forceinline__ Thermo thermo_begin(const GmParams &P, const GmDev &D, unsigned long long step, float kick)
+{
+    Thermo T;
+    T.sa = 1.0f; T.sb = 1.0f; T.on = false;
+    if (P.integrator != GM_NVT_NOSE_HOOVER && P.integrator != GM_NVT_BERENDSEN) return T;
+    T.on = true;
+    GmCtl *c = D.ctl;
+    const int r = (int)(step % 3ull), w = (int)((step + 1ull) % 3ull), z = (int)((step + 2ull) % 3ull);
+    const bool active = step > c->thermo_start;
+    double xi = c->xi[r];
+    if (active) {
+        const double dof = P.n > 1 ? 3.0 * P.n - 3.0 : 3.0;
+        const double t_half = c->ke2[r] / dof;
+        if (P.integrator == GM_NVT_BERENDSEN) {
+            const double lam = sqrt(1.0 + (double)P.dt * P.gamma * ((double)P.kT / t_half - 1.0));
+            T.sa = T.sb = (float)lam;
+        } else {
+            xi += (double)P.dt * P.gamma * P.gamma * (t_half / (double)P.kT - 1.0);
+            const double h = 0.5 * (double)P.dt * xi;
+            T.sa = (float)((1.0 - h) / (1.0 + h)); T.sb = (float)(1.0 / (1.0 + h));
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) { c->xi[w] = xi; c->ke2[z] = 0.0; }
+    (void)kick;
+    return T;
+}
+
+// sum of m u'^2 over the lanes that hold a bead -> the accumulator the next step reads (one double atomic per warp)
+__device__ __forceinline__ void thermo_accumulate(const GmDev &D, unsigned long long step, float m_u2)
+{
+    namespace cg = cooperative_groups;
+    const cg::coalesced_group g = cg::coalesced_threads();
+    const float sum = cg::reduce(g, m_u2, cg::plus<float>());
+    if (g.thread_rank() == 0) atomicAdd(&D.ctl->ke2[(int)((step + 1ull) % 3ull)], (double)sum);
+}
+
+// Andersen thermostat (c-29): the bead collides with the heat bath in this kick iff the top 24 bits of Philox(tag, 0,
+// step, 3) word 0 are below floor(nu dt 2^24); its new velocity is sqrt(kT / m) times three Box-Muller normals from the
+// words of Philox(tag, 0, step, 2).
+__device__ __forceinline__ void andersen_collide(const GmParams &P, const Src &S, int i, unsigned long long step, float mass,
+                                                 float &ux, float &uy, float &uz)
+{
+    const uint32_t tag = (uint32_t)S.tag[i];
+    const uint2 key = make_uint2(P.seed_lo, P.seed_hi);
+    const uint4 d = gm_philox4x32_10(make_uint4(tag, 0u, (uint32_t)step, 3u), key);
+    const float thr = floorf(P.gamma * P.dt * 16777216.0f);
+    if ((float)(d.x >> 8) < thr) {
+        const uint4 w = gm_philox4x32_10(make_uint4(tag, 0u, (uint32_t)step, 2u), key);
+        const float u0 = ((float)(w.x >> 8) + 0.5f) * (1.0f / 16777216.0f), u1 = ((float)(w.y >> 8) + 0.5f) * (1.0f / 16777216.0f);
+        const float u2 = ((float)(w.z >> 8) + 0.5f) * (1.0f / 16777216.0f), u3 = ((float)(w.w >> 8) + 0.5f) * (1.0f / 16777216.0f);
+        const float r0 = sqrtf(-2.0f * logf(u0)), r2 = sqrtf(-2.0f * logf(u2));
+        float s1, c1, s3, c3;
+        sincospif(2.0f * u1, &s1, &c1);
+        sincospif(2.0f * u3, &s3, &c3);
+        const float a = sqrtf(P.kT / mass);
+        ux = a * r0 * c1; uy = a * r0 * s1; uz = a * r2 * c3;
+    }
+}
+
 // ---- the per-step work of one bead (MODE_STEP) / its materialised force (MODE_FORCES) -----------------
 // Called by all threads of the CTA (window staging is a block-collective step); threads past the last bead
 // (valid = false) work on the pad slots (far away, NN = 0, no bonds) and store nothing.
@@ -584,7 +655,16 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
     // a8: kick, drift, wrap
     if (PAIR == GM_PAIR_DPD)
         D.vt[parity ^ 1][i] = make_float4(u.x + kick_vt * a.x, u.y + kick_vt * a.y, u.z + kick_vt * a.z, vti.w);
-    const float ux = u.x + kick * a.x, uy = u.y + kick * a.y, uz = u.z + kick * a.z;
+    float ux = u.x + kick * a.x, uy = u.y + kick * a.y, uz = u.z + kick * a.z;
+    if (P.integrator >= GM_NVT_NOSE_HOOVER) {
+        const Thermo th = thermo_begin(P, D, step, kick);
+        if (th.on) {
+            ux = th.sa * u.x + th.sb * kick * a.x; uy = th.sa * u.y + th.sb * kick * a.y; uz = th.sa * u.z + th.sb * kick * a.z;
+            thermo_accumulate(D, step, u.w * (ux * ux + uy * uy + uz * uz));
+        } else {
+            andersen_collide(P, S, i, step, u.w, ux, uy, uz);
+        }
+    }
     D.vel[i] = make_float4(ux, uy, uz, u.w);
     // positions are NOT wrapped here: between two rebuilds a bead may sit up to skin/2 outside the box (the
     // sort wraps it back), so that every listed pair keeps the periodic image it had at the build

@@ -58,6 +58,11 @@ struct GmCtl {
     int err;
     int go;                        // decision of the last k_gate: the rebuild chain runs iff != 0
     int n_glob_tiles;              // tiles of the current list that are NOT window-staged (32-bit rows, gathers from HBM/L2)
+    // NVT thermostats (Nose-Hoover, Berendsen): sum of m u^2 over the half-step velocities written by the step kernel of
+    // time level m goes to ke2[(m + 1) % 3]; that kernel reads ke2[m % 3] and clears ke2[(m + 2) % 3]; xi likewise
+    double ke2[3];
+    double xi[3];
+    unsigned long long thermo_start;   // time level of the first kick after a (re)start: the thermostat acts from the next
 };
 
 // Per-type-pair coefficients.  LJ:       c0 = r_c^2, c1 = 48 eps sigma^12, c2 = 24 eps sigma^6, c3 = U_shift.
@@ -153,6 +158,7 @@ void gm_launch_unpack(const GmParams &P, const GmDev &D, int cur, float *pos3, f
 void gm_launch_unpack_neighbors(const GmParams &P, const GmDev &D, int *nn_out, int *nl_out, long long stride,
                                 int t0, int t1, cudaStream_t st);
 void gm_launch_topo(const GmParams &P, const GmDev &D, int parity, cudaStream_t st);     // angle + dihedral forces -> D.ftopo
+void gm_launch_thermo_reset(const GmDev &D, int parity, cudaStream_t st);
 void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, int parity, cudaStream_t st);
 void gm_launch_init_pad(const GmParams &P, const GmDev &D, cudaStream_t st);
 

@@ -104,10 +104,22 @@ __global__ void k_set_ctl(GmDev D, unsigned long long step, int reset_all, int p
     c->need = GM_NEVER;
     c->rebuilt_at = fresh ? step : GM_NEVER;
     c->go = 0;
+    for (int q = 0; q < 3; ++q) { c->ke2[q] = 0.0; c->xi[q] = 0.0; }
+    c->thermo_start = step;
     if (reset_all) {
         c->n_rebuilds = 0; c->sum_nn = 0; c->max_nn = 0; c->err = 0; c->n_glob_tiles = 0;
     }
 }
+
+// gm_set_integrator: the thermostat state starts afresh at the current time level
+__global__ void k_thermo_reset(GmDev D, int parity)
+{
+    GmCtl *c = D.ctl;
+    for (int q = 0; q < 3; ++q) { c->ke2[q] = 0.0; c->xi[q] = 0.0; }
+    c->thermo_start = c->step[parity];
+}
+
+void gm_launch_thermo_reset(const GmDev &D, int parity, cudaStream_t st) { k_thermo_reset<<<1, 1, 0, st>>>(D, parity); }
 
 void gm_launch_set_ctl(const GmDev &D, unsigned long long step, int reset_all, int parity, cudaStream_t st)
 {
