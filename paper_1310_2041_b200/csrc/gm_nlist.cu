@@ -19,6 +19,9 @@
 // whatever the row capacity, which leaves the rest of the SM's 228 KB to L1 for the candidate loads.
 #include "gm_internal.cuh"
 
+#ifndef NL_MINB_WIN
+#define NL_MINB_WIN 6          // resident CTAs per SM the window-system build is compiled for (77 registers, no spills; 8 -> 64 registers with spills measured 1 % slower on C2 / C5)
+#endif
 #define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 8)
 #ifndef NL_WARPS
 #define NL_WARPS 4
@@ -292,7 +295,7 @@ __device__ __forceinline__ void nl_scan_bead(const GmParams &P, const GmDev &D, 
 // WINS: the system uses tile windows (GmParams::use_win) -- compiled apart so that systems without them (DPD) run the
 // plain kernel (56 registers, 9 CTAs per SM)
 template <int TRIP, bool WINS>
-__global__ void __launch_bounds__(NL_WARPS * 32, WINS ? 8 : 9)
+__global__ void __launch_bounds__(NL_WARPS * 32, WINS ? NL_MINB_WIN : 9)
 k_nl_build(const __grid_constant__ GmParams P, GmDev D)
 {
     if (!D.ctl->go) return;
