@@ -168,15 +168,14 @@ def describe(w) -> str:
 
 
 def src_sha16() -> str:
-    """Hash of the CUDA sources: the ncu-derived figures under profiles/ carry the hash of the code they were taken
-    on and are only quoted while it still matches (otherwise the field is null)."""
+    """Hash of the step kernel's CUDA sources: the ncu-derived figures under profiles/ carry the hash of the code they were
+    taken on and are only quoted while it still matches (otherwise the field is null)."""
     import hashlib
     h = hashlib.sha256()
     d = os.path.join(ROOT, "paper_1310_2041_b200", "csrc")
-    for f in sorted(os.listdir(d)):
-        if f.endswith((".cu", ".cuh")):
-            with open(os.path.join(d, f), "rb") as fh:
-                h.update(fh.read())
+    for f in ("gm_internal.cuh", "gm_force_impl.cuh", "gm_force.cu", "gm_force_dpd.cu"):
+        with open(os.path.join(d, f), "rb") as fh:
+            h.update(fh.read())
     return h.hexdigest()[:16]
 
 
