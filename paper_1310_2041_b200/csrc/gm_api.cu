@@ -680,16 +680,24 @@ static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
     s->cur = 0;
     cudaError_t e = cudaStreamBeginCapture(s->cap_st, cudaStreamCaptureModeRelaxed);
     bool ok = (e == cudaSuccess);
+    // one conditional handle per timestep (default 0 at every graph launch): timestep 0 is gated by a one-thread kernel
+    // that reads ctl->need; the step kernel of timestep k - 1 raises the handle of timestep k itself
+    std::vector<cudaGraphConditionalHandle> hs((size_t)nsteps);
+    if (ok && s->use_cond) {
+        cudaStreamCaptureStatus status;
+        cudaGraph_t g = nullptr;
+        ok = cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, nullptr, nullptr) == cudaSuccess;
+        for (int k = 0; ok && k < nsteps; ++k)
+            ok = cudaGraphConditionalHandleCreate(&hs[k], g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
+    }
     for (int k = 0; ok && k < nsteps; ++k) {
         if (s->use_cond) {
             cudaStreamCaptureStatus status;
             cudaGraph_t g = nullptr;
             const cudaGraphNode_t *deps = nullptr;
             size_t ndeps = 0;
-            ok = cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, &deps, &ndeps) == cudaSuccess;
-            cudaGraphConditionalHandle h;
-            ok = ok && cudaGraphConditionalHandleCreate(&h, g, 0, cudaGraphCondAssignDefault) == cudaSuccess;
-            if (ok) gm_launch_gate(s->D, 1, s->cur, (unsigned long long)h, 1, s->cap_st);
+            const cudaGraphConditionalHandle h = hs[k];
+            if (k == 0) gm_launch_gate(s->D, 1, s->cur, (unsigned long long)h, 1, s->cap_st);
             ok = ok && cudaStreamGetCaptureInfo(s->cap_st, &status, nullptr, &g, &deps, &ndeps) == cudaSuccess;
             cudaGraphNodeParams np = {};
             np.type = cudaGraphNodeTypeConditional;
@@ -703,6 +711,8 @@ static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
                 ok = cudaStreamBeginCaptureToGraph(s->cap_st2, body, nullptr, nullptr, 0,
                                                    cudaStreamCaptureModeRelaxed) == cudaSuccess;
                 if (ok) {
+                    // the body of a gate-less timestep starts with the gate's bookkeeping (ctl->go, rebuild counter)
+                    if (k > 0) gm_launch_gate(s->D, 1, s->cur, 0ull, 0, s->cap_st2);
                     gm_launch_sort(s->P, s->D, s->cur, s->cap_st2);
                     gm_launch_nl_build(s->P, s->D, s->cap_st2);
                     cudaGraph_t tmp = nullptr;
@@ -714,7 +724,11 @@ static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
         } else {
             enqueue_rebuild(s, 1, s->cap_st);
         }
-        if (ok) enqueue_step_kernel(s, true, s->cap_st);
+        if (ok) {
+            s->D.next_cond = (s->use_cond && k + 1 < nsteps) ? (unsigned long long)hs[k + 1] : 0ull;
+            enqueue_step_kernel(s, true, s->cap_st);
+            s->D.next_cond = 0ull;
+        }
     }
     e = cudaStreamEndCapture(s->cap_st, &graph);
     ok = ok && e == cudaSuccess && graph != nullptr;

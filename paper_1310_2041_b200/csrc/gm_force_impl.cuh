@@ -52,6 +52,14 @@ static_assert(WIDE_BLOCK == GM_TILE && FORCE_BLOCK == GM_TILE, "a CTA of the win
 #define GM_LJ_NQ 1               // quads (of 4 list entries) per batch of the LJ gather loop
 #endif
 
+// a4: the list must be rebuilt before the forces of time level step + 1.  Inside a step graph the conditional node of the
+// next timestep is switched on right here (GmDev::next_cond); otherwise the next gate kernel reads ctl->need.
+__device__ __forceinline__ void raise_rebuild(const GmDev &D, unsigned long long step)
+{
+    D.ctl->need = step + 1;
+    if (D.next_cond) cudaGraphSetConditional((cudaGraphConditionalHandle)D.next_cond, 1u);
+}
+
 struct BeadForce {
     float fx, fy, fz;
     float pe_pair, pe_bond;   // this bead's half share
@@ -672,7 +680,7 @@ __device__ __forceinline__ void bead_step(const GmParams &P, const GmDev &D, con
     D.pos[parity ^ 1][i] = make_float4(x, y, z, pi.w);
     // a4: displacement since the last NL build (ref holds the wrapped position the bead had then)
     const float dx = x - rf.x, dy = y - rf.y, dz = z - rf.z;
-    if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) D.ctl->need = step + 1;
+    if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) raise_rebuild(D, step);
 }
 
 // gm_compute_forces: one block per 128 beads.
@@ -707,7 +715,7 @@ k_step(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, floa
         // a2: at most sfc_period steps between two sorts
         if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
             step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
-            D.ctl->need = step + 1;
+            raise_rebuild(D, step);
     }
     const int i = blockIdx.x * BLOCK + threadIdx.x;
     GM_CPT_DECL(PAIR, BLOCK);
@@ -734,7 +742,7 @@ k_step_sub(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, 
         D.ctl->step[parity ^ 1] = step + 1;
         if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
             step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
-            D.ctl->need = step + 1;
+            raise_rebuild(D, step);
     }
     const long long gt = (long long)blockIdx.x * SUB_BLOCK + threadIdx.x;
     const int i = (int)(gt / SUBW), sub = (int)(gt % SUBW);
@@ -798,7 +806,7 @@ k_step_sub(const __grid_constant__ GmParams P, GmDev D, int parity, float kick, 
     const float x = pi.x + P.dt * ux, y = pi.y + P.dt * uy, z = pi.z + P.dt * uz;
     D.pos[parity ^ 1][i] = make_float4(x, y, z, pi.w);
     const float dx = x - rf.x, dy = y - rf.y, dz = z - rf.z;
-    if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) D.ctl->need = step + 1;
+    if (!(dx * dx + dy * dy + dz * dz <= P.half_skin2)) raise_rebuild(D, step);
 }
 
 // ---- a9 energies: grid-stride, fp64 accumulation, per-block partials in fixed order ----------------

@@ -131,6 +131,9 @@ struct GmDev {
     float *stage;            // 11 ns floats: I/O staging (pos3, vel3, force3, type, mass)
     double *esum;            // [GM_ESUM_BLOCKS * 8] partials, then [8] totals at the end
     GmCtl *ctl;
+    // Conditional-graph handle of the NEXT timestep's rebuild node (0 = none): inside a step graph the step kernel that
+    // sees a displacement beyond skin/2 raises it itself, so only the first timestep of a graph needs a gate kernel
+    unsigned long long next_cond;
 };
 
 #define GM_ESUM_BLOCKS 1184      // 8 x 148: grid of the energy reduction
