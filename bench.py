@@ -311,6 +311,9 @@ def main():
     ap.add_argument("--no-cond-nodes", action="store_true",
                     help="gate the rebuild with early-exit kernels instead of a conditional graph node "
                          "(ncu cannot profile kernel nodes of graphs that hold conditional nodes)")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="GM_FLAG_NO_GRAPH: launch kernel by kernel (for ncu: it does not profile graph kernel nodes that can "
+                         "set a conditional handle, which the step kernel can)")
     ap.add_argument("--skin", type=float, default=None,
                     help="override the config's neighbor skin (a tuning knob that never changes results; "
                          "BASELINE.json gives none for C4)")
@@ -354,7 +357,8 @@ def main():
 
     inner = args.inner or (w.sfc_period if w.sfc_period > 0 else 500)
     hbm_gbs, peak_src = load_peaks()
-    flags = (gm.GM_FLAG_NO_COND_NODES if args.no_cond_nodes else 0) | (gm.GM_FLAG_NO_WINDOWS if args.no_windows else 0)
+    flags = (gm.GM_FLAG_NO_COND_NODES if args.no_cond_nodes else 0) | (gm.GM_FLAG_NO_WINDOWS if args.no_windows else 0) | \
+            (gm.GM_FLAG_NO_GRAPH if args.no_graph else 0)
     tune = {k: int(v) for k, v in (kv.split("=") for kv in args.tune)}
     flags |= tune.pop("flags", 0)
     stream = torch.cuda.current_stream(dev)
