@@ -14,6 +14,7 @@ HEADERS = [os.path.join(CSRC, "gm_internal.cuh"), os.path.join(CSRC, "gm_force_i
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-Xptxas", "-v"]
+FLAGS += os.environ.get("GM_NVCC_FLAGS", "").split()      # extra -D switches of the kernel sources (e.g. -DNL_COOP=0)
 
 
 def stale() -> bool:

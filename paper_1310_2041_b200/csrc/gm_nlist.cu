@@ -23,6 +23,9 @@
 #define NL_MINB_WIN 6          // resident CTAs per SM the window-system build is compiled for (77 registers, no spills; 8 -> 64 registers with spills measured 1 % slower on C2 / C5)
 #endif
 #define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 8)
+#ifndef NL_COOP
+#define NL_COOP 1            // dense cells: warps of one piece scan the union of their lanes' runs together (nl_scan_warp)
+#endif
 #ifndef NL_WARPS
 #define NL_WARPS 4
 #endif
@@ -144,6 +147,123 @@ __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int 
         r.k = (int)(kb >> 7);
         if (r.k - r.flushed >= 16) nl_flush16<W16>(r);
     }
+}
+
+// ---- warp-cooperative scan (dense cells: TRIP == 8) ----------------------------------------------------------------
+// With several beads per cell the 32 beads of a warp sit in a handful of x-adjacent cells of ONE row, and their runs in
+// each of the nine neighbor rows overlap almost entirely: the union of the 32 runs is 1.7 x one run on C5.  Per-lane
+// scanning reads that union 32 times through the L1 data pipe (each LDG.128 of 32 slightly shifted addresses takes ~6
+// wavefronts; the pipe was at 89 % on C5).  Here the warp loads the union once, 32 candidates per coalesced LDG.128, into
+// a small shared-memory buffer, and every lane tests every candidate of the union from a broadcast LDS.128 (one wavefront
+// per candidate per warp).  A candidate outside the lane's own run is more than r_list away in x (sx cells), so the
+// distance test alone decides and the row comes out identical, entry for entry, to the per-lane scan.  All lanes run the
+// same trips, so the flush is taken together too.  Warps that are not of one piece (a lane near a periodic face, two
+// rows, pad lanes) keep the per-lane scan.
+template <bool SELF>
+__device__ __forceinline__ void nl_append_all(uint32_t &kb, uint32_t lb, float r2, float r_list2, int s, int i)
+{
+    if (SELF)
+        asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %5, %6, 0xEA;\n\t"
+                     "setp.lt.f32 p, %1, %2;\n\t"
+                     "setp.ne.and.s32 p, %3, %4, p;\n\t@p st.shared.b32 [t], %3;\n\t@p add.u32 %0, %0, 128;\n\t}"
+                     : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(s), "r"(i), "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
+    else
+        asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %5, %6, 0xEA;\n\t"
+                     "setp.lt.f32 p, %1, %2;\n\t"
+                     "@p st.shared.b32 [t], %3;\n\t@p add.u32 %0, %0, 128;\n\t}"
+                     : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(s), "r"(i), "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
+}
+
+// write entries [flushed, flushed + 8) of the row from the ring to the tile: one oct of window offsets or two quads
+template <bool W16>
+__device__ __forceinline__ void nl_flush8(NlRow &r)
+{
+    if (r.flushed + 8 <= r.cap) {
+        const int e = r.flushed;
+        int v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) v[u] = r.ring[((e + u) & (NL_STAGE - 1)) * 32];
+        if (W16) {
+            r.tile[(e >> 3) * 32] = make_int4((int)nl_pack2(v[0], v[1]), (int)nl_pack2(v[2], v[3]),
+                                              (int)nl_pack2(v[4], v[5]), (int)nl_pack2(v[6], v[7]));
+        } else {
+            r.tile[(e >> 2) * 32] = make_int4(v[0], v[1], v[2], v[3]);
+            r.tile[((e >> 2) + 1) * 32] = make_int4(v[4], v[5], v[6], v[7]);
+        }
+    }
+    r.flushed += 8;
+}
+
+// one row run of the union [u0, u1) against the warp's 32 beads; buf: the warp's [2][32] candidate buffer, b: the
+// half to fill next
+template <bool SELF, bool W16>
+__device__ __forceinline__ void nl_union_run(const float4 *__restrict__ ref, int u0, int u1, int delta, int i, const float4 pi,
+                                             float r_list2, NlRow &r, uint32_t &kb, float4 *buf, int &b)
+{
+    const unsigned full = 0xffffffffu;
+    const int lane = threadIdx.x & 31;
+    const int ie = i + delta;
+    if (u0 >= u1) return;
+    float4 qn = __ldg(ref + (u0 + lane < u1 ? u0 + lane : u0));
+    for (int base = u0; base < u1; base += 32) {
+        const int cnt = min(32, u1 - base);
+        float4 *cb = buf + b * 32;
+        cb[lane] = lane < cnt ? qn : make_float4(1e18f, 1e18f, 1e18f, 0.f);      // the tail of the chunk: far away
+        __syncwarp();
+        // the next chunk's candidates are in flight while this one is tested.  One __syncwarp per chunk is enough:
+        // half b is written again two chunks on, behind the barrier of the chunk in between
+        if (base + 32 < u1) qn = __ldg(ref + (base + 32 + lane < u1 ? base + 32 + lane : base + 32));
+        for (int j = 0; j < cnt; j += 8) {
+            float4 q[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) q[u] = cb[j + u];
+            const int se = base + j + delta;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const float dx = pi.x - q[u].x, dy = pi.y - q[u].y, dz = pi.z - q[u].z;
+                const float r2 = dx * dx + dy * dy + dz * dz;
+                nl_append_all<SELF>(kb, r.lb, r2, r_list2, se + u, ie);
+            }
+            // fewer than 16 entries are staged before a trip and at most 8 arrive: when any lane reaches 16, every lane
+            // holding a whole oct writes it, which leaves all lanes below 16 again (ring of 32)
+            r.k = (int)(kb >> 7);
+            if (__any_sync(full, r.k - r.flushed >= 16)) {
+                if (r.k - r.flushed >= 8) nl_flush8<W16>(r);
+            }
+        }
+        b ^= 1;
+    }
+}
+
+// the nine runs of a warp of one piece: all 32 lanes hold beads of row (cy, cz), cells cx_lo .. cx_hi, none within
+// sx cells of an x face or in a boundary row (so no periodic shifts and no wrapped pieces)
+template <bool WIN>
+__device__ __forceinline__ void nl_scan_warp(const GmParams &P, const GmDev &D, int i, const float4 pi, int cx_lo, int cx_hi,
+                                             int cy, int cz, const NlWin &W, NlRow &row, float4 *buf)
+{
+    const float4 *__restrict__ ref = D.ref;
+    const int *__restrict__ cstart = D.cstart;
+    const uint32_t *__restrict__ rr = D.row_rank;
+    const int ncx = P.nc[0], ncy = P.nc[1];
+    const float rl2 = P.r_list2;
+    const int c0 = cx_lo - P.sx, c1 = cx_hi + P.sx + 1;
+    uint32_t kb = (uint32_t)row.k * 128u;
+    int b = 0;
+#pragma unroll 1
+    for (int run = 0; run < 9; ++run) {
+        const int oz = run / 3 - 1, oy = run - 3 * (run / 3) - 1;
+        const int slot = W.group * 27 + run * 3;
+        const int r0 = (WIN && !W.whole) ? W.rng[slot].w : (int)__ldg(rr + (cz + oz) * ncy + cy + oy) * ncx;
+        const int u0 = __ldg(cstart + r0 + c0), u1 = __ldg(cstart + r0 + c1);
+        int delta = 0;
+        if (WIN) {
+            const int4 g = W.rng[slot];
+            delta = g.y - g.x;
+        }
+        if (run == 4) nl_union_run<true, WIN>(ref, u0, u1, delta, i, pi, rl2, row, kb, buf, b);
+        else nl_union_run<false, WIN>(ref, u0, u1, delta, i, pi, rl2, row, kb, buf, b);
+    }
+    row.k = (int)(kb >> 7);
 }
 
 // Window set-up of a tile (all threads of the CTA; block-level barriers inside): range slots -> rng[], descriptor ->
@@ -310,6 +430,7 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     int4 *rng = reinterpret_cast<int4 *>(nl_ring + NL_WARPS * NL_STAGE * 32);       // [GM_WIN_SLOTS], then cell[GM_TILE], mode
     int4 *cell = rng + GM_WIN_SLOTS;
     int *sh_mode = reinterpret_cast<int *>(cell + GM_TILE);
+    float4 *ubuf = reinterpret_cast<float4 *>(cell + GM_TILE + 1) + wid * 64;     // [NL_WARPS][2][32] candidates (TRIP == 8)
     NlWin W;
     W.rng = rng;
     W.group = 0;
@@ -332,11 +453,23 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     int mode = 0;
     if (WINS && (int)(blockIdx.x * blockDim.x) < P.n)           // CTA-uniform: the tile holds at least one bead
         mode = nl_window(P, D, blockIdx.x, valid, cx, cy, cz, rng, cell, sh_mode, &W.group);
-    if (valid) {
+    bool scanned = false;
+    if (TRIP == 8 && WINS && NL_COOP) {      // measured: C5 1 928 -> 1 899 us per timestep; the DPD melt C4 (no windows, 9 CTAs per SM) lost 1.7 % and keeps the per-lane scan
+        const unsigned full = 0xffffffffu;
+        const int cy0 = __shfl_sync(full, cy, 0), cz0 = __shfl_sync(full, cz, 0);
+        const bool inner = valid && cx >= P.sx && cx + P.sx <= P.nc[0] - 1 && cy > 0 && cy < P.nc[1] - 1 && cz > 0 && cz < P.nc[2] - 1;
+        if (__all_sync(full, inner && cy == cy0 && cz == cz0)) {
+            const int cx_lo = __reduce_min_sync(full, cx), cx_hi = __reduce_max_sync(full, cx);
+            if (WINS && mode) nl_scan_warp<true>(P, D, i, pi, cx_lo, cx_hi, cy, cz, W, row, ubuf);
+            else nl_scan_warp<false>(P, D, i, pi, cx_lo, cx_hi, cy, cz, W, row, ubuf);
+            scanned = true;
+        }
+    }
+    if (valid && !scanned) {
         if (WINS && mode) nl_scan_bead<TRIP, true>(P, D, i, pi, cx, cy, cz, W, row);
         else nl_scan_bead<TRIP, false>(P, D, i, pi, cx, cy, cz, W, row);
-        if (row.k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
     }
+    if (valid && row.k > cap) atomicOr(&D.ctl->err, GM_DEV_ERR_OVERFLOW);
     // the tail of the row: whole quads (octs), at least minq quads in all (the force kernel loads those before
     // it knows NN), padded with the far-away bead (index n; window offset 0)
     const int kc = min(row.k, cap);
@@ -420,7 +553,7 @@ int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 8 
 int gm_nl_smem_bytes(const GmParams &P)
 {
     (void)P;
-    return NL_WARPS * NL_STAGE * 32 * 4 + 4096 + (GM_WIN_SLOTS + GM_TILE + 1) * 16;
+    return NL_WARPS * NL_STAGE * 32 * 4 + 4096 + (GM_WIN_SLOTS + GM_TILE + 1) * 16 + NL_WARPS * 64 * 16;
 }
 
 cudaError_t gm_nl_prepare(const GmParams &P)
