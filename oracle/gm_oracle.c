@@ -29,6 +29,9 @@
  *     for cis, pi for trans: DESIGN.md readings c-26, c-27)
  *   - NVT by Nose-Hoover, Andersen or Berendsen thermostat: named only
  *     (leapfrog forms with the temperature of the half-step velocities; readings c-28..c-30)
+ *   - NPH / NPT by the Andersen barostat: named only
+ *     (Andersen 1980's extended Hamiltonian with the volume as a coordinate, integrated by a symmetric
+ *     splitting; NPT adds Andersen's stochastic collisions; reading c-31)
  *   - FENE, WCA, the DPD force law, Philox: not in PAPER.md; readings c-3..c-8:
  *     Kremer-Grest FENE, Groot-Warren DPD with uniform unit-variance noise, Philox4x32-10
  *     (Salmon et al., SC'11) keyed (seed; min tag, max tag, step, stream).
@@ -50,7 +53,8 @@
 
 enum { ORC_PAIR_NONE = 0, ORC_PAIR_LJ = 1, ORC_PAIR_DPD = 2, ORC_PAIR_HARMONIC = 3, ORC_PAIR_GAUSS = 4, ORC_PAIR_TABLE = 5 };
 enum { ORC_BOND_NONE = 0, ORC_BOND_FENE = 1, ORC_BOND_HARMONIC = 2 };
-enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2, ORC_NOSE_HOOVER = 3, ORC_ANDERSEN = 4, ORC_BERENDSEN = 5 };
+enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2, ORC_NOSE_HOOVER = 3, ORC_ANDERSEN = 4, ORC_BERENDSEN = 5,
+       ORC_NPH = 6, ORC_NPT = 7 };
 enum { ORC_OK = 0, ORC_ERR_BOND_OVERSTRETCH = -7, ORC_ERR_ARG = -1 };
 
 typedef struct {
@@ -91,6 +95,10 @@ typedef struct {
        coupling rate: Nose-Hoover 1/tau, Berendsen 1/tau_T, Andersen collision frequency nu.  thermo[0] = 1 once a
        half-step velocity exists, thermo[1] = its kinetic energy sum 1/2 m u^2, thermo[2] = Nose-Hoover xi.           */
     double *thermo;
+    /* Andersen barostat (reading c-31): baro[0] = P_ext, baro[1] = piston mass M, baro[2] = piston
+       momentum Pi = M dV/dt, baro[3] = virial W = sum over pairs and bonds of r_ij . F_ij at the current positions,
+       baro[4] = 1 once baro[3] is valid.  The volume is box[0] box[1] box[2]: orc_run rescales box[] in place.       */
+    double *baro;
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -526,6 +534,48 @@ int orc_pair_bond_forces(const orc_params *p, const double *pos, const double *v
     return status;
 }
 
+/* The virial W = sum over interacting pairs and bonds of r_ij . F_ij (F_ij: force on i from j, r_ij the minimum-image
+ * displacement; each pair once), written out as that definition: all pairs, O(N^2).  Angle and dihedral energies do not
+ * change under a uniform scaling of the coordinates, so they add nothing.  With it the instantaneous pressure is
+ * P = (2 K + W) / (3 V)  (Andersen 1980, Eq. 3.4c; PAPER.md:L133 names the barostat only).                       */
+int orc_virial(const orc_params *p, const double *pos, double *w_out)
+{
+    const int64_t n = p->n;
+    double w = 0.0;
+    int status = ORC_OK;
+    if (p->pair_style != ORC_PAIR_NONE) {
+#pragma omp parallel for schedule(static) reduction(+ : w)
+        for (int64_t i = 0; i < n; ++i)
+            for (int64_t j = i + 1; j < n; ++j) {
+                double f[3] = { 0, 0, 0 }, u = 0.0;
+                if (!pair_term(p, pos, pos, 0, i, j, f, &u)) continue;
+                for (int d = 0; d < 3; ++d)
+                    w += f[d] * orc_min_image(pos[3 * i + d] - pos[3 * j + d], p->box[d]);
+            }
+    }
+    if (p->bond_style != ORC_BOND_NONE) {
+        for (int64_t b = 0; b < p->n_bonds; ++b) {
+            int64_t i = p->bond_i[b], j = p->bond_j[b];
+            double k = p->bond_k[p->bond_type[b]], r0 = p->bond_r0[p->bond_type[b]];
+            double r2 = 0.0;
+            for (int d = 0; d < 3; ++d) {
+                double x = orc_min_image(pos[3 * i + d] - pos[3 * j + d], p->box[d]);
+                r2 += x * x;
+            }
+            if (p->bond_style == ORC_BOND_FENE) {
+                double q = 1.0 - r2 / (r0 * r0);                     /* F_ij = -k r_ij / q */
+                if (!(q > 0.0)) { status = ORC_ERR_BOND_OVERSTRETCH; continue; }
+                w += -k / q * r2;
+            } else {
+                double r = sqrt(r2);                                 /* F_ij = -2 k (r - r0) r_ij / r */
+                w += -2.0 * k * (r - r0) * r;
+            }
+        }
+    }
+    *w_out = w;
+    return status;
+}
+
 /* The force the integrator uses at time level `step` (O7):
  *   NVE, GW-VV : F(pos [, vel])
  *   Langevin   : F_c(pos) - gamma m v + sqrt(6 gamma m kT / dt) xi(tag, step)   (reading c-7)
@@ -548,7 +598,7 @@ int orc_compute_forces(const orc_params *p, const double *pos, const double *vel
 
 /* O7. n_steps of the integrator, starting at time level step0 with frc = orc_compute_forces(step0). */
 /* scratch: 6n doubles (GW-VV: v-tilde and the old acceleration).                                  */
-int orc_run(const orc_params *p, double *pos, double *vel, double *frc, uint64_t step0, int64_t n_steps,
+int orc_run(orc_params *p, double *pos, double *vel, double *frc, uint64_t step0, int64_t n_steps,
             double *scratch)
 {
     const int64_t n = p->n;
@@ -556,7 +606,7 @@ int orc_run(const orc_params *p, double *pos, double *vel, double *frc, uint64_t
     int status = ORC_OK;
     for (int64_t s = 0; s < n_steps; ++s) {
         uint64_t step = step0 + (uint64_t)s + 1;    /* time level of the new force */
-        if (p->integrator >= ORC_NOSE_HOOVER) {
+        if (p->integrator >= ORC_NOSE_HOOVER && p->integrator <= ORC_BERENDSEN) {
             /* Leapfrog with a thermostat on the half-step velocity u (vel holds the full-step v^m = u^{m-1/2} + dt/2 a^m
                between steps; a = frc / m is a^m).  First step after a (re)start: u^{1/2} = v^0 + dt/2 a^0, thermostat off.
                  Berendsen (c-30):   lambda = sqrt(1 + dt gamma (kT / T_half - 1));  u' = lambda (u + dt a)
@@ -599,6 +649,59 @@ int orc_run(const orc_params *p, double *pos, double *vel, double *frc, uint64_t
             p->thermo[0] = 1.0; p->thermo[1] = k_half;
             int st = orc_compute_forces(p, pos, vel, step, frc, NULL);
             if (st != ORC_OK) status = st;
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d)
+                    vel[3 * i + d] += 0.5 * dt * frc[3 * i + d] / p->mass[i];
+        } else if (p->integrator == ORC_NPH || p->integrator == ORC_NPT) {
+            /* Andersen barostat (PAPER.md:L133 names it; reading c-31).  Andersen 1980, Eq. 3.2: scaled coordinates
+               rho_i = r_i / V^(1/3) with momenta pi_i, the volume V with momentum Pi, and
+                   H = sum pi_i^2 / (2 m_i V^(2/3)) + U(V^(1/3) rho) + Pi^2 / (2 M) + P_ext V.
+               The physical velocity is v_i = pi_i / (m_i V^(1/3)).  H = H_kin(pi, V) + H_pot(rho, V) + H_pis(Pi), and each
+               part alone is solved exactly:
+                 H_pot for t:  pi_i += t V^(1/3) F_i  (v_i += t F_i / m_i),   Pi += t (W / (3 V) - P_ext)
+                 H_kin for t:  rho_i += t pi_i / (m_i V^(2/3))  (r_i += t v_i),   Pi += t 2 K / (3 V),  K = sum m v^2 / 2
+                 H_pis for t:  V += t Pi / M  at fixed rho, pi:  r_i *= mu, v_i /= mu, box *= mu, mu = (V'/V)^(1/3)
+               One step is the symmetric product  pot(dt/2) kin(dt/2) pis(dt) kin(dt/2) pot(dt/2): time-reversible and
+               second order, velocity-Verlet when M is infinite.  NPT (Andersen's own constant-T proposal, his section
+               IV): after the second kin part every bead is hit by the bath with probability nu dt and then draws
+               v = sqrt(kT/m) g, with the draws of the NVT Andersen thermostat (c-29).                                  */
+            double *b = p->baro;
+            if (b[4] == 0.0) { orc_virial(p, pos, &b[3]); b[4] = 1.0; }
+            double V = p->box[0] * p->box[1] * p->box[2];
+            double K = 0.0;
+            b[2] += 0.5 * dt * (b[3] / (3.0 * V) - b[0]);
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d) {
+                    vel[3 * i + d] += 0.5 * dt * frc[3 * i + d] / p->mass[i];
+                    pos[3 * i + d] += 0.5 * dt * vel[3 * i + d];
+                    K += 0.5 * p->mass[i] * vel[3 * i + d] * vel[3 * i + d];
+                }
+            b[2] += 0.5 * dt * 2.0 * K / (3.0 * V);
+            double Vn = V + dt * b[2] / b[1];
+            if (!(Vn > 0.0)) return ORC_ERR_ARG;
+            double mu = cbrt(Vn / V);
+            for (int d = 0; d < 3; ++d) p->box[d] *= mu;
+            K = 0.0;
+            for (int64_t i = 0; i < n; ++i)
+                for (int d = 0; d < 3; ++d) {
+                    vel[3 * i + d] /= mu;
+                    pos[3 * i + d] = pos[3 * i + d] * mu + 0.5 * dt * vel[3 * i + d];
+                    K += 0.5 * p->mass[i] * vel[3 * i + d] * vel[3 * i + d];
+                }
+            b[2] += 0.5 * dt * 2.0 * K / (3.0 * Vn);
+            for (int64_t i = 0; i < n; ++i) {
+                for (int d = 0; d < 3; ++d) pos[3 * i + d] = wrap1(pos[3 * i + d], p->box[d]);
+                if (p->integrator == ORC_NPT && orc_andersen_hit(p->seed, step - 1, i, p->gamma * dt)) {
+                    double g[3];
+                    orc_andersen_normals(p->seed, step - 1, i, g);
+                    for (int d = 0; d < 3; ++d) vel[3 * i + d] = sqrt(p->kT / p->mass[i]) * g[d];
+                }
+            }
+            int st = orc_compute_forces(p, pos, vel, step, frc, NULL);
+            if (st != ORC_OK) status = st;
+            st = orc_virial(p, pos, &b[3]);
+            if (st != ORC_OK) status = st;
+            b[2] += 0.5 * dt * (b[3] / (3.0 * Vn) - b[0]);
             for (int64_t i = 0; i < n; ++i)
                 for (int d = 0; d < 3; ++d)
                     vel[3 * i + d] += 0.5 * dt * frc[3 * i + d] / p->mass[i];

@@ -19,7 +19,7 @@ _LIB = os.path.join(_HERE, "libgm_oracle.so")
 
 PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 BOND = {"none": 0, "fene": 1, "harmonic": 2}
-INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5}
+INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5, "nph": 6, "npt": 7}
 ORC_ERR_BOND_OVERSTRETCH = -7
 
 
@@ -51,7 +51,7 @@ class _Params(C.Structure):
         ("n_dihedrals", C.c_int64),
         ("dih_i", C.c_void_p), ("dih_j", C.c_void_p), ("dih_k", C.c_void_p), ("dih_l", C.c_void_p), ("dih_type", C.c_void_p),
         ("dih_kk", C.c_void_p), ("dih_delta", C.c_void_p), ("dih_n", C.c_void_p),
-        ("thermo", C.c_void_p),
+        ("thermo", C.c_void_p), ("baro", C.c_void_p),
     ]
 
 
@@ -87,6 +87,8 @@ def lib():
                               C.c_int64, C.c_void_p]
         L.orc_run.restype = C.c_int
         L.orc_num_threads.restype = C.c_int
+        L.orc_virial.argtypes = [C.POINTER(_Params), C.c_void_p, C.c_void_p]
+        L.orc_virial.restype = C.c_int
         _lib = L
     return _lib
 
@@ -272,6 +274,11 @@ class Oracle:
         P.dih_kk = _p(self._dih_k).value; P.dih_delta = _p(self._dih_delta).value; P.dih_n = _p(self._dih_n).value
         self.thermo = np.zeros(4)       # [have half-step velocity, its kinetic energy, Nose-Hoover xi, -]
         P.thermo = _p(self.thermo).value
+        # Andersen barostat (integrators "nph", "npt"): [P_ext, piston mass, piston momentum Pi, virial, virial valid]
+        self.baro = np.zeros(5)
+        self.baro[0] = float(np.float32(getattr(w, "p_ext", 0.0)))
+        self.baro[1] = float(np.float32(getattr(w, "piston_mass", 1.0)))
+        P.baro = _p(self.baro).value
         if w.pair_style == "table":
             P.table = _p(self.table).value
             P.table_points = int(self.table.shape[2])
@@ -302,7 +309,34 @@ class Oracle:
                            int(n_steps), _p(scratch))
         self.step += int(n_steps)
         self.status = st
+        for d in range(3):              # the barostat rescales the box
+            self.box[d] = self.P.box[d]
         return st
+
+    def set_box(self, box):
+        """Change the box (the caller rescales positions); invalidates the stored virial."""
+        for d in range(3):
+            self.P.box[d] = float(box[d]); self.box[d] = float(box[d])
+        self.baro[4] = 0.0
+
+    def virial(self, pos=None) -> float:
+        """W = sum of r_ij . F_ij over pairs and bonds at the given positions (orc_virial: the definition, O(N^2))."""
+        pos = self.pos if pos is None else np.ascontiguousarray(pos, np.float64)
+        out = np.zeros(1)
+        self.status = lib().orc_virial(C.byref(self.P), _p(pos), _p(out))
+        return float(out[0])
+
+    def volume(self) -> float:
+        return float(self.box[0] * self.box[1] * self.box[2])
+
+    def pressure(self) -> float:
+        """Instantaneous pressure (2 K + W) / (3 V) of the current state."""
+        return (2.0 * self.kinetic() + self.virial()) / (3.0 * self.volume())
+
+    def enthalpy_like(self) -> float:
+        """Andersen's conserved H = K + U + P_ext V + Pi^2 / (2 M)."""
+        a, b, _ = self.potential()
+        return self.kinetic() + a + b + self.baro[0] * self.volume() + self.baro[2] ** 2 / (2.0 * self.baro[1])
 
     # -- observables (O8), plain numpy fp64 -------------------------------------------------------
     def kinetic(self) -> float:
