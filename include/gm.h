@@ -66,7 +66,8 @@ enum {
 enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2, GM_PAIR_HARMONIC = 3, GM_PAIR_GAUSS = 4, GM_PAIR_TABLE = 5 };
 enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2 };
 enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2,
-       GM_NVT_NOSE_HOOVER = 3, GM_NVT_ANDERSEN = 4, GM_NVT_BERENDSEN = 5 };   /* PAPER.md:L133, L137; DESIGN.md c-28..c-30 */
+       GM_NVT_NOSE_HOOVER = 3, GM_NVT_ANDERSEN = 4, GM_NVT_BERENDSEN = 5,     /* PAPER.md:L133, L137; DESIGN.md c-28..c-30 */
+       GM_NPH_ANDERSEN = 6, GM_NPT_ANDERSEN = 7 };                            /* Andersen barostat; DESIGN.md c-31 */
 enum { GM_ANGLE_NONE = 0, GM_ANGLE_HARMONIC = 1 /* Eq. (8): k (theta - theta0)^2 */, GM_ANGLE_COSINE = 2 /* Eq. (9): k (cos theta - cos theta0)^2 */ };
 
 #define GM_MAX_TYPES 8       /* particle types; pair tables are n_types x n_types */
@@ -87,7 +88,7 @@ typedef struct {
     uint64_t seed;                   /* key of the counter-based Philox4x32-10 noise               */
     int32_t pair_style;              /* GM_PAIR_*                                                  */
     int32_t bond_style;              /* GM_BOND_*                                                  */
-    int32_t integrator;              /* GM_NVE | GM_LANGEVIN | GM_DPD_GWVV | GM_NVT_*              */
+    int32_t integrator;              /* GM_NVE | GM_LANGEVIN | GM_DPD_GWVV | GM_NVT_* | GM_NP*_ANDERSEN */
     float kT, gamma, lambda;         /* thermostat temperature; friction (Langevin, DPD) or coupling rate of the NVT
                                         thermostats (Nose-Hoover 1/tau, Berendsen 1/tau_T, Andersen collision frequency);
                                         GW-VV lambda */
@@ -206,11 +207,34 @@ gm_status gm_compute_forces(gm_system *s);
 gm_status gm_step(gm_system *s, int64_t n_steps);
 
 /* Switch the integrator of an existing system (e.g. Langevin equilibration, then NVE: BASELINE.json
- * config 3).  integrator: GM_NVE | GM_LANGEVIN | GM_NVT_* (GM_DPD_GWVV only on a GM_PAIR_DPD system and vice
+ * config 3).  integrator: GM_NVE | GM_LANGEVIN | GM_NVT_* | GM_NP*_ANDERSEN (GM_DPD_GWVV only on a GM_PAIR_DPD system and vice
  * versa); kT, gamma as in gm_config.  The first step after a switch to an NVT thermostat runs without it (the
  * temperature of the half-step velocities it acts on is measured in that step).  The state (positions, half-step velocities, step counter,
  * neighbor list) is kept.  Errors: INVALID_ARG. */
 gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma);
+
+/* Andersen barostat ("the constant pressure can be controlled via Andersen barostat"; equations: DESIGN.md
+ * reading c-31).  Integrators GM_NPH_ANDERSEN (barostat alone) and GM_NPT_ANDERSEN (barostat + Andersen's stochastic
+ * collisions at frequency gamma, temperature kT).  The box changes isotropically: the device keeps every position in the
+ * box of gm_create ("scaled" coordinates) and one scale factor lambda = (V / V_create)^(1/3); forces, virial and energies are
+ * evaluated at the real distances lambda * s.  Pair styles GM_PAIR_LJ and GM_PAIR_NONE, bonds of any style; no angles /
+ * dihedrals, no DPD; such a system runs without tile windows and outside CUDA graphs (two kernels per timestep: forces +
+ * virial, then piston + kick + drift).  The neighbor list is built once for the scaled list radius r_cut_max + r_skin of
+ * gm_create; it stays complete while lambda > r_cut_max / (r_cut_max + r_skin) -- a box that shrinks further latches an
+ * error (GM_ERR_BOX_TOO_SMALL from the next synchronising call); build the system anew at the new size then.
+ *
+ * gm_set_barostat: external pressure and piston mass M (Andersen's M: M V'' = P_inst - P_ext; units of mass / length^4);
+ * the piston starts at rest.  Call it before gm_set_integrator(GM_NP*_ANDERSEN) / the first step.
+ * gm_set_box_state: volume and piston momentum Pi = M dV/dt of a restart; call it BEFORE gm_set_particles, whose
+ * positions are then taken in the box of that volume.  Errors: INVALID_ARG (p_ext < 0, mass <= 0, volume <= 0), STATE. */
+gm_status gm_set_barostat(gm_system *s, float p_ext, float piston_mass);
+gm_status gm_set_box_state(gm_system *s, double volume, double piston_momentum);
+
+/* out (HOST, 8 doubles): current box L_x, L_y, L_z, volume, piston momentum Pi (at the current time level), instantaneous
+ * pressure (2 K + W) / (3 V), virial W = sum over pairs and bonds of r_ij . F_ij, and Andersen's conserved
+ * H = K + U + P_ext V + Pi^2 / (2 M).  On a system without barostat: the box of gm_create, Pi = 0, and the same
+ * pressure / virial / H with P_ext = 0 are NOT computed (out[5..7] = 0).  Synchronises. */
+gm_status gm_get_box(gm_system *s, double out[8]);
 
 /* Measurement aid: n_steps timesteps exactly as gm_step would take them, but launched kernel by
  * kernel (no CUDA graph) with CUDA events on the system's stream around the fused force+integrate

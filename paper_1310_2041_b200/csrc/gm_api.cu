@@ -10,6 +10,7 @@
 #include <vector>
 
 #include "gm_internal.cuh"
+#include "gm_npt.cuh"
 
 #define GM_GRAPH_STEPS 16   // steps per big graph launch (even)
 
@@ -23,6 +24,8 @@ struct gm_system {
     uint64_t step;
     bool use_graph, use_cond;
     cudaGraphExec_t exec_big, exec_two;
+    // Andersen barostat (gm_npt.cuh): host copies of what gm_set_barostat / gm_set_box_state last set
+    double npt_vol0, npt_V, npt_Pi, npt_p_ext, npt_mass;
     char err[512];
 };
 
@@ -42,6 +45,8 @@ static gm_status fail(gm_system *s, gm_status code, const char *fmt, const char 
 
 static size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 
+static bool is_npt(const gm_system *s) { return s->P.integrator == GM_NPH_ANDERSEN || s->P.integrator == GM_NPT_ANDERSEN; }
+
 // ---- geometry and constants derived from the configuration ----------------------------------------
 static gm_status derive(const gm_config *c, GmParams *P)
 {
@@ -54,8 +59,12 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (c->table_points < 0 || c->table_points > (1 << 20) || ((c->pair_style == GM_PAIR_TABLE) != (c->table_points > 0)))
         return GM_ERR_INVALID_ARG;
     if (c->bond_style < GM_BOND_NONE || c->bond_style > GM_BOND_HARMONIC) return GM_ERR_INVALID_ARG;
-    if (c->integrator < GM_NVE || c->integrator > GM_NVT_BERENDSEN) return GM_ERR_INVALID_ARG;
+    if (c->integrator < GM_NVE || c->integrator > GM_NPT_ANDERSEN) return GM_ERR_INVALID_ARG;
     if ((c->integrator == GM_DPD_GWVV) != (c->pair_style == GM_PAIR_DPD)) return GM_ERR_INVALID_ARG;
+    const bool npt = c->integrator == GM_NPH_ANDERSEN || c->integrator == GM_NPT_ANDERSEN;
+    if (npt && ((c->pair_style != GM_PAIR_LJ && c->pair_style != GM_PAIR_NONE) || c->max_angles_per_particle > 0 ||
+                c->max_dihedrals_per_particle > 0 || (c->flags & GM_FLAG_STEP_SUBWARP)))
+        return GM_ERR_INVALID_ARG;
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
@@ -152,7 +161,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
         // gains 0.3 us, the rebuild loses 3), so they are chosen by the estimated list length; tile_windows overrides.
         const double nbar_w = (double)P->n / vol * (4.0 / 3.0) * 3.14159265358979323846 * r_list * r_list * r_list;
         const bool can = c->pair_style != GM_PAIR_NONE && c->pair_style != GM_PAIR_DPD && P->step_subw == 1 &&
-                         !(c->flags & GM_FLAG_NO_WINDOWS) && wc <= 8000;
+                         !(c->flags & GM_FLAG_NO_WINDOWS) && wc <= 8000 && !npt;      // the barostat path reads 32-bit rows
         P->use_win = (can && c->tile_windows != 2 && (c->tile_windows == 1 || nbar_w >= 40.0)) ? 1 : 0;
         if (P->n <= 4096 && P->use_win) wc = std::max(wc, (P->n + 7) / 8 * 8);
         P->win_cap = P->use_win ? wc : 0;
@@ -202,7 +211,7 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     d.scan_sums = (int *)take((((size_t)P.n_cells + 1 + per - 1) / per + 1) * 4);
     d.row_rank = (uint32_t *)take((size_t)P.nc[1] * P.nc[2] * 4);
     d.stage = (float *)take(n * 4 * 11);
-    d.esum = (double *)take(((size_t)GM_ESUM_BLOCKS + 1) * 8 * sizeof(double));
+    d.esum = (double *)take((((size_t)GM_ESUM_BLOCKS + 1) * 8 + GM_NPT_DOUBLES) * sizeof(double));     // + GmNpt (gm_npt.cuh)
     if (D) *D = d;
     return off;
 }
@@ -327,6 +336,9 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     if (e == cudaSuccess) {
         gm_launch_init_pad(P, s->D, s->st);
         gm_launch_set_ctl(s->D, 0, 1, 0, s->st);
+        s->npt_vol0 = (double)cfg->box[0] * (double)cfg->box[1] * (double)cfg->box[2];
+        s->npt_V = s->npt_vol0; s->npt_Pi = 0.0; s->npt_p_ext = 0.0; s->npt_mass = 1.0;
+        gm_launch_npt_init(s->D, 0, s->npt_vol0, s->npt_V, s->npt_Pi, s->npt_p_ext, s->npt_mass, s->st);
         e = cudaGetLastError();
     }
     if (e != cudaSuccess) {
@@ -566,7 +578,20 @@ extern "C" gm_status gm_set_particles(gm_system *s, const float *pos3, const flo
         dp = st; dv = st + 3 * n; dt = (const int *)(st + 9 * n); dm = mass ? st + 10 * n : nullptr;
         CU(cudaStreamSynchronize(s->st));      // "copies inputs in": the caller may reuse (pinned) buffers at once
     }
+    // Andersen barostat (gm_npt.cuh): the arrays hold s = r / lambda and c = lambda v; the box of gm_set_box_state applies
+    const double lam = std::cbrt(s->npt_V / s->npt_vol0);
+    if (lam != 1.0) {
+        float *st = s->D.stage;
+        if (on_device) {
+            CU(cudaMemcpyAsync(st, pos3, n * 12, cudaMemcpyDeviceToDevice, s->st));
+            CU(cudaMemcpyAsync(st + 3 * n, vel3, n * 12, cudaMemcpyDeviceToDevice, s->st));
+            dp = st; dv = st + 3 * n;
+        }
+        gm_launch_scale3(st, 3 * n, (float)(1.0 / lam), s->st);
+        gm_launch_scale3(st + 3 * n, 3 * n, (float)lam, s->st);
+    }
     s->cur = 0;
+    gm_launch_npt_init(s->D, 0, s->npt_vol0, s->npt_V, s->npt_Pi, s->npt_p_ext, s->npt_mass, s->st);
     gm_launch_set_ctl(s->D, 0, 1, 0, s->st);             // clears the latched device errors: before the pack
     gm_launch_pack(s->P, s->D, 0, dp, dv, dt, dm, s->st);
     CU(cudaGetLastError());
@@ -666,7 +691,11 @@ static void enqueue_step_kernel(gm_system *s, bool lagged, cudaStream_t st)
     float kick, kick_vt;
     kicks(s, &kick, &kick_vt);
     s->lagged = keep;
-    gm_launch_force(s->P, s->D, GM_MODE_STEP, s->cur, kick, kick_vt, 0, st);
+    if (is_npt(s)) {         // Andersen barostat: forces + virial, then piston + kick + drift (gm_npt.cu)
+        gm_launch_npt_force(s->P, s->D, s->cur, 0, st);
+        gm_launch_npt_update(s->P, s->D, s->cur, kick, st);
+    } else
+        gm_launch_force(s->P, s->D, GM_MODE_STEP, s->cur, kick, kick_vt, 0, st);
     s->cur ^= 1;
 }
 
@@ -771,7 +800,8 @@ extern "C" gm_status gm_compute_forces(gm_system *s)
     CU(cudaSetDevice(s->cfg.device));
     gm_status r = ensure_list(s);
     if (r != GM_OK) return r;
-    gm_launch_force(s->P, s->D, GM_MODE_FORCES, s->cur, 0.f, 0.f, 0, s->st);
+    if (is_npt(s)) gm_launch_npt_force(s->P, s->D, s->cur, 1, s->st);
+    else gm_launch_force(s->P, s->D, GM_MODE_FORCES, s->cur, 0.f, 0.f, 0, s->st);
     CU(cudaGetLastError());
     s->force_current = true;
     return GM_OK;
@@ -790,7 +820,7 @@ static gm_status step_impl(gm_system *s, int64_t n_steps, StepTiming *tm)
     int64_t done = 0;
     while (done < n_steps) {
         const int64_t rem = n_steps - done;
-        if (!tm && s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
+        if (!tm && s->use_graph && !is_npt(s) && s->lagged && s->cur == 0 && rem >= 2) {
             const bool big = rem >= GM_GRAPH_STEPS;
             cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
             const int ns = big ? GM_GRAPH_STEPS : 2;
@@ -858,8 +888,15 @@ extern "C" gm_status gm_step_timed(gm_system *s, int64_t n_steps, double out[4])
 extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma)
 {
     if (!s) return GM_ERR_INVALID_ARG;
-    if (integrator < GM_NVE || integrator > GM_NVT_BERENDSEN)
+    if (integrator < GM_NVE || integrator > GM_NPT_ANDERSEN)
         return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: unknown integrator%s");
+    const bool to_npt = integrator == GM_NPH_ANDERSEN || integrator == GM_NPT_ANDERSEN;
+    if (to_npt && (s->P.use_win || s->P.step_subw != 1 || s->P.max_angles + s->P.max_dihedrals > 0 ||
+                   (s->P.pair_style != GM_PAIR_LJ && s->P.pair_style != GM_PAIR_NONE)))
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: the barostat needs GM_PAIR_LJ or GM_PAIR_NONE, no angles / dihedrals, "
+                                           "and a system without tile windows (GM_FLAG_NO_WINDOWS, or created with an NP* integrator)%s");
+    if (!to_npt && is_npt(s))
+        return fail(s, GM_ERR_STATE, "gm_set_integrator: a system under the barostat stays under it (its box has changed)%s");
     if (integrator >= GM_NVT_NOSE_HOOVER && s->P.step_subw != 1)
         return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: the NVT thermostats do not run on the sub-warp step kernel%s");
     if ((integrator == GM_DPD_GWVV) != (s->P.pair_style == GM_PAIR_DPD))
@@ -881,6 +918,7 @@ extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, f
 static gm_status dev_error(gm_system *s, const GmCtl &c)
 {
     if (c.err & GM_DEV_ERR_BAD_INPUT) return fail(s, GM_ERR_INVALID_ARG, "gm_set_particles: a type outside [0, n_types) or a mass <= 0%s");
+    if (c.err & GM_DEV_ERR_BOX) return fail(s, GM_ERR_BOX_TOO_SMALL, "the barostat shrank the box below what the neighbor list of gm_create covers%s");
     if (c.err & GM_DEV_ERR_WINDOW) return fail(s, GM_ERR_CUDA, "a tile window copy did not complete (internal error)%s");
     if (c.err & GM_DEV_ERR_NONFINITE) return fail(s, GM_ERR_NONFINITE, "a coordinate became non-finite%s");
     if (c.err & GM_DEV_ERR_OVERSTRETCH) return fail(s, GM_ERR_BOND_OVERSTRETCH, "a FENE bond reached r >= R0%s");
@@ -897,12 +935,90 @@ static gm_status sync_and_check(gm_system *s, GmCtl *out = nullptr)
     return dev_error(s, c);
 }
 
+// Andersen barostat: one force evaluation at the current time level outside the time stepping, and what follows from its
+// sums -- the kinetic energy of the full-step velocities v = (c + h lambda F / m) / lambda, h = dt/2 once a half-step
+// velocity is stored, and the piston momentum completed by the same half kick
+struct NptProbe { double K, pe_pair, pe_bond, W, V, Pi, lam, P_inst, H; };
+
+static gm_status npt_probe(gm_system *s, NptProbe *o)
+{
+    gm_status r = ensure_list(s);
+    if (r != GM_OK) return r;
+    gm_launch_npt_force(s->P, s->D, s->cur, 1, s->st);
+    CU(cudaGetLastError());
+    s->force_current = true;
+    GmNpt h;
+    CU(cudaMemcpyAsync(&h, gm_npt_state(s->D), sizeof(h), cudaMemcpyDeviceToHost, s->st));
+    r = sync_and_check(s);
+    const double *sm = h.sum[2];
+    const double lam = h.lam[s->cur], V = h.V[s->cur], hk = s->lagged ? 0.5 * (double)s->P.dt : 0.0;
+    const double S = sm[1] + 2.0 * hk * lam * sm[2] + hk * hk * lam * lam * sm[3];
+    o->K = S / (2.0 * lam * lam);
+    o->pe_pair = sm[4]; o->pe_bond = sm[5]; o->W = sm[0]; o->V = V; o->lam = lam;
+    o->Pi = h.Pi[s->cur] + hk * (sm[0] / (3.0 * V) - h.p_ext);
+    o->P_inst = (2.0 * o->K + o->W) / (3.0 * V);
+    o->H = o->K + o->pe_pair + o->pe_bond + h.p_ext * V + o->Pi * o->Pi / (2.0 * h.mass);
+    return r;
+}
+
+extern "C" gm_status gm_set_barostat(gm_system *s, float p_ext, float piston_mass)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!(p_ext >= 0.f) || !(piston_mass > 0.f)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_barostat: p_ext >= 0 and piston_mass > 0%s");
+    if (s->have_particles && s->step > 0 && is_npt(s))
+        return fail(s, GM_ERR_STATE, "gm_set_barostat: call it before the first step under the barostat%s");
+    CU(cudaSetDevice(s->cfg.device));
+    s->npt_p_ext = (double)p_ext; s->npt_mass = (double)piston_mass;
+    gm_launch_npt_init(s->D, s->cur, s->npt_vol0, s->npt_V, s->npt_Pi, s->npt_p_ext, s->npt_mass, s->st);
+    CU(cudaGetLastError());
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_box_state(gm_system *s, double volume, double piston_momentum)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!(volume > 0.0) || !std::isfinite(piston_momentum)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_box_state: volume > 0%s");
+    if (s->have_particles) return fail(s, GM_ERR_STATE, "gm_set_box_state: call it before gm_set_particles%s");
+    CU(cudaSetDevice(s->cfg.device));
+    s->npt_V = volume; s->npt_Pi = piston_momentum;
+    gm_launch_npt_init(s->D, s->cur, s->npt_vol0, s->npt_V, s->npt_Pi, s->npt_p_ext, s->npt_mass, s->st);
+    CU(cudaGetLastError());
+    return GM_OK;
+}
+
+extern "C" gm_status gm_get_box(gm_system *s, double out[8])
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (!out) return fail(s, GM_ERR_INVALID_ARG, "gm_get_box: NULL out%s");
+    CU(cudaSetDevice(s->cfg.device));
+    for (int q = 0; q < 8; ++q) out[q] = 0.0;
+    if (!is_npt(s) || !s->have_particles) {
+        const double lam = std::cbrt(s->npt_V / s->npt_vol0);
+        for (int d = 0; d < 3; ++d) out[d] = lam * (double)s->cfg.box[d];
+        out[3] = s->npt_V; out[4] = s->npt_Pi;
+        return GM_OK;
+    }
+    NptProbe q;
+    gm_status r = npt_probe(s, &q);
+    for (int d = 0; d < 3; ++d) out[d] = q.lam * (double)s->cfg.box[d];
+    out[3] = q.V; out[4] = q.Pi; out[5] = q.P_inst; out[6] = q.W; out[7] = q.H;
+    return r;
+}
+
 extern "C" gm_status gm_energies(gm_system *s, double out[8])
 {
     if (!s) return GM_ERR_INVALID_ARG;
     if (!out) return fail(s, GM_ERR_INVALID_ARG, "gm_energies: NULL out%s");
     if (!s->have_particles) return fail(s, GM_ERR_STATE, "gm_energies: no particles set%s");
     CU(cudaSetDevice(s->cfg.device));
+    if (is_npt(s)) {
+        NptProbe q;
+        gm_status rq = npt_probe(s, &q);
+        const double dofq = s->P.n > 1 ? 3.0 * s->P.n - 3.0 : 3.0;
+        out[0] = q.K; out[1] = q.pe_pair; out[2] = q.pe_bond; out[3] = 2.0 * q.K / dofq;
+        out[4] = out[5] = out[6] = out[7] = 0.0;
+        return rq;
+    }
     gm_status r = ensure_list(s);
     if (r != GM_OK) return r;
     gm_launch_force(s->P, s->D, GM_MODE_ENERGY, s->cur, 0.f, 0.f, s->lagged ? 1 : 0, s->st);
@@ -932,7 +1048,14 @@ extern "C" gm_status gm_get_particles(gm_system *s, float *pos3, float *vel3, fl
     if (!on_device) {
         dp = pos3 ? st : nullptr; dv = vel3 ? st + 3 * n : nullptr; df = force3 ? st + 6 * n : nullptr;
     }
-    gm_launch_unpack(s->P, s->D, s->cur, dp, dv, df, s->lagged ? 1 : 0, s->st);
+    if (is_npt(s)) {
+        if (!s->force_current) {           // the real-unit output needs the forces of this time level in any case
+            gm_status r = gm_compute_forces(s);
+            if (r != GM_OK) return r;
+        }
+        gm_launch_npt_unpack(s->P, s->D, s->cur, dp, dv, df, s->lagged ? 1 : 0, s->st);
+    } else
+        gm_launch_unpack(s->P, s->D, s->cur, dp, dv, df, s->lagged ? 1 : 0, s->st);
     CU(cudaGetLastError());
     if (!on_device) {
         if (pos3) CU(cudaMemcpyAsync(pos3, dp, n * 12, cudaMemcpyDeviceToHost, s->st));

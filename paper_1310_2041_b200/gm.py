@@ -21,7 +21,7 @@ GM_ERR_INVALID_ARG, GM_ERR_STATE, GM_ERR_CUDA, GM_ERR_WORKSPACE_TOO_SMALL = -1, 
 GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_NONFINITE = -5, -6, -7, -8
 GM_PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
-GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5}
+GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5, "nph": 6, "npt": 7}
 GM_ANGLE = {"none": 0, "harmonic": 1, "cosine": 2}
 GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP, GM_FLAG_NO_WINDOWS = 1, 2, 4, 8
 
@@ -29,7 +29,7 @@ SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params"
            "gm_set_bond_params", "gm_set_angle_params", "gm_set_dihedral_params", "gm_set_angles", "gm_set_dihedrals",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
-           "gm_get_tuning",
+           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box",
            "gm_sfc_cell_order", "gm_last_error"]
 
 
@@ -86,6 +86,9 @@ def lib():
         L.gm_step_timed.argtypes = [vp, i64, vp]
         L.gm_set_integrator.argtypes = [vp, i32, C.c_float, C.c_float]
         L.gm_energies.argtypes = [vp, vp]
+        L.gm_set_barostat.argtypes = [vp, C.c_float, C.c_float]
+        L.gm_set_box_state.argtypes = [vp, C.c_double, C.c_double]
+        L.gm_get_box.argtypes = [vp, vp]
         L.gm_get_particles.argtypes = [vp, vp, vp, vp, i32]
         L.gm_get_neighbors.argtypes = [vp, vp, vp, i64, i32]
         L.gm_get_stats.argtypes = [vp, vp]
@@ -219,6 +222,20 @@ def gm_set_integrator(h, integrator: int, kT: float, gamma: float):
     _check(lib().gm_set_integrator(h, integrator, kT, gamma), h)
 
 
+def gm_set_barostat(h, p_ext: float, piston_mass: float):
+    _check(lib().gm_set_barostat(h, p_ext, piston_mass), h)
+
+
+def gm_set_box_state(h, volume: float, piston_momentum: float):
+    _check(lib().gm_set_box_state(h, volume, piston_momentum), h)
+
+
+def gm_get_box(h) -> np.ndarray:
+    out = np.zeros(8, dtype=np.float64)
+    _check(lib().gm_get_box(h, out.ctypes.data), h)
+    return out
+
+
 def gm_energies(h) -> np.ndarray:
     out = np.zeros(8, dtype=np.float64)
     _check(lib().gm_energies(h, out.ctypes.data), h)
@@ -346,6 +363,8 @@ class System:
             for dt_, (k, nn, dl) in enumerate(zip(topo["dihedral_k"], topo["dihedral_n"], topo["dihedral_delta"])):
                 gm_set_dihedral_params(self.h, dt_, float(np.float32(k)), int(nn), float(np.float32(dl)))
             gm_set_dihedrals(self.h, dih, topo.get("dihedral_type"))
+        if w.integrator in ("nph", "npt"):
+            gm_set_barostat(self.h, float(np.float32(getattr(w, "p_ext", 0.0))), float(np.float32(getattr(w, "piston_mass", 1.0))))
         if load:
             self.set_particles(w.pos, w.vel, w.type, w.mass)
             if cfg.max_bonds_per_particle:
@@ -383,6 +402,16 @@ class System:
 
     def set_integrator(self, name: str, kT: float = 1.0, gamma: float = 0.0):
         gm_set_integrator(self.h, GM_INTEG[name], kT, gamma)
+
+    def set_barostat(self, p_ext: float, piston_mass: float):
+        gm_set_barostat(self.h, p_ext, piston_mass)
+
+    def set_box_state(self, volume: float, piston_momentum: float = 0.0):
+        gm_set_box_state(self.h, volume, piston_momentum)
+
+    def box_state(self) -> dict:
+        b = gm_get_box(self.h)
+        return dict(box=b[0:3].copy(), volume=b[3], piston_momentum=b[4], pressure=b[5], virial=b[6], H=b[7])
 
     def energies(self) -> dict:
         e = gm_energies(self.h)
