@@ -62,8 +62,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (c->integrator < GM_NVE || c->integrator > GM_NPT_ANDERSEN) return GM_ERR_INVALID_ARG;
     if ((c->integrator == GM_DPD_GWVV) != (c->pair_style == GM_PAIR_DPD)) return GM_ERR_INVALID_ARG;
     const bool npt = c->integrator == GM_NPH_ANDERSEN || c->integrator == GM_NPT_ANDERSEN;
-    if (npt && ((c->pair_style != GM_PAIR_LJ && c->pair_style != GM_PAIR_NONE) || c->max_angles_per_particle > 0 ||
-                c->max_dihedrals_per_particle > 0 || (c->flags & GM_FLAG_STEP_SUBWARP)))
+    if (npt && ((c->pair_style != GM_PAIR_LJ && c->pair_style != GM_PAIR_NONE) || (c->flags & GM_FLAG_STEP_SUBWARP)))
         return GM_ERR_INVALID_ARG;
     if (!(c->r_cut_max > 0.f) || !(c->r_skin >= 0.f) || !(c->dt > 0.f)) return GM_ERR_INVALID_ARG;
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
@@ -891,9 +890,8 @@ extern "C" gm_status gm_set_integrator(gm_system *s, int integrator, float kT, f
     if (integrator < GM_NVE || integrator > GM_NPT_ANDERSEN)
         return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: unknown integrator%s");
     const bool to_npt = integrator == GM_NPH_ANDERSEN || integrator == GM_NPT_ANDERSEN;
-    if (to_npt && (s->P.use_win || s->P.step_subw != 1 || s->P.max_angles + s->P.max_dihedrals > 0 ||
-                   (s->P.pair_style != GM_PAIR_LJ && s->P.pair_style != GM_PAIR_NONE)))
-        return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: the barostat needs GM_PAIR_LJ or GM_PAIR_NONE, no angles / dihedrals, "
+    if (to_npt && (s->P.use_win || s->P.step_subw != 1 || (s->P.pair_style != GM_PAIR_LJ && s->P.pair_style != GM_PAIR_NONE)))
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_integrator: the barostat needs GM_PAIR_LJ or GM_PAIR_NONE "
                                            "and a system without tile windows (GM_FLAG_NO_WINDOWS, or created with an NP* integrator)%s");
     if (!to_npt && is_npt(s))
         return fail(s, GM_ERR_STATE, "gm_set_integrator: a system under the barostat stays under it (its box has changed)%s");

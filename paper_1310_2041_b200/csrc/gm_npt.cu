@@ -101,6 +101,14 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
                 w += fs * r2;
             }
         }
+        // a7: angle and dihedral forces were evaluated on the scaled coordinates (gm_topo.cu); an angle does not change
+        // under a uniform scaling, so U is the same, F = -dU/dr = (1 / lambda) (-dU/ds), and the virial gets nothing
+        if (P.max_angles + P.max_dihedrals > 0) {
+            const float4 ft = D.ftopo[i];
+            const float il = 1.0f / lam;
+            fx += il * ft.x; fy += il * ft.y; fz += il * ft.z;
+            pe_bond += 2.0f * ft.w;
+        }
         D.frc[i] = make_float4(fx, fy, fz, 0.5f * (pe_pair + pe_bond));
         const float im = 1.0f / c.w;
         acc[0] = 0.5 * (double)w;
@@ -238,6 +246,7 @@ static void npt_force_b(const GmParams &P, const GmDev &D, int parity, int probe
 void gm_launch_npt_force(const GmParams &P, const GmDev &D, int parity, int probe, cudaStream_t st)
 {
     if (probe) cudaMemsetAsync(gm_npt_state(D)->sum[2], 0, 8 * sizeof(double), st);
+    gm_launch_topo(P, D, parity, st);        // angle + dihedral forces of this time level -> D.ftopo (no-op without them)
     if (P.n_types == 1) npt_force_b<true>(P, D, parity, probe, st);
     else npt_force_b<false>(P, D, parity, probe, st);
 }

@@ -45,7 +45,7 @@ def lj(n, **kw):
     return with_barostat(make_config("F4LJ", n=n), **kw)
 
 
-def compare_state(s, o, tol_pos=1e-4):
+def compare_state(s, o, tol_pos=1e-4, positions_only=False):
     pos, vel, frc = s.get_particles(True, True, True)
     b = s.box_state()
     np.testing.assert_allclose(b["box"], o.box, rtol=1e-5)
@@ -53,6 +53,9 @@ def compare_state(s, o, tol_pos=1e-4):
     d -= o.box * np.rint(d / o.box)
     rms = np.sqrt((d * d).sum(axis=1).mean())
     assert rms <= tol_pos, f"RMS position difference {rms:.3e}"
+    assert b["volume"] == pytest.approx(o.volume(), rel=1e-5)
+    if positions_only:
+        return
     assert np.sqrt(((vel - o.vel) ** 2).sum(axis=1).mean()) <= 10 * tol_pos
     frms = np.sqrt((o.frc ** 2).sum(axis=1).mean())
     assert np.abs(frc - o.frc).max() <= 2e-3 * frms            # after chaotic amplification of 1e-4 position differences
@@ -190,4 +193,22 @@ def test_box_that_shrinks_past_the_list_radius_is_reported(gm):
         for _ in range(50):
             s.step(20)
             s.stats()
+    s.close()
+
+
+def test_trajectory_with_angles_and_dihedrals(gm):
+    # angle and dihedral energies are scale-free: forces divide by the scale factor, the virial gets nothing from them
+    from tests.test_gpu_topo import with_topology
+    w = with_topology(kg(1.0, integrator="nph", p_ext=5.0, piston_mass=0.01), "cosine")
+    s = gm.System(w)
+    o = orc.Oracle(w, use_cells=True)
+    o.compute_forces()
+    e = s.energies()
+    pp, pb, _ = o.potential()
+    assert e["pe_bond"] == pytest.approx(pb, rel=1e-5)
+    assert s.box_state()["virial"] == pytest.approx(o.virial(), rel=1e-5)
+    s.step(10)
+    o.run(10)
+    # the straight chains of the start make the dihedral forces ill-conditioned (as in test_gpu_topo): positions and box only
+    compare_state(s, o, positions_only=True)
     s.close()

@@ -57,6 +57,21 @@ def test_virial_is_minus_the_scaling_derivative_of_the_energy():
         assert abs(W) > 1.0
 
 
+def test_angle_and_dihedral_energies_are_scale_free():
+    # orc_virial leaves angles and dihedrals out: their energy must not change when coordinates and box are scaled
+    from tests.test_gpu_topo import with_topology
+    w = with_topology(kg_small(), "harmonic")
+    w.pair_style = "none"
+    w.bond_style = "none"
+    o = orc.Oracle(w, use_cells=False)
+    u0 = o.pair_bond_forces()[2]
+    assert abs(u0) > 1.0
+    pos0, box0 = o.pos.copy(), o.box.copy()
+    o.set_box(box0 * 1.07)
+    assert o.pair_bond_forces(pos=pos0 * 1.07)[2] == pytest.approx(u0, rel=1e-12)
+    assert o.virial(pos0 * 1.07) == 0.0
+
+
 def ideal_gas(n=64, box=6.0, p_ext=0.7, piston_mass=0.02, dt=0.01):
     w = make_random_box(n, [box] * 3, seed=3)
     w.pair_style = "none"
