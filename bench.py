@@ -206,6 +206,8 @@ def measure(gm, torch, w, local, stream, inner, steps, warmup, flags, tune, barr
     s = gm.System(w_run, device=local, flags=flags, tune=tune)
     if w.equil_steps:
         s.step(w.equil_steps)                   # C3: 1,000 Langevin steps (kT=1, gamma=1), then NVE
+        if w.integrator in ("nph", "npt"):
+            s.set_barostat(float(w.p_ext), float(w.piston_mass))
         s.set_integrator(w.integrator, w.kT, 0.0)
     for _ in range(warmup):
         s.step(inner)
@@ -320,6 +322,9 @@ def main():
     ap.add_argument("--tune", action="append", default=[], metavar="FIELD=INT",
                     help="gm_config tuning override (x_cell_div, nl_scan_trip, step_shape, win_capacity); never changes results")
     ap.add_argument("--no-windows", action="store_true", help="GM_FLAG_NO_WINDOWS: 32-bit neighbor rows and L1/L2 gathers")
+    ap.add_argument("--barostat", default=None, metavar="P_EXT,PISTON_MASS",
+                    help="run the config under the Andersen barostat (NPH; information only: two plain kernels per timestep, "
+                         "no CUDA graph, no tile windows -- the roofline block then describes the barostat's force kernel)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true",
@@ -332,6 +337,9 @@ def main():
     w = make_config(args.config, scale=args.scale, n=args.beads)
     if args.skin is not None:
         w.r_skin = float(args.skin)
+    if args.barostat:
+        p_ext, piston = (float(x) for x in args.barostat.split(","))
+        w.integrator, w.p_ext, w.piston_mass = "nph", p_ext, piston
     if args.impl == "reference":
         run_reference(args, w)
         return
