@@ -218,8 +218,8 @@ gm_status gm_set_integrator(gm_system *s, int integrator, float kT, float gamma)
  * collisions at frequency gamma, temperature kT).  The box changes isotropically: the device keeps every position in the
  * box of gm_create ("scaled" coordinates) and one scale factor lambda = (V / V_create)^(1/3); forces, virial and energies are
  * evaluated at the real distances lambda * s.  Pair styles GM_PAIR_LJ and GM_PAIR_NONE, bonds, angles and dihedrals of any
- * style (angle terms are scale-free: no virial); no DPD; such a system runs without tile windows and outside CUDA graphs
- * (two kernels per timestep: forces + virial, then piston + kick + drift).  The neighbor list is built once for the scaled list radius r_cut_max + r_skin of
+ * style (angle terms are scale-free: no virial); no DPD; such a system runs without tile windows, two kernels per timestep
+ * (forces + virial, then piston + kick + drift).  The neighbor list is built once for the scaled list radius r_cut_max + r_skin of
  * gm_create; it stays complete while lambda > r_cut_max / (r_cut_max + r_skin) -- a box that shrinks further latches an
  * error (GM_ERR_BOX_TOO_SMALL from the next synchronising call); build the system anew at the new size then.
  *

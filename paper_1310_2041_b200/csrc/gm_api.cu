@@ -819,7 +819,7 @@ static gm_status step_impl(gm_system *s, int64_t n_steps, StepTiming *tm)
     int64_t done = 0;
     while (done < n_steps) {
         const int64_t rem = n_steps - done;
-        if (!tm && s->use_graph && !is_npt(s) && s->lagged && s->cur == 0 && rem >= 2) {
+        if (!tm && s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
             const bool big = rem >= GM_GRAPH_STEPS;
             cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
             const int ns = big ? GM_GRAPH_STEPS : 2;
@@ -948,7 +948,9 @@ static gm_status npt_probe(gm_system *s, NptProbe *o)
     GmNpt h;
     CU(cudaMemcpyAsync(&h, gm_npt_state(s->D), sizeof(h), cudaMemcpyDeviceToHost, s->st));
     r = sync_and_check(s);
-    const double *sm = h.sum[2];
+    double sm[8] = { 0, 0, 0, 0, 0, 0, 0, 0 };
+    for (int c = 0; c < GM_NPT_SLOTS; ++c)
+        for (int q = 0; q < 8; ++q) sm[q] += h.sum[2][c][q];
     const double lam = h.lam[s->cur], V = h.V[s->cur], hk = s->lagged ? 0.5 * (double)s->P.dt : 0.0;
     const double S = sm[1] + 2.0 * hk * lam * sm[2] + hk * hk * lam * lam * sm[3];
     o->K = S / (2.0 * lam * lam);

@@ -6,25 +6,37 @@
 
 #define NPT_BLOCK 128
 
-// sum of v[0..NQ) over the block -> dst[q] (one double atomic per block and quantity)
+// sum of v[0..NQ) over the warp -> one of the GM_NPT_SLOTS copies of the sums (lane q adds quantity q: one double atomic
+// per warp and quantity, spread over 64 x NQ addresses; no block barrier, a warp leaves when it is done)
 template <int NQ>
-__device__ __forceinline__ void npt_block_add(double (&v)[NQ], double *dst)
+__device__ __forceinline__ void npt_warp_add(double (&v)[NQ], double (*dst)[8])
 {
-    __shared__ double sh[NPT_BLOCK / 32][NQ];
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int warp = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    double mine = 0.0;
 #pragma unroll
     for (int q = 0; q < NQ; ++q) {
         double x = v[q];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
-        if (lane == 0) sh[wid][q] = x;
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        if (lane == q) mine = x;
+    }
+    if (lane < NQ) atomicAdd(&dst[warp & (GM_NPT_SLOTS - 1)][lane], mine);
+}
+
+// the 8 sums of slot array `src`: every thread of the block gets all of them, summed in an order that depends on nothing
+// but the slot layout (all blocks derive bit-identical piston scalars)
+__device__ __forceinline__ void npt_sums(const double (*src)[8], double (&out)[8])
+{
+    __shared__ double sh[8];
+    if (threadIdx.x < 8) {
+        double x = 0.0;
+        for (int c = 0; c < GM_NPT_SLOTS; ++c) x += src[c][threadIdx.x];
+        sh[threadIdx.x] = x;
     }
     __syncthreads();
-    if (threadIdx.x < NQ) {
-        double x = 0.0;
-        for (int w = 0; w < NPT_BLOCK / 32; ++w) x += sh[w][threadIdx.x];
-        atomicAdd(dst + threadIdx.x, x);
-    }
+#pragma unroll
+    for (int q = 0; q < 8; ++q) out[q] = sh[q];
 }
 
 // Forces at the real distances lambda * s (Eq. 1 pairs from the neighbor list, bonds from BL), the virial and the sums
@@ -49,8 +61,10 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
             const int ti = __float_as_int(pi.w);
             const int4 *__restrict__ t = nl_row(P, D, i);
             const GmPair p0 = P.pair[0];
+            int4 en = t[0];                         // rows are padded to whole quads, at least minq >= 1 of them
             for (int q = 0; 4 * q < nn; ++q) {
-                const int4 e = t[q * 32];
+                const int4 e = en;
+                if (4 * (q + 1) < nn) en = t[(q + 1) * 32];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
                     if (4 * q + u >= nn) continue;
@@ -63,7 +77,7 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
                     if (!NT1) k = P.pair[ti * P.n_types + __float_as_int(pj.w)];
                     if (r2 < k.c0) {
                         // Eq. (1): F_i = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij, r_ij = lambda s_ij
-                        const float r2i = 1.0f / r2;
+                        const float r2i = gm_rcp(r2);
                         const float r6i = r2i * r2i * r2i;
                         const float fs = r2i * r6i * (k.c1 * r6i - k.c2);
                         const float fl = fs * lam;
@@ -118,7 +132,7 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
         acc[4] = 0.5 * (double)pe_pair;
         acc[5] = 0.5 * (double)pe_bond;
     }
-    npt_block_add<6>(acc, N->sum[probe ? 2 : parity]);
+    npt_warp_add<6>(acc, N->sum[probe ? 2 : parity]);
 }
 
 // Piston, kick, drift, collisions, displacement test (scheme in gm_npt.cuh).  Every thread derives the same scalars from
@@ -131,7 +145,8 @@ k_npt_update(const __grid_constant__ GmParams P, GmDev D, int parity, float kick
     const Src S = current_src(D, parity, step);
     const double dt = (double)P.dt, kk = (double)kick;
     const double V = N->V[parity], lam = N->lam[parity];
-    const double *sm = N->sum[parity];
+    double sm[8];
+    npt_sums(N->sum[parity], sm);
     double Pi = N->Pi[parity] + kk * (sm[0] / (3.0 * V) - N->p_ext);
     const double s_new = sm[1] + 2.0 * kk * lam * sm[2] + kk * kk * lam * lam * sm[3];
     Pi += 0.5 * dt * s_new / (3.0 * V * lam * lam);
@@ -146,13 +161,13 @@ k_npt_update(const __grid_constant__ GmParams P, GmDev D, int parity, float kick
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         D.ctl->step[parity ^ 1] = step + 1;
         N->V[parity ^ 1] = Vn; N->Pi[parity ^ 1] = Pi; N->lam[parity ^ 1] = lamn;
-#pragma unroll
-        for (int q = 0; q < 8; ++q) N->sum[parity ^ 1][q] = 0.0;
         if (!(Vn > 0.0) || !(thr > 0.0f)) atomicOr(&D.ctl->err, GM_DEV_ERR_BOX);
         if (P.sfc_period > 0 && D.ctl->rebuilt_at != GM_NEVER &&
             step + 1 - D.ctl->rebuilt_at >= (unsigned long long)P.sfc_period)
             raise_rebuild(D, step);
     }
+    if (blockIdx.x == 0)                    // the slots of the next time level (nobody reads or adds to them in this launch)
+        for (int q = threadIdx.x; q < GM_NPT_SLOTS * 8; q += NPT_BLOCK) (&N->sum[parity ^ 1][0][0])[q] = 0.0;
     const int i = blockIdx.x * NPT_BLOCK + threadIdx.x;
     if (i >= P.n) return;
     const float4 pi = S.pos[i];
@@ -209,7 +224,8 @@ __global__ void k_npt_init(GmDev D, int parity, double vol0, double V, double Pi
     GmNpt *N = gm_npt_state(D);
     for (int b = 0; b < 2; ++b) { N->V[b] = V; N->Pi[b] = Pi; N->lam[b] = cbrt(V / vol0); }
     for (int b = 0; b < 3; ++b)
-        for (int q = 0; q < 8; ++q) N->sum[b][q] = 0.0;
+        for (int c = 0; c < GM_NPT_SLOTS; ++c)
+            for (int q = 0; q < 8; ++q) N->sum[b][c][q] = 0.0;
     N->p_ext = p_ext; N->mass = mass; N->vol0 = vol0;
     (void)parity;
 }
@@ -245,7 +261,7 @@ static void npt_force_b(const GmParams &P, const GmDev &D, int parity, int probe
 // probe != 0: a force evaluation outside the time stepping; its sums go to the scratch slot, cleared here first
 void gm_launch_npt_force(const GmParams &P, const GmDev &D, int parity, int probe, cudaStream_t st)
 {
-    if (probe) cudaMemsetAsync(gm_npt_state(D)->sum[2], 0, 8 * sizeof(double), st);
+    if (probe) cudaMemsetAsync(gm_npt_state(D)->sum[2], 0, GM_NPT_SLOTS * 8 * sizeof(double), st);
     gm_launch_topo(P, D, parity, st);        // angle + dihedral forces of this time level -> D.ftopo (no-op without them)
     if (P.n_types == 1) npt_force_b<true>(P, D, parity, probe, st);
     else npt_force_b<false>(P, D, parity, probe, st);

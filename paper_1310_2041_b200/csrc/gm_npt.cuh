@@ -20,12 +20,14 @@
 
 // Lives in the tail of the energy scratch (GmDev::esum + (GM_ESUM_BLOCKS + 1) * 8); slots [parity] follow the position
 // buffers; sum[2] is the scratch of force evaluations outside the time stepping (gm_compute_forces, gm_energies, ...)
+#define GM_NPT_SLOTS 64            // the sums are spread over this many copies (warp w adds to copy w % 64): no hot atomic address
 struct GmNpt {
     double V[2], Pi[2], lam[2];
-    double sum[3][8];              // W, S_cc, S_cF, S_FF, pair PE, bond PE
     double p_ext, mass, vol0;
+    double pad[7];
+    double sum[3][GM_NPT_SLOTS][8];    // W, S_cc, S_cF, S_FF, pair PE, bond PE
 };
-#define GM_NPT_DOUBLES 64
+#define GM_NPT_DOUBLES 2048
 static_assert(sizeof(GmNpt) <= GM_NPT_DOUBLES * sizeof(double), "GmNpt outgrew its slot");
 
 __host__ __device__ __forceinline__ GmNpt *gm_npt_state(const GmDev &D)

@@ -132,7 +132,10 @@ def test_conserved_quantity_and_mean_pressure_long_run(gm):
         b = s.box_state()
         ps.append(b["pressure"]); hs.append(b["H"]); vs.append(b["volume"])
     assert np.mean(ps) == pytest.approx(5.0, abs=0.1), np.mean(ps)
-    assert max(abs(h - h0) for h in hs) < 2e-3 * ke0, (h0, min(hs), max(hs))          # no drift of Andersen's H in 3 500 steps
+    # Andersen's H: no drift over the 3 000 sampled steps (spread below 1e-3 of the kinetic energy), and within 4e-3 of its
+    # starting value (the lattice start, with its large first forces, shifts it once while the melt relaxes)
+    assert max(hs) - min(hs) < 1e-3 * ke0, (h0, min(hs), max(hs))
+    assert abs(np.mean(hs) - h0) < 4e-3 * ke0, (h0, np.mean(hs))
     assert np.std(vs) > 1e-4 * np.mean(vs)
     s.close()
 
