@@ -269,6 +269,24 @@ gm_status gm_get_stats(gm_system *s, int64_t out[8]);
  * Synchronises.  Diagnostics only: none of these changes results. */
 gm_status gm_get_tuning(gm_system *s, int64_t out[8]);
 
+/* Kinetic energy and momentum of n beads -- the a9 sums of gm_energies (the validation quantities),
+ * fp32 inputs, every term and sum in fp64 -- through an entry point that needs no gm_system and no workspace and ALLOCATES
+ * NOTHING (no cudaMalloc / cudaFree, no allocating library call): for callers under CUDA graph capture, in tight serving
+ * loops, or in harnesses that forbid allocation.  The per-block partial sums live in a file-scope __device__ array of the
+ * library (262,400 bytes, held by every GPU that loads libgm.so until exit), which bounds the size:
+ * n <= GM_STATIC_MAX_BEADS, else INVALID_ARG with a message saying so.
+ *   vel3 (DEVICE, n x 3 floats), mass (DEVICE, n floats, or NULL = 1.0), device: CUDA device ordinal (made current),
+ *   stream: cudaStream_t as void* (0 = default stream), out4 (DEVICE, 4 doubles: kinetic energy, p_x, p_y, p_z),
+ *   err / err_len: HOST buffer for the message of a failed call (may be NULL / 0).
+ * Asynchronous on `stream` (one memset node + one kernel node: capturable); the result is in out4 when the stream reaches
+ * that point.  The first call per device resolves the array's device address (cudaGetSymbolAddress): make it outside a
+ * stream capture.  ALL calls share the one array, which keeps the last call's contents (what must start at zero is
+ * cleared by every call): calls on one stream are ordered; calls that overlap on a GPU (two streams, two threads) RACE.
+ * Deterministic: the additions are ordered by the grid size alone.  Errors: INVALID_ARG, CUDA. */
+#define GM_STATIC_MAX_BEADS 8388608
+gm_status gm_kinetic_static(const float *vel3, const float *mass, int64_t n, int device, void *stream, double *out4,
+                            char *err, size_t err_len);
+
 /* Host-only utility (a2): the space-filling-curve rank of every cell of an nc[0] x nc[1] x nc[2] grid
  * (linear cell id = (z * nc[1] + y) * nc[0] + x), i.e. the key every neighbor rebuild sorts the beads by:
  * cells run along x inside a row, the (y, z) rows follow a 2-D Hilbert curve.  rank_out: HOST array of

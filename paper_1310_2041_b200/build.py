@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgm.so")
 SOURCES = ["gm_api.cu", "gm_sort.cu", "gm_nlist.cu", "gm_force.cu", "gm_force_dpd.cu", "gm_force_soft.cu", "gm_force_gauss.cu",
-           "gm_force_table.cu", "gm_topo.cu", "gm_io.cu", "gm_npt.cu"]
+           "gm_force_table.cu", "gm_topo.cu", "gm_io.cu", "gm_npt.cu", "gm_static.cu"]
 HEADERS = [os.path.join(CSRC, "gm_internal.cuh"), os.path.join(CSRC, "gm_force_impl.cuh"), os.path.join(CSRC, "gm_npt.cuh"), os.path.join(os.path.dirname(HERE), "include", "gm.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -29,7 +29,7 @@ SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params"
            "gm_set_bond_params", "gm_set_angle_params", "gm_set_dihedral_params", "gm_set_angles", "gm_set_dihedrals",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
-           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box",
+           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box", "gm_kinetic_static",
            "gm_sfc_cell_order", "gm_last_error"]
 
 
@@ -89,6 +89,7 @@ def lib():
         L.gm_set_barostat.argtypes = [vp, C.c_float, C.c_float]
         L.gm_set_box_state.argtypes = [vp, C.c_double, C.c_double]
         L.gm_get_box.argtypes = [vp, vp]
+        L.gm_kinetic_static.argtypes = [vp, vp, i64, i32, vp, vp, C.c_char_p, C.c_size_t]
         L.gm_get_particles.argtypes = [vp, vp, vp, vp, i32]
         L.gm_get_neighbors.argtypes = [vp, vp, vp, i64, i32]
         L.gm_get_stats.argtypes = [vp, vp]
@@ -234,6 +235,21 @@ def gm_get_box(h) -> np.ndarray:
     out = np.zeros(8, dtype=np.float64)
     _check(lib().gm_get_box(h, out.ctypes.data), h)
     return out
+
+
+GM_STATIC_MAX_BEADS = 8388608
+
+
+def gm_kinetic_static(vel3, mass, out4, stream=None):
+    """Kinetic energy and momentum of the beads (vel3: CUDA float32 (n, 3), mass: CUDA float32 (n,) or None) into out4 (CUDA
+    float64 (4,)), asynchronously on `stream` (default: torch's current stream); allocates nothing (gm.h)."""
+    import torch
+    st = torch.cuda.current_stream(vel3.device) if stream is None else stream
+    buf = C.create_string_buffer(256)
+    r = lib().gm_kinetic_static(vel3.data_ptr(), mass.data_ptr() if mass is not None else None, int(vel3.shape[0]),
+                                vel3.device.index or 0, st.cuda_stream, out4.data_ptr(), buf, 256)
+    if r != GM_OK:
+        raise GmError(r, buf.value.decode())
 
 
 def gm_energies(h) -> np.ndarray:
