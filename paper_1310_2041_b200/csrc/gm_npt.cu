@@ -39,6 +39,50 @@ __device__ __forceinline__ void npt_sums(const double (*src)[8], double (&out)[8
     for (int q = 0; q < 8; ++q) out[q] = sh[q];
 }
 
+// Eq. (1) over row i of the neighbor list at the real distances lambda * s; e0: the row's first quad (already loaded).
+// MI: minimum-image differences (a warp with a bead near a face), else plain ones.  The four gathers of a quad are
+// issued together; slots past NN hold the far-away pad bead, which the branch-free term turns into zero.
+template <bool NT1, bool MI>
+__device__ __forceinline__ void npt_pairs(const GmParams &P, const GmDev &D, const Src &S, int i, const float4 pi, int nn,
+                                          int4 e0, float lam, float lam2, float &fx, float &fy, float &fz, float &w,
+                                          float &pe_pair)
+{
+    const int ti = __float_as_int(pi.w);
+    const int4 *__restrict__ t = nl_row(P, D, i);
+    const GmPair p0 = P.pair[0];
+    int4 en = e0;
+    for (int q = 0; 4 * q < nn; ++q) {
+        const int4 e = en;
+        if (4 * (q + 1) < nn) en = t[(q + 1) * 32];
+        float4 pj[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) pj[u] = __ldg(S.pos + quad_get(e, u));
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            float dx, dy, dz;
+            if (MI) {
+                dx = gm_min_image(pi.x, pj[u].x, P.half[0]);
+                dy = gm_min_image(pi.y, pj[u].y, P.half[1]);
+                dz = gm_min_image(pi.z, pj[u].z, P.half[2]);
+            } else {
+                dx = pi.x - pj[u].x; dy = pi.y - pj[u].y; dz = pi.z - pj[u].z;
+            }
+            const float r2 = lam2 * (dx * dx + dy * dy + dz * dz);
+            GmPair k = p0;
+            if (!NT1) k = P.pair[ti * P.n_types + __float_as_int(pj[u].w)];
+            // Eq. (1): F_i = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij, r_ij = lambda s_ij
+            const bool in = r2 < k.c0;
+            const float r2i = gm_rcp(r2);
+            const float r6i = r2i * r2i * r2i;
+            const float fs = in ? r2i * r6i * (k.c1 * r6i - k.c2) : 0.0f;
+            const float fl = fs * lam;
+            fx += fl * dx; fy += fl * dy; fz += fl * dz;
+            w += in ? fs * r2 : 0.0f;
+            pe_pair += in ? r6i * (k.c1 * (1.0f / 12.0f) * r6i - k.c2 * (1.0f / 6.0f)) - k.c3 : 0.0f;
+        }
+    }
+}
+
 // Forces at the real distances lambda * s (Eq. 1 pairs from the neighbor list, bonds from BL), the virial and the sums
 // the piston needs.  D.frc[i] = (F, the bead's half share of the potential energy).
 template <bool NT1, int BOND, bool PAIRS>
@@ -53,40 +97,19 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
     const int i = blockIdx.x * NPT_BLOCK + threadIdx.x;
     double acc[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     if (i < P.n) {
+        // every stream of the bead is requested before anything is used
         const float4 pi = S.pos[i];
+        const int4 e0 = PAIRS ? nl_row(P, D, i)[0] : make_int4(0, 0, 0, 0);
+        const int nn = PAIRS ? D.nn[i] : 0;
         const float4 c = S.vel[i];
         float fx = 0.f, fy = 0.f, fz = 0.f, w = 0.f, pe_pair = 0.f, pe_bond = 0.f;
         if (PAIRS) {
-            const int nn = D.nn[i];
-            const int ti = __float_as_int(pi.w);
-            const int4 *__restrict__ t = nl_row(P, D, i);
-            const GmPair p0 = P.pair[0];
-            int4 en = t[0];                         // rows are padded to whole quads, at least minq >= 1 of them
-            for (int q = 0; 4 * q < nn; ++q) {
-                const int4 e = en;
-                if (4 * (q + 1) < nn) en = t[(q + 1) * 32];
-#pragma unroll
-                for (int u = 0; u < 4; ++u) {
-                    if (4 * q + u >= nn) continue;
-                    const float4 pj = __ldg(S.pos + quad_get(e, u));
-                    const float dx = gm_min_image(pi.x, pj.x, P.half[0]);
-                    const float dy = gm_min_image(pi.y, pj.y, P.half[1]);
-                    const float dz = gm_min_image(pi.z, pj.z, P.half[2]);
-                    const float r2 = lam2 * (dx * dx + dy * dy + dz * dz);
-                    GmPair k = p0;
-                    if (!NT1) k = P.pair[ti * P.n_types + __float_as_int(pj.w)];
-                    if (r2 < k.c0) {
-                        // Eq. (1): F_i = r^-2 r^-6 (48 eps s^12 r^-6 - 24 eps s^6) r_ij, r_ij = lambda s_ij
-                        const float r2i = gm_rcp(r2);
-                        const float r6i = r2i * r2i * r2i;
-                        const float fs = r2i * r6i * (k.c1 * r6i - k.c2);
-                        const float fl = fs * lam;
-                        fx += fl * dx; fy += fl * dy; fz += fl * dz;
-                        w += fs * r2;
-                        pe_pair += r6i * (k.c1 * (1.0f / 12.0f) * r6i - k.c2 * (1.0f / 6.0f)) - k.c3;
-                    }
-                }
-            }
+            // a bead further than r_list + skin (scaled) from every face has no listed partner across the boundary:
+            // plain differences; decided per warp so that a warp runs one of the two loops
+            const float m = P.edge_margin;
+            const bool interior = fabsf(pi.x) < P.half[0] - m && fabsf(pi.y) < P.half[1] - m && fabsf(pi.z) < P.half[2] - m;
+            if (__all_sync(__activemask(), interior)) npt_pairs<NT1, false>(P, D, S, i, pi, nn, e0, lam, lam2, fx, fy, fz, w, pe_pair);
+            else npt_pairs<NT1, true>(P, D, S, i, pi, nn, e0, lam, lam2, fx, fy, fz, w, pe_pair);
         }
         if (BOND != GM_BOND_NONE) {
             for (int b = 0; b < P.max_bonds; ++b) {
