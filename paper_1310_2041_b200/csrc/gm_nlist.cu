@@ -15,14 +15,18 @@
 // [NL_STAGE][32]: conflict-free and private to the lane, so no synchronisation); candidates are scanned
 // four at a time, and after each four every lane that holds 16 or more staged entries writes four whole
 // int4 quads of its NL row (gm_internal.cuh: entries 4q..4q+3 of a bead are one int4; the 32 int4 of a
-// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 20 KB per CTA
-// whatever the row capacity, which leaves the rest of the SM's 228 KB to L1 for the candidate loads.
+// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 10 KB (four candidates per
+// trip: ring of 16, flushed by halves) or 20 KB (eight: ring of 32) per CTA whatever the row capacity, which leaves
+// the rest of the SM's 228 KB to L1 for the candidate loads.
 #include "gm_internal.cuh"
 
 #ifndef NL_MINB_WIN
 #define NL_MINB_WIN 6          // resident CTAs per SM the window-system build is compiled for (77 registers, no spills; 8 -> 64 registers with spills measured 1 % slower on C2 / C5)
 #endif
-#define NL_STAGE 32          // ring entries per lane (power of two, >= 16 + 8)
+#define NL_STAGE 32          // ring entries per lane of the kernels that scan 8 candidates per trip (power of two)
+// ring entries per lane by trip width: a lane flushes half a ring when that much is staged, so the ring must hold
+// (half - 1) + TRIP entries: 16 for TRIP = 4 (8 KB per CTA), 32 for TRIP = 8
+#define NL_STAGE_OF(TRIP) ((TRIP) == 4 ? 16 : 32)
 #ifndef NL_COOP
 #define NL_COOP 1            // dense cells: warps of one piece scan the union of their lanes' runs together (nl_scan_warp)
 #endif
@@ -63,32 +67,33 @@ struct NlRow {
 
 __device__ __forceinline__ uint32_t nl_pack2(int lo, int hi) { return (uint32_t)lo | ((uint32_t)hi << 16); }
 
-// write entries [flushed, flushed + 16) of the row from the ring to the tile: four quads of 32-bit bead indices, or
-// (W16) two octs of 16-bit window offsets
-template <bool W16>
-__device__ __forceinline__ void nl_flush16(NlRow &r)
+// write entries [flushed, flushed + STAGE / 2) of the row from the ring to the tile: quads of 32-bit bead indices, or
+// (W16) octs of 16-bit window offsets
+template <int STAGE, bool W16>
+__device__ __forceinline__ void nl_flush_half(NlRow &r)
 {
-    if (r.flushed + 16 <= r.cap) {
+    constexpr int H = STAGE / 2;
+    if (r.flushed + H <= r.cap) {
         if (W16) {
 #pragma unroll
-            for (int o = 0; o < 2; ++o) {
+            for (int o = 0; o < H / 8; ++o) {
                 const int e = r.flushed + 8 * o;
                 int v[8];
 #pragma unroll
-                for (int u = 0; u < 8; ++u) v[u] = r.ring[((e + u) & (NL_STAGE - 1)) * 32];
+                for (int u = 0; u < 8; ++u) v[u] = r.ring[((e + u) & (STAGE - 1)) * 32];
                 r.tile[(e >> 3) * 32] = make_int4((int)nl_pack2(v[0], v[1]), (int)nl_pack2(v[2], v[3]),
                                                   (int)nl_pack2(v[4], v[5]), (int)nl_pack2(v[6], v[7]));
             }
         } else {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
+            for (int q = 0; q < H / 4; ++q) {
                 const int e = r.flushed + 4 * q;
-                r.tile[(e >> 2) * 32] = make_int4(r.ring[((e + 0) & (NL_STAGE - 1)) * 32], r.ring[((e + 1) & (NL_STAGE - 1)) * 32],
-                                                  r.ring[((e + 2) & (NL_STAGE - 1)) * 32], r.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+                r.tile[(e >> 2) * 32] = make_int4(r.ring[((e + 0) & (STAGE - 1)) * 32], r.ring[((e + 1) & (STAGE - 1)) * 32],
+                                                  r.ring[((e + 2) & (STAGE - 1)) * 32], r.ring[((e + 3) & (STAGE - 1)) * 32]);
             }
         }
     }
-    r.flushed += 16;
+    r.flushed += H;
 }
 
 // Append candidate s to the lane's ring column if it is inside the run (u < left), inside r_list and
@@ -96,7 +101,7 @@ __device__ __forceinline__ void nl_flush16(NlRow &r)
 // The address is (kb & mask) | lb, one LOP3 (the warp's ring is 4 KB-aligned, so the two terms share no
 // bits); store and increment are predicated on the hit (written in PTX: the compiler otherwise builds the
 // increment from three selects).
-template <bool SELF>
+template <bool SELF, int STAGE>
 __device__ __forceinline__ void nl_append(uint32_t &kb, uint32_t lb, float r2, float r_list2, int left, int u,
                                           int s, int i)
 {
@@ -105,13 +110,13 @@ __device__ __forceinline__ void nl_append(uint32_t &kb, uint32_t lb, float r2, f
                      "setp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
                      "setp.ne.and.s32 p, %5, %6, p;\n\t@p st.shared.b32 [t], %5;\n\t@p add.u32 %0, %0, 128;\n\t}"
                      : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u), "r"(s), "r"(i),
-                       "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
+                       "n"((STAGE - 1) * 128), "r"(lb) : "memory");
     else
         asm volatile("{\n\t.reg .pred v, p;\n\t.reg .b32 t;\n\tlop3.b32 t, %0, %7, %8, 0xEA;\n\t"
                      "setp.gt.s32 v, %3, %4;\n\tsetp.lt.and.f32 p, %1, %2, v;\n\t"
                      "@p st.shared.b32 [t], %5;\n\t@p add.u32 %0, %0, 128;\n\t}"
                      : "+r"(kb) : "f"(r2), "f"(r_list2), "r"(left), "r"(u), "r"(s), "r"(i),
-                       "n"((NL_STAGE - 1) * 128), "r"(lb) : "memory");
+                       "n"((STAGE - 1) * 128), "r"(lb) : "memory");
 }
 
 // One run of candidates ref[s0 .. s1) against bead i, TRIP at a time, every one predicated on s < s1 (the
@@ -125,6 +130,7 @@ __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int 
                                             float ay, float az, float hx, float hy, float hz, float r_list2,
                                             NlRow &r)
 {
+    constexpr int STAGE = NL_STAGE_OF(TRIP);
     uint32_t kb = (uint32_t)r.k * 128u;
     const int ie = i + delta;
     for (int s = s0; s < s1; s += TRIP) {
@@ -141,11 +147,11 @@ __device__ __forceinline__ void nl_scan_run(const float4 *__restrict__ ref, int 
             if (SHIFT) { dx = ax - (q[u].x + hx); dy = ay - (q[u].y + hy); dz = az - (q[u].z + hz); }
             else { dx = ax - q[u].x; dy = ay - q[u].y; dz = az - q[u].z; }
             const float r2 = dx * dx + dy * dy + dz * dz;
-            nl_append<SELF>(kb, r.lb, r2, r_list2, left, u, se + u, ie);
+            nl_append<SELF, STAGE>(kb, r.lb, r2, r_list2, left, u, se + u, ie);
         }
-        // at most TRIP <= 8 new entries per trip: flush as soon as 16 are staged (ring of 32)
+        // at most TRIP new entries per trip: flush as soon as half a ring is staged
         r.k = (int)(kb >> 7);
-        if (r.k - r.flushed >= 16) nl_flush16<W16>(r);
+        if (r.k - r.flushed >= STAGE / 2) nl_flush_half<STAGE, W16>(r);
     }
 }
 
@@ -421,22 +427,26 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     if (!D.ctl->go) return;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    // shared memory: [NL_WARPS][NL_STAGE][32] ring ints, 4 KB per warp, aligned by hand to 4 KB in the shared window
-    // (nl_append ORs the entry offset into the lane's base address; the launch asks for 4 KB of slack), then the
-    // range slots of the CTA's tile window and the scratch of its set-up
+    // shared memory: [NL_WARPS][STAGE][32] ring ints, a warp's ring (STAGE * 128 bytes: 2 or 4 KB) aligned by hand to its
+    // size in the shared window (nl_append ORs the entry offset into the lane's base address; the launch asks for that
+    // much slack), then the range slots of the CTA's tile window and the scratch of its set-up
+    constexpr int STAGE = NL_STAGE_OF(TRIP);
+    constexpr uint32_t RALIGN = STAGE * 128u;
     extern __shared__ int nl_smem_raw[];
     const uint32_t raw = (uint32_t)__cvta_generic_to_shared(nl_smem_raw);
-    int *nl_ring = nl_smem_raw + (((raw + 4095u) & ~4095u) - raw) / 4;
-    int4 *rng = reinterpret_cast<int4 *>(nl_ring + NL_WARPS * NL_STAGE * 32);       // [GM_WIN_SLOTS], then cell[GM_TILE], mode
+    int *nl_ring = nl_smem_raw + (((raw + RALIGN - 1u) & ~(RALIGN - 1u)) - raw) / 4;
+    // behind the rings, window systems only: [GM_WIN_SLOTS] range slots, cell[GM_TILE], mode, then (TRIP == 8) the candidate
+    // buffers [NL_WARPS][2][32] of the union scan
+    int4 *rng = reinterpret_cast<int4 *>(nl_ring + NL_WARPS * STAGE * 32);
     int4 *cell = rng + GM_WIN_SLOTS;
     int *sh_mode = reinterpret_cast<int *>(cell + GM_TILE);
-    float4 *ubuf = reinterpret_cast<float4 *>(cell + GM_TILE + 1) + wid * 64;     // [NL_WARPS][2][32] candidates (TRIP == 8)
+    float4 *ubuf = reinterpret_cast<float4 *>(cell + GM_TILE + 1) + wid * 64;
     NlWin W;
     W.rng = rng;
     W.group = 0;
     W.whole = WINS && P.n <= P.win_cap;
     NlRow row;
-    row.ring = nl_ring + wid * (NL_STAGE * 32) + lane;
+    row.ring = nl_ring + wid * (STAGE * 32) + lane;
     row.lb = (uint32_t)__cvta_generic_to_shared(row.ring);
     row.tile = D.nl + ((size_t)(i >> 5) * P.capq) * 32 + lane;
     row.k = 0; row.flushed = 0; row.cap = P.nl_cap;
@@ -475,22 +485,22 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     const int kc = min(row.k, cap);
     if (WINS && mode) {
         const int no = max((kc + 7) >> 3, P.minq >> 1);
-        for (int e = max(kc, row.flushed); e < 8 * no; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = 0;
+        for (int e = max(kc, row.flushed); e < 8 * no; ++e) row.ring[(e & (STAGE - 1)) * 32] = 0;
         for (int o = row.flushed >> 3; o < no; ++o) {
             const int e = 8 * o;
             int v[8];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) v[u] = row.ring[((e + u) & (NL_STAGE - 1)) * 32];
+            for (int u = 0; u < 8; ++u) v[u] = row.ring[((e + u) & (STAGE - 1)) * 32];
             row.tile[o * 32] = make_int4((int)nl_pack2(v[0], v[1]), (int)nl_pack2(v[2], v[3]),
                                          (int)nl_pack2(v[4], v[5]), (int)nl_pack2(v[6], v[7]));
         }
     } else {
         const int nq = max((kc + 3) >> 2, P.minq);
-        for (int e = max(kc, row.flushed); e < 4 * nq; ++e) row.ring[(e & (NL_STAGE - 1)) * 32] = P.n;
+        for (int e = max(kc, row.flushed); e < 4 * nq; ++e) row.ring[(e & (STAGE - 1)) * 32] = P.n;
         for (int q = row.flushed >> 2; q < nq; ++q) {
             const int e = 4 * q;
-            row.tile[q * 32] = make_int4(row.ring[((e + 0) & (NL_STAGE - 1)) * 32], row.ring[((e + 1) & (NL_STAGE - 1)) * 32],
-                                         row.ring[((e + 2) & (NL_STAGE - 1)) * 32], row.ring[((e + 3) & (NL_STAGE - 1)) * 32]);
+            row.tile[q * 32] = make_int4(row.ring[((e + 0) & (STAGE - 1)) * 32], row.ring[((e + 1) & (STAGE - 1)) * 32],
+                                         row.ring[((e + 2) & (STAGE - 1)) * 32], row.ring[((e + 3) & (STAGE - 1)) * 32]);
         }
     }
     if (i < P.ns) D.nn[i] = kc;
@@ -549,11 +559,13 @@ k_bl_remap(const __grid_constant__ GmParams P, GmDev D)
 
 int gm_nl_capacity_ok(const GmParams &P) { return P.nl_cap >= 8 && P.nl_cap % 8 == 0; }
 
-// dynamic shared memory of k_nl_build: the rings (+ 4 KB of alignment slack), the range slots and the set-up scratch
+// dynamic shared memory of k_nl_build: the rings (+ one warp's ring of alignment slack), then what the variant needs
 int gm_nl_smem_bytes(const GmParams &P)
 {
-    (void)P;
-    return NL_WARPS * NL_STAGE * 32 * 4 + 4096 + (GM_WIN_SLOTS + GM_TILE + 1) * 16 + NL_WARPS * 64 * 16;
+    const int stage = NL_STAGE_OF(P.nl_trip);
+    int b = NL_WARPS * stage * 32 * 4 + stage * 128;
+    if (P.use_win) b += (GM_WIN_SLOTS + GM_TILE + 1) * 16 + (P.nl_trip == 8 ? NL_WARPS * 64 * 16 : 0);
+    return b;
 }
 
 cudaError_t gm_nl_prepare(const GmParams &P)
