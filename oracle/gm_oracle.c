@@ -23,6 +23,8 @@
  *   - harmonic repulsion Eq. (2), Gaussian repulsion Eq. (3)
  *   - tabulated pair potential: cubic spline in z = r^2, Eq. (12); F = -2 r dV/dz, Eq. (11);
  *     cutoff = "point < Npoint", Alg. 2 lines 8-12
+ *   - tabulated bond potential: the same spline in z = r^2 per bond type (L118: "numerical non-bonded,
+ *     bond ... potentials"); a bond past the end of its table is an error (reading c-32)
  *   - angle potentials Eqs. (8), (9) and the periodic dihedral Eq. (10), each interaction
  *     stored under every member with its position
  *     (theta = angle at the middle bead between the two bonds, pi for a straight chain; phi = 0
@@ -52,7 +54,7 @@
 #endif
 
 enum { ORC_PAIR_NONE = 0, ORC_PAIR_LJ = 1, ORC_PAIR_DPD = 2, ORC_PAIR_HARMONIC = 3, ORC_PAIR_GAUSS = 4, ORC_PAIR_TABLE = 5 };
-enum { ORC_BOND_NONE = 0, ORC_BOND_FENE = 1, ORC_BOND_HARMONIC = 2 };
+enum { ORC_BOND_NONE = 0, ORC_BOND_FENE = 1, ORC_BOND_HARMONIC = 2, ORC_BOND_TABLE = 3 };
 enum { ORC_NVE = 0, ORC_LANGEVIN = 1, ORC_GWVV = 2, ORC_NOSE_HOOVER = 3, ORC_ANDERSEN = 4, ORC_BERENDSEN = 5,
        ORC_NPH = 6, ORC_NPT = 7 };
 enum { ORC_OK = 0, ORC_ERR_BOND_OVERSTRETCH = -7, ORC_ERR_ARG = -1 };
@@ -99,6 +101,13 @@ typedef struct {
        momentum Pi = M dV/dt, baro[3] = virial W = sum over pairs and bonds of r_ij . F_ij at the current positions,
        baro[4] = 1 once baro[3] is valid.  The volume is box[0] box[1] box[2]: orc_run rescales box[] in place.       */
     double *baro;
+    /* ORC_BOND_TABLE: "numerical ... bond ... potentials" as cubic splines on a grid of z = r^2, Eq. (12),
+       F = -2 r dV/dz, Eq. (11): btable[(bond_type * btable_points + point) * 4 + {0,1,2,3}] = c0..c3 with one grid interval
+       per bond type.  A bond stretched past its table (point >= btable_points) has no defined energy: reported as
+       ORC_ERR_BOND_OVERSTRETCH, no force (reading c-32).                                                    */
+    const double *btable;
+    int32_t btable_points;
+    const double *btable_interval;      /* per bond type */
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -450,6 +459,15 @@ int orc_pair_bond_forces(const orc_params *p, const double *pos, const double *v
                 if (!(q > 0.0)) { status = ORC_ERR_BOND_OVERSTRETCH; continue; }
                 fs = -k / q;
                 pe_bond += -0.5 * k * r0 * r0 * log(q);
+            } else if (p->bond_style == ORC_BOND_TABLE) {
+                /* Eqs. (11)-(12) with x = z = r^2: point = int(z / interval); delta = z - point * interval */
+                double h = p->btable_interval[p->bond_type[b]];
+                long point = (long)(r2 / h);
+                if (!(point < p->btable_points)) { status = ORC_ERR_BOND_OVERSTRETCH; continue; }
+                const double *c = p->btable + ((size_t)p->bond_type[b] * p->btable_points + point) * 4;
+                double d = r2 - (double)point * h;
+                fs = -2.0 * (c[1] + 2.0 * c[2] * d + 3.0 * c[3] * d * d);
+                pe_bond += c[0] + c[1] * d + c[2] * d * d + c[3] * d * d * d;
             } else {
                 /* Eq. (7): U = k (r - r0)^2;  F_i = -2 k (1 - r0/r) r_ij */
                 double r = sqrt(r2);
@@ -566,6 +584,13 @@ int orc_virial(const orc_params *p, const double *pos, double *w_out)
                 double q = 1.0 - r2 / (r0 * r0);                     /* F_ij = -k r_ij / q */
                 if (!(q > 0.0)) { status = ORC_ERR_BOND_OVERSTRETCH; continue; }
                 w += -k / q * r2;
+            } else if (p->bond_style == ORC_BOND_TABLE) {
+                double h = p->btable_interval[p->bond_type[b]];           /* F_ij = -2 dV/dz r_ij */
+                long point = (long)(r2 / h);
+                if (!(point < p->btable_points)) { status = ORC_ERR_BOND_OVERSTRETCH; continue; }
+                const double *c = p->btable + ((size_t)p->bond_type[b] * p->btable_points + point) * 4;
+                double d = r2 - (double)point * h;
+                w += -2.0 * (c[1] + 2.0 * c[2] * d + 3.0 * c[3] * d * d) * r2;
             } else {
                 double r = sqrt(r2);                                 /* F_ij = -2 k (r - r0) r_ij / r */
                 w += -2.0 * k * (r - r0) * r;

@@ -18,7 +18,7 @@ _SRC = os.path.join(_HERE, "gm_oracle.c")
 _LIB = os.path.join(_HERE, "libgm_oracle.so")
 
 PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
-BOND = {"none": 0, "fene": 1, "harmonic": 2}
+BOND = {"none": 0, "fene": 1, "harmonic": 2, "table": 3}
 INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5, "nph": 6, "npt": 7}
 ORC_ERR_BOND_OVERSTRETCH = -7
 
@@ -52,6 +52,7 @@ class _Params(C.Structure):
         ("dih_i", C.c_void_p), ("dih_j", C.c_void_p), ("dih_k", C.c_void_p), ("dih_l", C.c_void_p), ("dih_type", C.c_void_p),
         ("dih_kk", C.c_void_p), ("dih_delta", C.c_void_p), ("dih_n", C.c_void_p),
         ("thermo", C.c_void_p), ("baro", C.c_void_p),
+        ("btable", C.c_void_p), ("btable_points", C.c_int32), ("btable_interval", C.c_void_p),
     ]
 
 
@@ -227,8 +228,8 @@ class Oracle:
         self.bond_i = np.ascontiguousarray(b[:, 0])
         self.bond_j = np.ascontiguousarray(b[:, 1])
         self.bond_type = np.ascontiguousarray(w.bond_type, dtype=np.int32)
-        self.bond_k = np.ascontiguousarray(w.bond["k"], dtype=np.float64)
-        self.bond_r0 = np.ascontiguousarray(w.bond["r0"], dtype=np.float64)
+        self.bond_k = np.ascontiguousarray(w.bond.get("k", [0.0]), dtype=np.float64)
+        self.bond_r0 = np.ascontiguousarray(w.bond.get("r0", [0.0]), dtype=np.float64)
         self.step = 0
         self.P = _Params()
         P = self.P
@@ -279,6 +280,14 @@ class Oracle:
         self.baro[0] = float(np.float32(getattr(w, "p_ext", 0.0)))
         self.baro[1] = float(np.float32(getattr(w, "piston_mass", 1.0)))
         P.baro = _p(self.baro).value
+        if w.bond_style == "table":
+            # w.bond = dict(table=(n_bond_types, Npoint, 4) fp32 coefficients as the GPU gets them, interval=(n_bond_types,))
+            self.btable = np.ascontiguousarray(w.bond["table"], np.float64)
+            self.btable = self.btable.reshape(-1, self.btable.shape[-2], 4)
+            self.btable_interval = np.ascontiguousarray(np.asarray(w.bond["interval"], np.float32).reshape(-1), np.float64)
+            P.btable = _p(self.btable).value
+            P.btable_points = int(self.btable.shape[1])
+            P.btable_interval = _p(self.btable_interval).value
         if w.pair_style == "table":
             P.table = _p(self.table).value
             P.table_points = int(self.table.shape[2])
