@@ -64,7 +64,7 @@ enum {
 };
 
 enum { GM_PAIR_NONE = 0, GM_PAIR_LJ = 1, GM_PAIR_DPD = 2, GM_PAIR_HARMONIC = 3, GM_PAIR_GAUSS = 4, GM_PAIR_TABLE = 5 };
-enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2 };
+enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2, GM_BOND_TABLE = 3 };
 enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2,
        GM_NVT_NOSE_HOOVER = 3, GM_NVT_ANDERSEN = 4, GM_NVT_BERENDSEN = 5,     /* PAPER.md:L133, L137; DESIGN.md c-28..c-30 */
        GM_NPH_ANDERSEN = 6, GM_NPT_ANDERSEN = 7 };                            /* Andersen barostat; DESIGN.md c-31 */
@@ -106,6 +106,7 @@ typedef struct {
     int32_t angle_style;             /* GM_ANGLE_*                                                                     */
     int32_t max_angles_per_particle; /* rows of the per-particle angle table; 0 = no angles              */
     int32_t max_dihedrals_per_particle; /* rows of the per-particle dihedral table; 0 = no dihedrals (Eq. (10))         */
+    int32_t bond_table_points;       /* GM_BOND_TABLE: grid points of every bond table; else 0                          */
 } gm_config;
 
 enum {
@@ -158,6 +159,14 @@ gm_status gm_fit_pair_table(int n_point, double interval, const double *v, float
 /* Bond parameters of bond type `btype`: FENE (k, R0): U = -1/2 k R0^2 ln(1 - r^2/R0^2);
  * harmonic (k, r0): U = k (r - r0)^2 -- Eq. (7), no factor 1/2. */
 gm_status gm_set_bond_params(gm_system *s, int btype, float k, float r0_or_R0);
+
+/* GM_BOND_TABLE ("numerical non-bonded, bond, angle, and torsion potentials", Eqs. (11)-(12)): the potential
+ * of bond type `btype` as cubic-spline coefficients on a grid of z = r^2, in the layout of gm_set_pair_table: c4 is a HOST
+ * array of 4 * cfg.bond_table_points floats, V(z_k + d) = c0 + c1 d + c2 d^2 + c3 d^3 with z_k = k * interval, force
+ * F_i = -2 r_ij dV/dz (gm_fit_pair_table fits such a table through values on the grid).  A bond stretched past the end of
+ * its table, int(r^2 / interval) >= bond_table_points, has no defined energy: it exerts no force and latches
+ * GM_ERR_BOND_OVERSTRETCH (reading c-32).  Copies c4 in (synchronises).  Errors: STATE, INVALID_ARG. */
+gm_status gm_set_bond_table(gm_system *s, int btype, float interval, const float *c4);
 
 /* Particles in tag order, length N each: pos3/vel3 are (N,3) row-major floats, type is int32 in
  * [0, n_types), mass may be NULL (all 1).  Positions outside the box are wrapped in.  Resets the

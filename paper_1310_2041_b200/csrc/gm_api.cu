@@ -58,7 +58,9 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (c->pair_style < GM_PAIR_NONE || c->pair_style > GM_PAIR_TABLE) return GM_ERR_INVALID_ARG;
     if (c->table_points < 0 || c->table_points > (1 << 20) || ((c->pair_style == GM_PAIR_TABLE) != (c->table_points > 0)))
         return GM_ERR_INVALID_ARG;
-    if (c->bond_style < GM_BOND_NONE || c->bond_style > GM_BOND_HARMONIC) return GM_ERR_INVALID_ARG;
+    if (c->bond_style < GM_BOND_NONE || c->bond_style > GM_BOND_TABLE) return GM_ERR_INVALID_ARG;
+    if (c->bond_table_points < 0 || c->bond_table_points > (1 << 20) || ((c->bond_style == GM_BOND_TABLE) != (c->bond_table_points > 0)))
+        return GM_ERR_INVALID_ARG;
     if (c->integrator < GM_NVE || c->integrator > GM_NPT_ANDERSEN) return GM_ERR_INVALID_ARG;
     if ((c->integrator == GM_DPD_GWVV) != (c->pair_style == GM_PAIR_DPD)) return GM_ERR_INVALID_ARG;
     const bool npt = c->integrator == GM_NPH_ANDERSEN || c->integrator == GM_NPT_ANDERSEN;
@@ -167,6 +169,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     }
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
     P->table_points = c->table_points;      // (memset above: every pair coefficient starts at 0 = no interaction)
+    P->bond_table_points = c->bond_table_points;
     return GM_OK;
 }
 
@@ -191,6 +194,7 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     }
     d.frc = (float4 *)take(n * 16);
     if (P.table_points > 0) d.table = (float4 *)take((size_t)P.n_types * P.n_types * P.table_points * 16);
+    if (P.bond_table_points > 0) d.btable = (float4 *)take((size_t)GM_MAX_BOND_TYPES * P.bond_table_points * 16);
     if (P.max_angles + P.max_dihedrals > 0) d.ftopo = (float4 *)take(n * 16);
     if (P.max_angles > 0) d.at = (int4 *)take(n * 16 * (size_t)P.max_angles);
     if (P.max_dihedrals > 0) d.dt = (int4 *)take(n * 16 * (size_t)P.max_dihedrals);
@@ -307,6 +311,7 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     s->P = P;
     carve(P, *cfg, (char *)dev_workspace, &s->D);
     s->P.table = s->D.table;
+    s->P.btable = s->D.btable;
     s->st = (cudaStream_t)cfg->stream;
     s->use_graph = !(cfg->flags & GM_FLAG_NO_GRAPH);
     s->use_cond = !(cfg->flags & GM_FLAG_NO_COND_NODES);
@@ -475,10 +480,29 @@ extern "C" gm_status gm_set_bond_params(gm_system *s, int btype, float k, float 
 {
     if (!s) return GM_ERR_INVALID_ARG;
     if (btype < 0 || btype >= GM_MAX_BOND_TYPES) return fail(s, GM_ERR_INVALID_ARG, "gm_set_bond_params: bad bond type%s");
+    if (s->P.bond_style == GM_BOND_TABLE) return fail(s, GM_ERR_STATE, "gm_set_bond_params: tables are set with gm_set_bond_table%s");
     if (s->P.bond_style == GM_BOND_FENE && !(r0 > 0.f)) return fail(s, GM_ERR_INVALID_ARG, "gm_set_bond_params: FENE needs R0 > 0%s");
     s->P.bond_k[btype] = k;
     s->P.bond_r0[btype] = r0;
     s->P.bond_c[btype] = (r0 != 0.f) ? (float)(1.0 / ((double)r0 * (double)r0)) : 0.f;
+    s->force_current = false;
+    drop_graphs(s);
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_bond_table(gm_system *s, int btype, float interval, const float *c4)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    if (s->P.bond_style != GM_BOND_TABLE) return fail(s, GM_ERR_STATE, "gm_set_bond_table: bond_style is not GM_BOND_TABLE%s");
+    if (!c4 || btype < 0 || btype >= GM_MAX_BOND_TYPES || !(interval > 0.f))
+        return fail(s, GM_ERR_INVALID_ARG, "gm_set_bond_table: bad bond type, interval or NULL%s");
+    CU(cudaSetDevice(s->cfg.device));
+    const int np = s->P.bond_table_points;
+    CU(cudaMemcpyAsync(s->D.btable + (size_t)btype * np, c4, (size_t)np * 16, cudaMemcpyHostToDevice, s->st));
+    CU(cudaStreamSynchronize(s->st));              // the caller may reuse c4 at once
+    s->P.bond_k[btype] = (float)(1.0 / (double)interval);
+    s->P.bond_r0[btype] = interval;
+    s->P.bond_c[btype] = 0.f;
     s->force_current = false;
     drop_graphs(s);
     return GM_OK;

@@ -473,6 +473,14 @@ __device__ __forceinline__ void bond_loop(const GmParams &P, const GmDev &D, con
                 if (!(q > 0.0f)) { atomicOr(&D.ctl->err, GM_DEV_ERR_OVERSTRETCH); continue; }
                 fs = -kb * gm_rcp(q);
                 if (ENERGY) pe += -0.5f * kb * r0 * r0 * logf(q);
+            } else if (BOND == GM_BOND_TABLE) {
+                // Eqs. (11)-(12) in z = r^2: kb = 1 / interval, r0 = interval of this bond type
+                const int point = (int)(r2 * kb);
+                if (!(point < P.bond_table_points)) { atomicOr(&D.ctl->err, GM_DEV_ERR_OVERSTRETCH); continue; }
+                const float4 c = __ldg(P.btable + bt * P.bond_table_points + point);
+                const float d = r2 - (float)point * r0;
+                fs = -2.0f * (c.y + d * (2.0f * c.z + 3.0f * c.w * d));
+                if (ENERGY) pe += c.x + d * (c.y + d * (c.z + d * c.w));
             } else {
                 // Eq. (7): U = k (r - r0)^2;  F_i = -2 k (1 - r0/r) r_ij
                 if (r0 == 0.0f) {
@@ -946,6 +954,7 @@ static void launch_force_b(const GmParams &P, const GmDev &D, int mode, int pari
 {
     const int bond = (P.max_bonds > 0) ? P.bond_style : GM_BOND_NONE;
     if (bond == GM_BOND_FENE) launch_force_t<PAIR, NT1, GM_BOND_FENE>(P, D, mode, parity, kick, kick_vt, lagged, st);
+    else if (bond == GM_BOND_TABLE) launch_force_t<PAIR, NT1, GM_BOND_TABLE>(P, D, mode, parity, kick, kick_vt, lagged, st);
     else if (bond == GM_BOND_HARMONIC)
         launch_force_t<PAIR, NT1, GM_BOND_HARMONIC>(P, D, mode, parity, kick, kick_vt, lagged, st);
     else launch_force_t<PAIR, NT1, GM_BOND_NONE>(P, D, mode, parity, kick, kick_vt, lagged, st);

@@ -104,6 +104,10 @@ struct GmParams {
     int dih_n[GM_MAX_BOND_TYPES];
     const float4 *table;               // GM_PAIR_TABLE: (c0, c1, c2, c3) per grid point, n_types^2 tables of table_points
     int table_points;
+    // GM_BOND_TABLE: (c0, c1, c2, c3) per grid point of z = r^2, GM_MAX_BOND_TYPES tables of bond_table_points;
+    // bond_k[t] = 1 / interval, bond_r0[t] = interval of bond type t
+    const float4 *btable;
+    int bond_table_points;
 };
 
 // Device pointers.
@@ -114,6 +118,7 @@ struct GmDev {
     float4 *vt[2], *svt;
     float4 *frc;
     float4 *table;           // GM_PAIR_TABLE: spline coefficients, [n_types^2][table_points]
+    float4 *btable;          // GM_BOND_TABLE: spline coefficients, [GM_MAX_BOND_TYPES][bond_table_points]
     float4 *ftopo;           // angle + dihedral force (x, y, z) and energy share (w) of every bead, storage order
     int4 *at;                // angle table in TAG order: at[k * ns + tag] = (tag a, tag b, own position 0/1/2, type); x < 0: none
     int4 *dt;                // dihedral table in TAG order: dt[k * ns + tag] = (tag a, tag b, tag c, own position | type << 2)

@@ -128,6 +128,13 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
                     if (!(q > 0.0f)) { atomicOr(&D.ctl->err, GM_DEV_ERR_OVERSTRETCH); continue; }
                     fs = -kb / q;
                     pe_bond += -0.5f * kb * r0 * r0 * logf(q);
+                } else if (BOND == GM_BOND_TABLE) {
+                    const int point = (int)(r2 * kb);
+                    if (!(point < P.bond_table_points)) { atomicOr(&D.ctl->err, GM_DEV_ERR_OVERSTRETCH); continue; }
+                    const float4 cf = __ldg(P.btable + bt * P.bond_table_points + point);
+                    const float d = r2 - (float)point * r0;
+                    fs = -2.0f * (cf.y + d * (2.0f * cf.z + 3.0f * cf.w * d));
+                    pe_bond += cf.x + d * (cf.y + d * (cf.z + d * cf.w));
                 } else {
                     const float r = sqrtf(r2);
                     fs = (r0 == 0.0f) ? -2.0f * kb : ((r > 0.0f) ? -2.0f * kb * (1.0f - r0 / r) : 0.0f);
@@ -278,6 +285,7 @@ static void npt_force_b(const GmParams &P, const GmDev &D, int parity, int probe
     const int bond = (P.max_bonds > 0) ? P.bond_style : GM_BOND_NONE;
     if (bond == GM_BOND_FENE) npt_force_p<NT1, GM_BOND_FENE>(P, D, parity, probe, st);
     else if (bond == GM_BOND_HARMONIC) npt_force_p<NT1, GM_BOND_HARMONIC>(P, D, parity, probe, st);
+    else if (bond == GM_BOND_TABLE) npt_force_p<NT1, GM_BOND_TABLE>(P, D, parity, probe, st);
     else npt_force_p<NT1, GM_BOND_NONE>(P, D, parity, probe, st);
 }
 

@@ -20,7 +20,7 @@ GM_OK = 0
 GM_ERR_INVALID_ARG, GM_ERR_STATE, GM_ERR_CUDA, GM_ERR_WORKSPACE_TOO_SMALL = -1, -2, -3, -4
 GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_NONFINITE = -5, -6, -7, -8
 GM_PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
-GM_BOND = {"none": 0, "fene": 1, "harmonic": 2}
+GM_BOND = {"none": 0, "fene": 1, "harmonic": 2, "table": 3}
 GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5, "nph": 6, "npt": 7}
 GM_ANGLE = {"none": 0, "harmonic": 1, "cosine": 2}
 GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP, GM_FLAG_NO_WINDOWS = 1, 2, 4, 8
@@ -29,7 +29,7 @@ SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params"
            "gm_set_bond_params", "gm_set_angle_params", "gm_set_dihedral_params", "gm_set_angles", "gm_set_dihedrals",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
-           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box", "gm_kinetic_static",
+           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box", "gm_kinetic_static", "gm_set_bond_table",
            "gm_sfc_cell_order", "gm_last_error"]
 
 
@@ -45,6 +45,7 @@ class gm_config(C.Structure):
         ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
         ("table_points", C.c_int32), ("win_capacity", C.c_int32), ("tile_windows", C.c_int32),
         ("angle_style", C.c_int32), ("max_angles_per_particle", C.c_int32), ("max_dihedrals_per_particle", C.c_int32),
+        ("bond_table_points", C.c_int32),
     ]
 
 
@@ -73,6 +74,7 @@ def lib():
         L.gm_set_pair_table.argtypes = [vp, i32, i32, C.c_float, vp]
         L.gm_fit_pair_table.argtypes = [i32, C.c_double, vp, vp]
         L.gm_set_bond_params.argtypes = [vp, i32, C.c_float, C.c_float]
+        L.gm_set_bond_table.argtypes = [vp, i32, C.c_float, vp]
         L.gm_set_angle_params.argtypes = [vp, i32, C.c_float, C.c_float]
         L.gm_set_dihedral_params.argtypes = [vp, i32, C.c_float, i32, C.c_float]
         L.gm_set_angles.argtypes = [vp, i64, vp, vp]
@@ -164,6 +166,11 @@ def gm_fit_pair_table(v, interval: float) -> np.ndarray:
 
 def gm_set_bond_params(h, btype: int, k: float, r0: float):
     _check(lib().gm_set_bond_params(h, btype, k, r0), h)
+
+
+def gm_set_bond_table(h, btype: int, interval: float, c4):
+    c4 = np.ascontiguousarray(c4, dtype=np.float32)
+    _check(lib().gm_set_bond_table(h, btype, interval, c4.ctypes.data), h)
 
 
 def gm_set_angle_params(h, atype: int, k: float, theta0: float):
@@ -333,6 +340,8 @@ class System:
         cfg.seed = int(w.seed)
         cfg.pair_style = GM_PAIR[w.pair_style]
         cfg.bond_style = GM_BOND[w.bond_style] if cfg.max_bonds_per_particle else 0
+        if cfg.bond_style == GM_BOND["table"]:
+            cfg.bond_table_points = int(np.asarray(w.bond["table"]).shape[-2])
         cfg.integrator = GM_INTEG[w.integrator]
         cfg.kT, cfg.gamma, cfg.lam = float(w.kT), float(w.gamma), float(w.lam)
         cfg.sfc_period = int(w.sfc_period if sfc_period is None else sfc_period)
@@ -368,7 +377,12 @@ class System:
                                                         pair["rc"][ti][tj], 1.0 if pair.get("shift", True) else 0.0])
                 elif w.pair_style == "table":
                     gm_set_pair_table(self.h, ti, tj, float(pair["interval"]), pair["table"][ti][tj])
-        if cfg.bond_style:
+        if cfg.bond_style == GM_BOND["table"]:
+            tb = np.asarray(w.bond["table"], np.float32)
+            tb = tb.reshape(-1, tb.shape[-2], 4)
+            for bt in range(len(tb)):
+                gm_set_bond_table(self.h, bt, float(np.asarray(w.bond["interval"], np.float32).reshape(-1)[bt]), tb[bt])
+        elif cfg.bond_style:
             for bt in range(len(w.bond["k"])):
                 gm_set_bond_params(self.h, bt, float(w.bond["k"][bt]), float(w.bond["r0"][bt]))
         if len(ang):
