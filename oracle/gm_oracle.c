@@ -23,6 +23,8 @@
  *   - harmonic repulsion Eq. (2), Gaussian repulsion Eq. (3)
  *   - tabulated pair potential: cubic spline in z = r^2, Eq. (12); F = -2 r dV/dz, Eq. (11);
  *     cutoff = "point < Npoint", Alg. 2 lines 8-12
+ *   - tabulated angle and torsion potentials: Eq. (12) with x = theta on [0, pi] and x = phi on [-pi, pi]
+ *     (L118, L127: "x corresponds to z, theta, and phi")
  *   - tabulated bond potential: the same spline in z = r^2 per bond type (L118: "numerical non-bonded,
  *     bond ... potentials"); a bond past the end of its table is an error (reading c-32)
  *   - angle potentials Eqs. (8), (9) and the periodic dihedral Eq. (10), each interaction
@@ -45,6 +47,7 @@
  * temperatures.  Unpinned: equilibrium <Rg^2> of the melts in absolute terms ("parity unpinned";
  * compared GPU-vs-oracle only).
  */
+#define _GNU_SOURCE
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
@@ -108,6 +111,13 @@ typedef struct {
     const double *btable;
     int32_t btable_points;
     const double *btable_interval;      /* per bond type */
+    /* angle_style 3 / dtable_points > 0: "numerical ... angle, and torsion potentials", Eq. (12) with
+       x = theta on [0, pi] (interval pi / atable_points) and x = phi on [-pi, pi] (interval 2 pi / dtable_points,
+       grid point k at -pi + k interval); atable[(angle_type * atable_points + point) * 4 + {0..3}], dtable likewise.   */
+    const double *atable;
+    int32_t atable_points;
+    const double *dtable;
+    int32_t dtable_points;
 } orc_params;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -503,6 +513,17 @@ int orc_pair_bond_forces(const orc_params *p, const double *pos, const double *v
                 if (sn < 1e-12) sn = 1e-12;
                 pe_bond += kk * (th - t0) * (th - t0);
                 dudc = -2.0 * kk * (th - t0) / sn;
+            } else if (p->angle_style == 3) {
+                /* Eq. (12) with x = theta: point = int(theta / h), delta = theta - point h; dU/dcos = -U'(theta) / sin */
+                double th = acos(c), sn = sqrt(1.0 - c * c);
+                if (sn < 1e-12) sn = 1e-12;
+                double h = M_PI / p->atable_points;
+                long point = (long)(th / h);
+                if (point > p->atable_points - 1) point = p->atable_points - 1;
+                const double *cf = p->atable + ((size_t)p->angle_type[q] * p->atable_points + point) * 4;
+                double d = th - (double)point * h;
+                pe_bond += cf[0] + cf[1] * d + cf[2] * d * d + cf[3] * d * d * d;
+                dudc = -(cf[1] + 2.0 * cf[2] * d + 3.0 * cf[3] * d * d) / sn;
             } else {
                 /* Eq. (9): U = k (cos(theta) - cos(theta0))^2 */
                 double dc = c - cos(t0);
@@ -537,8 +558,21 @@ int orc_pair_bond_forces(const orc_params *p, const double *pos, const double *v
         double n2s = n2[0] * n2[0] + n2[1] * n2[1] + n2[2] * n2[2];
         if (n1s < 1e-24 || n2s < 1e-24) continue;     /* three beads in line: phi undefined, no force */
         double phi = atan2(l2 * (b1[0] * n2[0] + b1[1] * n2[1] + b1[2] * n2[2]), n1[0] * n2[0] + n1[1] * n2[1] + n1[2] * n2[2]);
-        pe_bond += kk * (1.0 + cos(nn * phi - dl));
-        double dudphi = -kk * nn * sin(nn * phi - dl);
+        double dudphi;
+        if (p->dtable_points > 0) {
+            /* Eq. (12) with x = phi: grid point k at -pi + k h, h = 2 pi / Npoint */
+            double h = 2.0 * M_PI / p->dtable_points, x = phi + M_PI;
+            long point = (long)(x / h);
+            if (point < 0) point = 0;
+            if (point > p->dtable_points - 1) point = p->dtable_points - 1;
+            const double *cf = p->dtable + ((size_t)p->dih_type[q] * p->dtable_points + point) * 4;
+            double d = x - (double)point * h;
+            pe_bond += cf[0] + cf[1] * d + cf[2] * d * d + cf[3] * d * d * d;
+            dudphi = cf[1] + 2.0 * cf[2] * d + 3.0 * cf[3] * d * d;
+        } else {
+            pe_bond += kk * (1.0 + cos(nn * phi - dl));
+            dudphi = -kk * nn * sin(nn * phi - dl);
+        }
         double s12 = (b1[0] * b2[0] + b1[1] * b2[1] + b1[2] * b2[2]) / (l2 * l2);
         double s32 = (b3[0] * b2[0] + b3[1] * b2[1] + b3[2] * b2[2]) / (l2 * l2);
         for (int d = 0; d < 3; ++d) {

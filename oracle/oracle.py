@@ -53,6 +53,7 @@ class _Params(C.Structure):
         ("dih_kk", C.c_void_p), ("dih_delta", C.c_void_p), ("dih_n", C.c_void_p),
         ("thermo", C.c_void_p), ("baro", C.c_void_p),
         ("btable", C.c_void_p), ("btable_points", C.c_int32), ("btable_interval", C.c_void_p),
+        ("atable", C.c_void_p), ("atable_points", C.c_int32), ("dtable", C.c_void_p), ("dtable_points", C.c_int32),
     ]
 
 
@@ -252,7 +253,7 @@ class Oracle:
         # angles / dihedrals (optional attributes of the workload: w.topo = dict(angle_style, angles (n,3), angle_type,
         # angle_k, angle_t0, dihedrals (n,4), dihedral_type, dihedral_k, dihedral_n, dihedral_delta))
         topo = getattr(w, "topo", None) or {}
-        ANG = {"none": 0, "harmonic": 1, "cosine": 2}
+        ANG = {"none": 0, "harmonic": 1, "cosine": 2, "table": 3}
         self._ang = np.ascontiguousarray(topo.get("angles", np.zeros((0, 3))), np.int32).reshape(-1, 3)
         self._ang_cols = [np.ascontiguousarray(self._ang[:, c]) for c in range(3)]
         self._ang_type = np.ascontiguousarray(topo.get("angle_type", np.zeros(len(self._ang))), np.int32)
@@ -273,6 +274,16 @@ class Oracle:
         P.dih_i, P.dih_j, P.dih_k, P.dih_l = (_p(c).value for c in self._dih_cols)
         P.dih_type = _p(self._dih_type).value
         P.dih_kk = _p(self._dih_k).value; P.dih_delta = _p(self._dih_delta).value; P.dih_n = _p(self._dih_n).value
+        # tabulated angle / torsion potentials: topo["angle_table"] (n_types, Npoint, 4) on theta in [0, pi] with
+        # angle_style "table"; topo["dihedral_table"] (n_types, Npoint, 4) on phi in [-pi, pi] replaces Eq. (10)
+        if P.angle_style == 3:
+            self._atable = np.ascontiguousarray(topo["angle_table"], np.float32).astype(np.float64)
+            self._atable = self._atable.reshape(-1, self._atable.shape[-2], 4)
+            P.atable = _p(self._atable).value; P.atable_points = int(self._atable.shape[1])
+        if len(self._dih) and topo.get("dihedral_table") is not None:
+            self._dtable = np.ascontiguousarray(topo["dihedral_table"], np.float32).astype(np.float64)
+            self._dtable = self._dtable.reshape(-1, self._dtable.shape[-2], 4)
+            P.dtable = _p(self._dtable).value; P.dtable_points = int(self._dtable.shape[1])
         self.thermo = np.zeros(4)       # [have half-step velocity, its kinetic energy, Nose-Hoover xi, -]
         P.thermo = _p(self.thermo).value
         # Andersen barostat (integrators "nph", "npt"): [P_ext, piston mass, piston momentum Pi, virial, virial valid]
