@@ -68,7 +68,8 @@ enum { GM_BOND_NONE = 0, GM_BOND_FENE = 1, GM_BOND_HARMONIC = 2, GM_BOND_TABLE =
 enum { GM_NVE = 0, GM_LANGEVIN = 1, GM_DPD_GWVV = 2,
        GM_NVT_NOSE_HOOVER = 3, GM_NVT_ANDERSEN = 4, GM_NVT_BERENDSEN = 5,     /* PAPER.md:L133, L137; DESIGN.md c-28..c-30 */
        GM_NPH_ANDERSEN = 6, GM_NPT_ANDERSEN = 7 };                            /* Andersen barostat; DESIGN.md c-31 */
-enum { GM_ANGLE_NONE = 0, GM_ANGLE_HARMONIC = 1 /* Eq. (8): k (theta - theta0)^2 */, GM_ANGLE_COSINE = 2 /* Eq. (9): k (cos theta - cos theta0)^2 */ };
+enum { GM_ANGLE_NONE = 0, GM_ANGLE_HARMONIC = 1 /* Eq. (8): k (theta - theta0)^2 */, GM_ANGLE_COSINE = 2 /* Eq. (9): k (cos theta - cos theta0)^2 */,
+       GM_ANGLE_TABLE = 3 /* Eq. (12) with x = theta */ };
 
 #define GM_MAX_TYPES 8       /* particle types; pair tables are n_types x n_types */
 #define GM_MAX_BOND_TYPES 8
@@ -107,6 +108,8 @@ typedef struct {
     int32_t max_angles_per_particle; /* rows of the per-particle angle table; 0 = no angles              */
     int32_t max_dihedrals_per_particle; /* rows of the per-particle dihedral table; 0 = no dihedrals (Eq. (10))         */
     int32_t bond_table_points;       /* GM_BOND_TABLE: grid points of every bond table; else 0                          */
+    int32_t angle_table_points;      /* GM_ANGLE_TABLE: grid intervals of every angle table on [0, pi]; else 0           */
+    int32_t dihedral_table_points;   /* > 0: dihedrals are tabulated on [-pi, pi] with this many intervals (instead of Eq. (10)) */
 } gm_config;
 
 enum {
@@ -190,6 +193,15 @@ gm_status gm_set_angle_params(gm_system *s, int atype, float k, float theta0);
 /* Dihedral parameters of dihedral type `dtype`: Eq. (10) U = k [1 + cos(n phi - delta)]; phi = 0 for
  * cis, pi for trans (DESIGN.md c-27). */
 gm_status gm_set_dihedral_params(gm_system *s, int dtype, float k, int n, float delta);
+
+/* Tabulated angle and torsion potentials ("numerical ... angle, and torsion potentials"; L127: Eq. (12) with
+ * "x corresponds to z, theta, and phi"): c4 is a HOST array of 4 * Npoint floats, V(x_k + d) = c0 + c1 d + c2 d^2 + c3 d^3.
+ * Angles (cfg.angle_style = GM_ANGLE_TABLE, Npoint = cfg.angle_table_points): x = theta, x_k = k pi / Npoint.
+ * Dihedrals (cfg.dihedral_table_points = Npoint > 0): x = phi, x_k = -pi + 2 pi k / Npoint; the tables cover the whole range
+ * of the variable, so there is no cutoff.  Conventions for theta and phi as above.  gm_fit_pair_table fits such a table (natural
+ * ends) through Npoint + 1 values on the grid.  Copies c4 in (synchronises).  Errors: STATE, INVALID_ARG. */
+gm_status gm_set_angle_table(gm_system *s, int atype, const float *c4);
+gm_status gm_set_dihedral_table(gm_system *s, int dtype, const float *c4);
 
 /* Angles as n_angles tag triples (i, j, k), j the middle bead, + a type each (NULL = all 0); dihedrals as tag
  * quadruples (i, j, k, l).  Each is entered in the per-particle table of EVERY member together with the member's

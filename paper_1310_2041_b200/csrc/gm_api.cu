@@ -70,7 +70,10 @@ static gm_status derive(const gm_config *c, GmParams *P)
     for (int d = 0; d < 3; ++d) if (!(c->box[d] > 0.f)) return GM_ERR_INVALID_ARG;
     if (c->x_cell_div < 0 || c->x_cell_div > 8 || (c->nl_scan_trip != 0 && c->nl_scan_trip != 4 && c->nl_scan_trip != 8) ||
         c->step_shape < 0 || c->step_shape > 2 || c->win_capacity < 0 || c->win_capacity > 8000 || c->tile_windows < 0 || c->tile_windows > 2 ||
-        c->angle_style < GM_ANGLE_NONE || c->angle_style > GM_ANGLE_COSINE || c->max_angles_per_particle < 0 ||
+        c->angle_style < GM_ANGLE_NONE || c->angle_style > GM_ANGLE_TABLE || c->max_angles_per_particle < 0 ||
+        c->angle_table_points < 0 || c->angle_table_points > (1 << 20) || ((c->angle_style == GM_ANGLE_TABLE) != (c->angle_table_points > 0)) ||
+        c->dihedral_table_points < 0 || c->dihedral_table_points > (1 << 20) ||
+        (c->dihedral_table_points > 0 && c->max_dihedrals_per_particle == 0) ||
         c->max_angles_per_particle > 64 || c->max_dihedrals_per_particle < 0 || c->max_dihedrals_per_particle > 64 ||
         (c->max_angles_per_particle > 0 && c->angle_style == GM_ANGLE_NONE))
         return GM_ERR_INVALID_ARG;
@@ -170,6 +173,7 @@ static gm_status derive(const gm_config *c, GmParams *P)
     if (!gm_nl_capacity_ok(*P)) return GM_ERR_INVALID_ARG;
     P->table_points = c->table_points;      // (memset above: every pair coefficient starts at 0 = no interaction)
     P->bond_table_points = c->bond_table_points;
+    P->angle_table_points = c->angle_table_points; P->dihedral_table_points = c->dihedral_table_points;
     return GM_OK;
 }
 
@@ -195,6 +199,8 @@ static size_t carve(const GmParams &P, const gm_config &c, char *base, GmDev *D)
     d.frc = (float4 *)take(n * 16);
     if (P.table_points > 0) d.table = (float4 *)take((size_t)P.n_types * P.n_types * P.table_points * 16);
     if (P.bond_table_points > 0) d.btable = (float4 *)take((size_t)GM_MAX_BOND_TYPES * P.bond_table_points * 16);
+    if (P.angle_table_points > 0) d.atable = (float4 *)take((size_t)GM_MAX_BOND_TYPES * P.angle_table_points * 16);
+    if (P.dihedral_table_points > 0) d.dtable = (float4 *)take((size_t)GM_MAX_BOND_TYPES * P.dihedral_table_points * 16);
     if (P.max_angles + P.max_dihedrals > 0) d.ftopo = (float4 *)take(n * 16);
     if (P.max_angles > 0) d.at = (int4 *)take(n * 16 * (size_t)P.max_angles);
     if (P.max_dihedrals > 0) d.dt = (int4 *)take(n * 16 * (size_t)P.max_dihedrals);
@@ -312,6 +318,7 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     carve(P, *cfg, (char *)dev_workspace, &s->D);
     s->P.table = s->D.table;
     s->P.btable = s->D.btable;
+    s->P.atable = s->D.atable; s->P.dtable = s->D.dtable;
     s->st = (cudaStream_t)cfg->stream;
     s->use_graph = !(cfg->flags & GM_FLAG_NO_GRAPH);
     s->use_cond = !(cfg->flags & GM_FLAG_NO_COND_NODES);
@@ -526,6 +533,29 @@ extern "C" gm_status gm_set_dihedral_params(gm_system *s, int dtype, float k, in
     s->force_current = false;
     drop_graphs(s);
     return GM_OK;
+}
+
+static gm_status set_topo_table(gm_system *s, int type, const float *c4, float4 *dst, int np, const char *who)
+{
+    if (np <= 0) return fail(s, GM_ERR_STATE, "%s: the system was not created with such tables", who);
+    if (!c4 || type < 0 || type >= GM_MAX_BOND_TYPES) return fail(s, GM_ERR_INVALID_ARG, "%s: bad type or NULL", who);
+    CU(cudaSetDevice(s->cfg.device));
+    CU(cudaMemcpyAsync(dst + (size_t)type * np, c4, (size_t)np * 16, cudaMemcpyHostToDevice, s->st));
+    CU(cudaStreamSynchronize(s->st));              // the caller may reuse c4 at once
+    s->force_current = false;
+    return GM_OK;
+}
+
+extern "C" gm_status gm_set_angle_table(gm_system *s, int atype, const float *c4)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    return set_topo_table(s, atype, c4, s->D.atable, s->P.angle_table_points, "gm_set_angle_table");
+}
+
+extern "C" gm_status gm_set_dihedral_table(gm_system *s, int dtype, const float *c4)
+{
+    if (!s) return GM_ERR_INVALID_ARG;
+    return set_topo_table(s, dtype, c4, s->D.dtable, s->P.dihedral_table_points, "gm_set_dihedral_table");
 }
 
 // Per-particle angle / dihedral tables: every interaction under every member, with the member's

@@ -108,6 +108,9 @@ struct GmParams {
     // bond_k[t] = 1 / interval, bond_r0[t] = interval of bond type t
     const float4 *btable;
     int bond_table_points;
+    // GM_ANGLE_TABLE / tabulated dihedrals: (c0..c3) per grid interval of theta in [0, pi] / phi in [-pi, pi]
+    const float4 *atable, *dtable;
+    int angle_table_points, dihedral_table_points;
 };
 
 // Device pointers.
@@ -119,6 +122,7 @@ struct GmDev {
     float4 *frc;
     float4 *table;           // GM_PAIR_TABLE: spline coefficients, [n_types^2][table_points]
     float4 *btable;          // GM_BOND_TABLE: spline coefficients, [GM_MAX_BOND_TYPES][bond_table_points]
+    float4 *atable, *dtable; // tabulated angle / dihedral potentials, [GM_MAX_BOND_TYPES][points]
     float4 *ftopo;           // angle + dihedral force (x, y, z) and energy share (w) of every bead, storage order
     int4 *at;                // angle table in TAG order: at[k * ns + tag] = (tag a, tag b, own position 0/1/2, type); x < 0: none
     int4 *dt;                // dihedral table in TAG order: dt[k * ns + tag] = (tag a, tag b, tag c, own position | type << 2)

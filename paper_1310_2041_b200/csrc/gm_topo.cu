@@ -58,6 +58,17 @@ k_topo(const __grid_constant__ GmParams P, GmDev D, int parity)
             const float d = th - P.angle_t0[e.w];
             pe += kk * d * d * (1.0f / 3.0f);
             dudc = -2.0f * kk * d / sn;
+        } else if (P.angle_style == GM_ANGLE_TABLE) {     // Eq. (12) with x = theta
+            const float3 x = cross3(a, b);
+            const float sn = fmaxf(sqrtf(dot3(x, x)) * ia * ib, 1e-12f);
+            const float th = atan2f(sn, c);
+            const int np = P.angle_table_points;
+            const float h = 3.14159265358979323846f / (float)np;
+            const int point = min((int)(th / h), np - 1);
+            const float4 cf = __ldg(P.atable + e.w * np + point);
+            const float d = th - (float)point * h;
+            pe += (cf.x + d * (cf.y + d * (cf.z + d * cf.w))) * (1.0f / 3.0f);
+            dudc = -(cf.y + d * (2.0f * cf.z + 3.0f * cf.w * d)) / sn;
         } else {                                          // Eq. (9)
             const float d = c - P.angle_c0[e.w];
             pe += kk * d * d * (1.0f / 3.0f);
@@ -88,11 +99,23 @@ k_topo(const __grid_constant__ GmParams P, GmDev D, int parity)
         if (n1s < 1e-20f || n2s < 1e-20f) continue;       // three beads in line: phi undefined, no force
         const float l2 = sqrtf(b2s);
         const float phi = atan2f(l2 * dot3(b1, n2), dot3(n1, n2));
-        const float arg = (float)P.dih_n[ty] * phi - P.dih_delta[ty];
-        float sn, cs;
-        sincosf(arg, &sn, &cs);
-        pe += P.dih_k[ty] * (1.0f + cs) * 0.25f;
-        const float dudphi = -P.dih_k[ty] * (float)P.dih_n[ty] * sn;
+        float dudphi;
+        if (P.dihedral_table_points > 0) {                // Eq. (12) with x = phi, grid point k at -pi + k h
+            const int np = P.dihedral_table_points;
+            const float h = 6.28318530717958647692f / (float)np;
+            const float x = phi + 3.14159265358979323846f;
+            const int point = min(max((int)(x / h), 0), np - 1);
+            const float4 cf = __ldg(P.dtable + ty * np + point);
+            const float d = x - (float)point * h;
+            pe += (cf.x + d * (cf.y + d * (cf.z + d * cf.w))) * 0.25f;
+            dudphi = cf.y + d * (2.0f * cf.z + 3.0f * cf.w * d);
+        } else {
+            const float arg = (float)P.dih_n[ty] * phi - P.dih_delta[ty];
+            float sn, cs;
+            sincosf(arg, &sn, &cs);
+            pe += P.dih_k[ty] * (1.0f + cs) * 0.25f;
+            dudphi = -P.dih_k[ty] * (float)P.dih_n[ty] * sn;
+        }
         const float wi = -l2 / n1s, wl = l2 / n2s;        // d phi / d r_i = wi n1,  d phi / d r_l = wl n2
         const float s12 = dot3(b1, b2) / b2s, s32 = dot3(b3, b2) / b2s;
         float ci, cl;                                     // d phi / d r_own = ci wi n1 + cl wl n2

@@ -22,14 +22,14 @@ GM_ERR_BOX_TOO_SMALL, GM_ERR_NEIGHBOR_OVERFLOW, GM_ERR_BOND_OVERSTRETCH, GM_ERR_
 GM_PAIR = {"none": 0, "lj": 1, "dpd": 2, "harmonic": 3, "gauss": 4, "table": 5}
 GM_BOND = {"none": 0, "fene": 1, "harmonic": 2, "table": 3}
 GM_INTEG = {"nve": 0, "langevin": 1, "gwvv": 2, "nose_hoover": 3, "andersen": 4, "berendsen": 5, "nph": 6, "npt": 7}
-GM_ANGLE = {"none": 0, "harmonic": 1, "cosine": 2}
+GM_ANGLE = {"none": 0, "harmonic": 1, "cosine": 2, "table": 3}
 GM_FLAG_NO_GRAPH, GM_FLAG_NO_COND_NODES, GM_FLAG_STEP_SUBWARP, GM_FLAG_NO_WINDOWS = 1, 2, 4, 8
 
 SYMBOLS = ["gm_query_workspace", "gm_create", "gm_destroy", "gm_set_pair_params", "gm_set_pair_table", "gm_fit_pair_table",
            "gm_set_bond_params", "gm_set_angle_params", "gm_set_dihedral_params", "gm_set_angles", "gm_set_dihedrals",
            "gm_set_particles", "gm_set_bonds", "gm_set_step", "gm_build_neighbors", "gm_compute_forces",
            "gm_step", "gm_step_timed", "gm_set_integrator", "gm_energies", "gm_get_particles", "gm_get_neighbors", "gm_get_stats",
-           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box", "gm_kinetic_static", "gm_set_bond_table",
+           "gm_get_tuning", "gm_set_barostat", "gm_set_box_state", "gm_get_box", "gm_kinetic_static", "gm_set_bond_table", "gm_set_angle_table", "gm_set_dihedral_table",
            "gm_sfc_cell_order", "gm_last_error"]
 
 
@@ -45,7 +45,7 @@ class gm_config(C.Structure):
         ("x_cell_div", C.c_int32), ("nl_scan_trip", C.c_int32), ("step_shape", C.c_int32),
         ("table_points", C.c_int32), ("win_capacity", C.c_int32), ("tile_windows", C.c_int32),
         ("angle_style", C.c_int32), ("max_angles_per_particle", C.c_int32), ("max_dihedrals_per_particle", C.c_int32),
-        ("bond_table_points", C.c_int32),
+        ("bond_table_points", C.c_int32), ("angle_table_points", C.c_int32), ("dihedral_table_points", C.c_int32),
     ]
 
 
@@ -75,6 +75,8 @@ def lib():
         L.gm_fit_pair_table.argtypes = [i32, C.c_double, vp, vp]
         L.gm_set_bond_params.argtypes = [vp, i32, C.c_float, C.c_float]
         L.gm_set_bond_table.argtypes = [vp, i32, C.c_float, vp]
+        L.gm_set_angle_table.argtypes = [vp, i32, vp]
+        L.gm_set_dihedral_table.argtypes = [vp, i32, vp]
         L.gm_set_angle_params.argtypes = [vp, i32, C.c_float, C.c_float]
         L.gm_set_dihedral_params.argtypes = [vp, i32, C.c_float, i32, C.c_float]
         L.gm_set_angles.argtypes = [vp, i64, vp, vp]
@@ -171,6 +173,16 @@ def gm_set_bond_params(h, btype: int, k: float, r0: float):
 def gm_set_bond_table(h, btype: int, interval: float, c4):
     c4 = np.ascontiguousarray(c4, dtype=np.float32)
     _check(lib().gm_set_bond_table(h, btype, interval, c4.ctypes.data), h)
+
+
+def gm_set_angle_table(h, atype: int, c4):
+    c4 = np.ascontiguousarray(c4, dtype=np.float32)
+    _check(lib().gm_set_angle_table(h, atype, c4.ctypes.data), h)
+
+
+def gm_set_dihedral_table(h, dtype: int, c4):
+    c4 = np.ascontiguousarray(c4, dtype=np.float32)
+    _check(lib().gm_set_dihedral_table(h, dtype, c4.ctypes.data), h)
 
 
 def gm_set_angle_params(h, atype: int, k: float, theta0: float):
@@ -353,8 +365,12 @@ class System:
         if len(ang):
             cfg.angle_style = GM_ANGLE[topo.get("angle_style", "harmonic")]
             cfg.max_angles_per_particle = int(np.bincount(ang.ravel(), minlength=self.n).max())
+            if cfg.angle_style == GM_ANGLE["table"]:
+                cfg.angle_table_points = int(np.asarray(topo["angle_table"]).shape[-2])
         if len(dih):
             cfg.max_dihedrals_per_particle = int(np.bincount(dih.ravel(), minlength=self.n).max())
+            if topo.get("dihedral_table") is not None:
+                cfg.dihedral_table_points = int(np.asarray(topo["dihedral_table"]).shape[-2])
         for k, v in (tune or {}).items():       # gm_config tuning overrides: x_cell_div, nl_scan_trip, step_shape
             setattr(cfg, k, int(v))
         self.cfg = cfg
@@ -386,12 +402,22 @@ class System:
             for bt in range(len(w.bond["k"])):
                 gm_set_bond_params(self.h, bt, float(w.bond["k"][bt]), float(w.bond["r0"][bt]))
         if len(ang):
-            for at, (k, t0) in enumerate(zip(topo["angle_k"], topo["angle_t0"])):
-                gm_set_angle_params(self.h, at, float(np.float32(k)), float(np.float32(t0)))
+            if cfg.angle_table_points:
+                tb = np.asarray(topo["angle_table"], np.float32)
+                for at, t4 in enumerate(tb.reshape(-1, tb.shape[-2], 4)):
+                    gm_set_angle_table(self.h, at, t4)
+            else:
+                for at, (k, t0) in enumerate(zip(topo["angle_k"], topo["angle_t0"])):
+                    gm_set_angle_params(self.h, at, float(np.float32(k)), float(np.float32(t0)))
             gm_set_angles(self.h, ang, topo.get("angle_type"))
         if len(dih):
-            for dt_, (k, nn, dl) in enumerate(zip(topo["dihedral_k"], topo["dihedral_n"], topo["dihedral_delta"])):
-                gm_set_dihedral_params(self.h, dt_, float(np.float32(k)), int(nn), float(np.float32(dl)))
+            if cfg.dihedral_table_points:
+                tb = np.asarray(topo["dihedral_table"], np.float32)
+                for dt_, t4 in enumerate(tb.reshape(-1, tb.shape[-2], 4)):
+                    gm_set_dihedral_table(self.h, dt_, t4)
+            else:
+                for dt_, (k, nn, dl) in enumerate(zip(topo["dihedral_k"], topo["dihedral_n"], topo["dihedral_delta"])):
+                    gm_set_dihedral_params(self.h, dt_, float(np.float32(k)), int(nn), float(np.float32(dl)))
             gm_set_dihedrals(self.h, dih, topo.get("dihedral_type"))
         if w.integrator in ("nph", "npt"):
             gm_set_barostat(self.h, float(np.float32(getattr(w, "p_ext", 0.0))), float(np.float32(getattr(w, "piston_mass", 1.0))))

@@ -78,3 +78,28 @@ def test_angles_and_dihedrals_trajectory_c3_scaled(gm):
     # ill-conditioned (an fp32 and an fp64 trajectory part within a few steps whatever the code): the 10-step gate is
     # taken from the state after 60 steps, when the angle terms have bent the chains
     trajectory_after(gm, w, 60)
+
+
+# ---- tabulated angle and torsion potentials (Eq. (12) with x = theta, phi) -----------------------
+def test_tabulated_angles_and_dihedrals_forces_and_trajectory(gm):
+    from tests.test_oracle_pins_topotable import melt_with_tables
+    w, wt = melt_with_tables(n_point=2000)                 # C1 scaled by 0.5 with Eq. (8) / Eq. (10) given as tables
+    forces_parity(gm, wt, steps_before=25)
+    trajectory_parity(gm, wt, n_steps=10)
+    # against the analytic kernels on the same state: spline error of 2 000 intervals + fp32
+    a, b = gm.System(w), gm.System(wt)
+    a.step(25); b.step(25)
+    fa = a.get_particles(False, False, True)[2]
+    fb = b.get_particles(False, False, True)[2]
+    frms = np.sqrt((fa.astype(np.float64) ** 2).sum(axis=1).mean())
+    assert np.abs(fa - fb).max() <= 5e-3 * frms            # two fp32 trajectories of 25 steps apart + the spline
+    ea, eb = a.energies(), b.energies()
+    assert eb["pe_bond"] == pytest.approx(ea["pe_bond"], rel=1e-4)
+    a.close(); b.close()
+    # configuration errors
+    c = gm.System(w)
+    with pytest.raises(gm.GmError):
+        gm.gm_set_angle_table(c.h, 0, np.zeros((16, 4), np.float32))
+    with pytest.raises(gm.GmError):
+        gm.gm_set_dihedral_table(c.h, 0, np.zeros((16, 4), np.float32))
+    c.close()
