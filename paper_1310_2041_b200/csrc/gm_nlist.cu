@@ -15,18 +15,22 @@
 // [NL_STAGE][32]: conflict-free and private to the lane, so no synchronisation); candidates are scanned
 // four at a time, and after each four every lane that holds 16 or more staged entries writes four whole
 // int4 quads of its NL row (gm_internal.cuh: entries 4q..4q+3 of a bead are one int4; the 32 int4 of a
-// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 10 KB (four candidates per
-// trip: ring of 16, flushed by halves) or 20 KB (eight: ring of 32) per CTA whatever the row capacity, which leaves
-// the rest of the SM's 228 KB to L1 for the candidate loads.
+// quad are contiguous, so a warp stores 512-byte lines).  The ring keeps shared memory at 20 KB per CTA
+// whatever the row capacity (window systems add their set-up scratch and, for dense cells, the union scan's buffers),
+// which leaves the rest of the SM's 228 KB to L1 for the candidate loads.
 #include "gm_internal.cuh"
 
 #ifndef NL_MINB_WIN
 #define NL_MINB_WIN 6          // resident CTAs per SM the window-system build is compiled for (77 registers, no spills; 8 -> 64 registers with spills measured 1 % slower on C2 / C5)
 #endif
 #define NL_STAGE 32          // ring entries per lane of the kernels that scan 8 candidates per trip (power of two)
-// ring entries per lane by trip width: a lane flushes half a ring when that much is staged, so the ring must hold
-// (half - 1) + TRIP entries: 16 for TRIP = 4 (8 KB per CTA), 32 for TRIP = 8
-#define NL_STAGE_OF(TRIP) ((TRIP) == 4 ? 16 : 32)
+// Ring entries per lane by trip width: a lane flushes half a ring when that much is staged, so the ring must hold
+// (half - 1) + TRIP entries.  A ring of 16 would do for TRIP = 4 (8 KB per CTA instead of 16), but it flushes twice as
+// often: measured on C3 70.35 against 69.87 us per timestep with the ring of 32 (same box) -- 32 for both.
+#ifndef NL_STAGE4
+#define NL_STAGE4 32
+#endif
+#define NL_STAGE_OF(TRIP) ((TRIP) == 4 ? NL_STAGE4 : 32)
 #ifndef NL_COOP
 #define NL_COOP 1            // dense cells: warps of one piece scan the union of their lanes' runs together (nl_scan_warp)
 #endif
