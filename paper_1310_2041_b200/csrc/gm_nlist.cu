@@ -468,7 +468,7 @@ k_nl_build(const __grid_constant__ GmParams P, GmDev D)
     if (WINS && (int)(blockIdx.x * blockDim.x) < P.n)           // CTA-uniform: the tile holds at least one bead
         mode = nl_window(P, D, blockIdx.x, valid, cx, cy, cz, rng, cell, sh_mode, &W.group);
     bool scanned = false;
-    if (TRIP == 8 && WINS && NL_COOP) {      // measured: C5 1 928 -> 1 899 us per timestep; the DPD melt C4 (no windows, 9 CTAs per SM) lost 1.7 % and keeps the per-lane scan
+    if (TRIP == 8 && WINS && NL_COOP) {      // measured: C5 1 928 -> 1 899 us per timestep; the DPD melt C4 (no windows) lost 1.7 % at 7 CTAs per SM and 0.4 % at 9, and keeps the per-lane scan
         const unsigned full = 0xffffffffu;
         const int cy0 = __shfl_sync(full, cy, 0), cz0 = __shfl_sync(full, cz, 0);
         const bool inner = valid && cx >= P.sx && cx + P.sx <= P.nc[0] - 1 && cy > 0 && cy < P.nc[1] - 1 && cz > 0 && cz < P.nc[2] - 1;

@@ -5,6 +5,10 @@
 #include "gm_force_impl.cuh"
 
 #define NPT_BLOCK 128
+#ifndef NPT_FBLOCK
+#define NPT_FBLOCK 32            // threads per CTA of the force kernel (no block-level step in it): one-warp CTAs, 32 per SM,
+#define NPT_FMINB 32             // as the short-list step kernel (measured on C3: 103.1 us per timestep; 64 x 16 and 128 x 8 the same)
+#endif
 
 // sum of v[0..NQ) over the warp -> one of the GM_NPT_SLOTS copies of the sums (lane q adds quantity q: one double atomic
 // per warp and quantity, spread over 64 x NQ addresses; no block barrier, a warp leaves when it is done)
@@ -86,7 +90,7 @@ __device__ __forceinline__ void npt_pairs(const GmParams &P, const GmDev &D, con
 // Forces at the real distances lambda * s (Eq. 1 pairs from the neighbor list, bonds from BL), the virial and the sums
 // the piston needs.  D.frc[i] = (F, the bead's half share of the potential energy).
 template <bool NT1, int BOND, bool PAIRS>
-__global__ void __launch_bounds__(NPT_BLOCK)
+__global__ void __launch_bounds__(NPT_FBLOCK, NPT_FMINB)
 k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
 {
     GmNpt *N = gm_npt_state(D);
@@ -94,7 +98,7 @@ k_npt_force(const __grid_constant__ GmParams P, GmDev D, int parity, int probe)
     const Src S = current_src(D, parity, step);
     const float lam = (float)N->lam[parity];
     const float lam2 = lam * lam;
-    const int i = blockIdx.x * NPT_BLOCK + threadIdx.x;
+    const int i = blockIdx.x * NPT_FBLOCK + threadIdx.x;
     double acc[6] = { 0.0, 0.0, 0.0, 0.0, 0.0, 0.0 };
     if (i < P.n) {
         // every stream of the bead is requested before anything is used
@@ -274,9 +278,9 @@ void gm_launch_npt_init(const GmDev &D, int parity, double vol0, double V, doubl
 template <bool NT1, int BOND>
 static void npt_force_p(const GmParams &P, const GmDev &D, int parity, int probe, cudaStream_t st)
 {
-    const int nb = (P.n + NPT_BLOCK - 1) / NPT_BLOCK;
-    if (P.pair_style == GM_PAIR_LJ) k_npt_force<NT1, BOND, true><<<nb, NPT_BLOCK, 0, st>>>(P, D, parity, probe);
-    else k_npt_force<NT1, BOND, false><<<nb, NPT_BLOCK, 0, st>>>(P, D, parity, probe);
+    const int nb = (P.n + NPT_FBLOCK - 1) / NPT_FBLOCK;
+    if (P.pair_style == GM_PAIR_LJ) k_npt_force<NT1, BOND, true><<<nb, NPT_FBLOCK, 0, st>>>(P, D, parity, probe);
+    else k_npt_force<NT1, BOND, false><<<nb, NPT_FBLOCK, 0, st>>>(P, D, parity, probe);
 }
 
 template <bool NT1>
