@@ -78,3 +78,25 @@ def test_sizes_beyond_the_static_array_are_rejected(gm):
     assert r == gm.GM_ERR_INVALID_ARG and b"exceeds the static scratch array" in buf.value and b"8388608" in buf.value
     r = gm.lib().gm_kinetic_static(None, None, 8, 0, None, out.data_ptr(), buf, 256)
     assert r == gm.GM_ERR_INVALID_ARG
+
+
+def test_capturable_in_a_cuda_graph(gm):
+    # the use case the entry point exists for: one memset node + one kernel node, no allocation while capturing
+    import torch
+    w = make_config("C1")
+    vel = torch.from_numpy(w.vel).cuda()
+    out = torch.zeros(4, dtype=torch.float64, device="cuda")
+    gm.gm_kinetic_static(vel, None, out)                    # outside the capture: resolves the array's address on this device
+    torch.cuda.synchronize()
+    expect = out.clone()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        gm.gm_kinetic_static(vel, None, out)
+    for scale in (2.0, 3.0):
+        vel.mul_(scale)
+        expect = expect * torch.tensor([scale * scale, scale, scale, scale], dtype=torch.float64, device="cuda")
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert out[0].item() == pytest.approx(expect[0].item(), rel=1e-6)
+        assert torch.allclose(out[1:], expect[1:], rtol=0, atol=1e-6 * float(np.abs(w.vel).sum()) * 6)
