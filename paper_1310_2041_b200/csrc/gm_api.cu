@@ -12,7 +12,11 @@
 #include "gm_internal.cuh"
 #include "gm_npt.cuh"
 
-#define GM_GRAPH_STEPS 16   // steps per big graph launch (even)
+// Timesteps per graph launch (even): a launch costs ~7 us of device time (the one gate kernel of its first timestep and the
+// gap to the next graph), so long runs go in graphs of 64 (measured against 16: C3 70.18 -> 69.85, C1 17.75 -> 17.33 us per
+// timestep), what is left in graphs of 16, then of 2
+#define GM_GRAPH_STEPS 64
+#define GM_GRAPH_STEPS_MID 16
 
 struct gm_system {
     gm_config cfg;
@@ -23,7 +27,7 @@ struct gm_system {
     bool have_particles, lagged, nl_valid, force_current, bonds_dirty, pair_set_any;
     uint64_t step;
     bool use_graph, use_cond;
-    cudaGraphExec_t exec_big, exec_two;
+    cudaGraphExec_t exec_big, exec_mid, exec_two;
     // Andersen barostat (gm_npt.cuh): host copies of what gm_set_barostat / gm_set_box_state last set
     double npt_vol0, npt_V, npt_Pi, npt_p_ext, npt_mass;
     char err[512];
@@ -298,6 +302,7 @@ extern "C" gm_status gm_query_workspace(const gm_config *cfg, size_t *bytes)
 static void drop_graphs(gm_system *s)
 {
     if (s->exec_big) { cudaGraphExecDestroy(s->exec_big); s->exec_big = nullptr; }
+    if (s->exec_mid) { cudaGraphExecDestroy(s->exec_mid); s->exec_mid = nullptr; }
     if (s->exec_two) { cudaGraphExecDestroy(s->exec_two); s->exec_two = nullptr; }
 }
 
@@ -874,9 +879,8 @@ static gm_status step_impl(gm_system *s, int64_t n_steps, StepTiming *tm)
     while (done < n_steps) {
         const int64_t rem = n_steps - done;
         if (!tm && s->use_graph && s->lagged && s->cur == 0 && rem >= 2) {
-            const bool big = rem >= GM_GRAPH_STEPS;
-            cudaGraphExec_t *slot = big ? &s->exec_big : &s->exec_two;
-            const int ns = big ? GM_GRAPH_STEPS : 2;
+            cudaGraphExec_t *slot = rem >= GM_GRAPH_STEPS ? &s->exec_big : (rem >= GM_GRAPH_STEPS_MID ? &s->exec_mid : &s->exec_two);
+            const int ns = rem >= GM_GRAPH_STEPS ? GM_GRAPH_STEPS : (rem >= GM_GRAPH_STEPS_MID ? GM_GRAPH_STEPS_MID : 2);
             gm_status r = get_graph(s, ns, slot);
             if (r != GM_OK) return r;
             CU(cudaGraphLaunch(*slot, s->st));
