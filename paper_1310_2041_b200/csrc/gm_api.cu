@@ -23,6 +23,7 @@ struct gm_system {
     GmParams P;
     GmDev D;
     cudaStream_t st, cap_st, cap_st2;
+    GmFork fk;                     // side branch of the rebuild (gm_launch_nl_build)
     int cur;                       // which pos/vt buffer holds the current time level
     bool have_particles, lagged, nl_valid, force_current, bonds_dirty, pair_set_any;
     uint64_t step;
@@ -331,6 +332,9 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     cudaError_t e = cudaSetDevice(cfg->device);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->cap_st2, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s->fk.side, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->fk.fork, cudaEventDisableTiming);
+    if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->fk.join, cudaEventDisableTiming);
     if (e == cudaSuccess) e = gm_nl_prepare(P);
     if (e == cudaSuccess) {
         std::vector<uint32_t> rr;
@@ -360,6 +364,9 @@ extern "C" gm_status gm_create(const gm_config *cfg, void *dev_workspace, size_t
     if (e != cudaSuccess) {
         if (s->cap_st) cudaStreamDestroy(s->cap_st);
         if (s->cap_st2) cudaStreamDestroy(s->cap_st2);
+        if (s->fk.side) cudaStreamDestroy(s->fk.side);
+        if (s->fk.fork) cudaEventDestroy(s->fk.fork);
+        if (s->fk.join) cudaEventDestroy(s->fk.join);
         delete s;
         return GM_ERR_CUDA;
     }
@@ -376,6 +383,9 @@ extern "C" gm_status gm_destroy(gm_system *s)
     drop_graphs(s);
     cudaStreamDestroy(s->cap_st);
     cudaStreamDestroy(s->cap_st2);
+    cudaStreamDestroy(s->fk.side);
+    cudaEventDestroy(s->fk.fork);
+    cudaEventDestroy(s->fk.join);
     delete s;
     return GM_OK;
 }
@@ -719,7 +729,7 @@ static void enqueue_rebuild(gm_system *s, int gate, cudaStream_t st)
 {
     gm_launch_gate(s->D, gate, s->cur, 0ull, 0, st);
     gm_launch_sort(s->P, s->D, s->cur, st);
-    gm_launch_nl_build(s->P, s->D, st);
+    gm_launch_nl_build(s->P, s->D, st, &s->fk);
 }
 
 // Make the NL usable for a force evaluation at the current time level, outside the graphs.
@@ -801,7 +811,7 @@ static gm_status capture_graph(gm_system *s, int nsteps, cudaGraphExec_t *exec)
                     // the body of a gate-less timestep starts with the gate's bookkeeping (ctl->go, rebuild counter)
                     if (k > 0) gm_launch_gate(s->D, 1, s->cur, 0ull, 0, s->cap_st2);
                     gm_launch_sort(s->P, s->D, s->cur, s->cap_st2);
-                    gm_launch_nl_build(s->P, s->D, s->cap_st2);
+                    gm_launch_nl_build(s->P, s->D, s->cap_st2, &s->fk);
                     cudaGraph_t tmp = nullptr;
                     ok = cudaStreamEndCapture(s->cap_st2, &tmp) == cudaSuccess;
                 }

@@ -156,7 +156,13 @@ enum { GM_MODE_STEP = 0, GM_MODE_FORCES = 1, GM_MODE_ENERGY = 2 };
 void gm_launch_gate(const GmDev &D, int gate, int parity, unsigned long long cond_handle, int use_handle,
                     cudaStream_t st);                                                  // decides, publishes ctl->go
 void gm_launch_sort(const GmParams &P, const GmDev &D, int parity, cudaStream_t st);    // a1 + a2 (if ctl->go)
-void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st);            // a3      (if ctl->go)
+// A side stream and two events (no timing) of one system: work that only the step kernel waits for (the BL remap of systems
+// without tile windows) runs beside the neighbor build -- as a parallel branch when the launches are being captured
+struct GmFork {
+    cudaStream_t side;
+    cudaEvent_t fork, join;
+};
+void gm_launch_nl_build(const GmParams &P, const GmDev &D, cudaStream_t st, const GmFork *fk = nullptr);   // a3 (if ctl->go)
 int gm_nl_capacity_ok(const GmParams &P);
 int gm_nl_smem_bytes(const GmParams &P);
 cudaError_t gm_nl_prepare(const GmParams &P);      // opt-in shared-memory sizes of the kernels that stage windows
